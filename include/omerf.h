@@ -1,0 +1,116 @@
+/*
+ * omerf.h — C-ABI of the B200-native Oblique-MERF renderer (arxiv 2404.09531).
+ *
+ * The boundary follows the paper's problem statement: baked assets + camera -> image
+ * (PAPER.md:186-188 sec. 4.4, :79-81 Eq. 4) and BASELINE.json:north_star's entry points.
+ * Plain pointers and sizes only; every pointer is marked HOST or DEVICE.  All work
+ * (layout, pyramid, ray generation, marching, gathers, compositing, MLP) runs in
+ * hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * Conventions:
+ *   world box [0,X]x[0,Y]x[0,Z], z up.  Host arrays are C-contiguous, first
+ *   named axis slowest, channel last.  Channel 0 = density, 1..3 = diffuse RGB,
+ *   4..7 = specular features (Eq. 3).
+ *   Pixel (u,v): row v = 0 is the TOP row, centre (u+0.5, v+0.5); the ray through it is
+ *   normalize(fwd + ((u+0.5-cx)/fx) right - ((v+0.5-cy)/fy) up); right/up/fwd orthonormal.
+ *
+ * Errors: every int-returning call returns OMERF_OK (0) or a negative code and never throws or
+ * aborts; omerf_last_error() gives a thread-local message for the last failure.
+ */
+#ifndef OMERF_H
+#define OMERF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OMERF_OK 0
+#define OMERF_ERR_INVALID (-1) /* null pointer, non-positive size, step <= 0, t_stop not in (0,1), mlp shape */
+#define OMERF_ERR_NOMEM (-2)   /* out of device memory */
+#define OMERF_ERR_CUDA (-3)    /* any other CUDA failure (message in omerf_last_error) */
+
+#define OMERF_SAMPLER_PLANE 0 /* occupancy-plane march — the method */
+#define OMERF_SAMPLER_GRID 1  /* binary occupancy-grid DDA (the structure PAPER.md:188 replaces; BASELINE.json configs[4]) */
+
+typedef struct omerf_scene omerf_scene; /* opaque; owns all device memory of one baked scene */
+
+/* Baked scene on the HOST.  omerf_scene_create deep-copies everything. */
+typedef struct {
+    float box[3];      /* X, Y, Z */
+    int32_t hf_n[2];   /* Mx, My: grid points of the occupancy plane P_o; vertex-centred, spacing X/(Mx-1) */
+    const float *h_lo; /* HOST [Mx][My] z_min */
+    const float *h_up; /* HOST [Mx][My] z_max; h_up < h_lo marks an empty column */
+    int32_t grid_n[3]; /* Gx, Gy, Gz */
+    const uint8_t *grid; /* HOST [Gx][Gy][Gz][8] low-res voxel grid V */
+    int32_t xy_n[2], xz_n[2], yz_n[2];
+    const uint8_t *plane_xy; /* HOST [Ax][Ay][8], sampled with (x,y) */
+    const uint8_t *plane_xz; /* HOST [Ax][Az][8], sampled with (x,z) */
+    const uint8_t *plane_yz; /* HOST [Ay][Az][8], sampled with (y,z) */
+    float deq_scale, deq_bias; /* pre-activation of one source = u8*deq_scale + deq_bias (28/255, -14) */
+    int32_t mlp_in, mlp_hidden; /* must be 34 and 16: G is 34 -> 16 -> 16 -> 3 (Eq. 4) */
+    const float *W0, *b0, *W1, *b1, *W2, *b2; /* HOST, row-major [out][in] */
+    float step;     /* sample spacing delta along the ray (world units) */
+    float t_stop;   /* early-termination transmittance, in (0,1) */
+    float bg[3];    /* background colour */
+    int32_t sampler; /* OMERF_SAMPLER_PLANE or OMERF_SAMPLER_GRID */
+    int32_t occ_n[3]; /* sampler GRID: bitfield resolution (e.g. 2048,2048,256); derived on the device from the slab */
+} omerf_scene_desc;
+
+/* Pinhole camera, world frame. */
+typedef struct {
+    float origin[3], right[3], up[3], fwd[3];
+    float fx, fy, cx, cy; /* pixels */
+} omerf_camera;
+
+typedef struct {
+    uint64_t device_bytes;  /* device memory held by the scene (features + occupancy structures) */
+    int32_t pyramid_levels; /* levels of the min/max pyramid of (h_lo, h_up), level 0 = P_o itself */
+    int32_t sampler;
+    uint64_t occ_bits_set;  /* sampler GRID: number of set voxels of the derived bitfield, else 0 */
+} omerf_scene_info;
+
+/* S0 + S1 (+ S10 derivation): validate, upload, re-lay out for gathers, build the min/max pyramid
+ * ("2D max pooling to obtain multiple low-resolution occupancy planes") and, for
+ * sampler GRID, the occupancy bitfield.  Synchronous; on return the caller may free every host array.
+ * The scene is immutable afterwards. */
+int omerf_scene_create(const omerf_scene_desc *desc /*HOST*/, omerf_scene **out_scene);
+
+/* S2..S9: render n_views images of W x H pixels (PAPER.md:188 marching; Eq. 1-4, 7-8).
+ *   cameras       HOST  [n_views]; read before the call returns
+ *   out_rgb       DEVICE [n_views][H][W][3] float32, 4-byte aligned
+ *   out_nsamples  DEVICE [n_views][H][W] uint32: samples fetched per pixel (Fig. 1)
+ *   stream        cudaStream_t (NULL = default stream)
+ * Asynchronous: kernels are enqueued on `stream`; results are valid once the caller has synchronised
+ * it.  Calls on one scene must be stream-ordered or externally serialised. */
+int omerf_render(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W, int H,
+                 float *out_rgb /*DEVICE*/, uint32_t *out_nsamples /*DEVICE*/, void *stream);
+
+/* Same path with HOST outputs (pinned or pageable): renders into scene-owned device scratch on
+ * `stream`, copies both images back and synchronises the stream before returning. */
+int omerf_render_host(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W,
+                      int H, float *out_rgb /*HOST*/, uint32_t *out_nsamples /*HOST*/, void *stream);
+
+/* Number of kernels of this library the last omerf_render / omerf_render_host on this scene launched. */
+int omerf_last_launch_count(const omerf_scene *scene);
+
+int omerf_scene_get_info(const omerf_scene *scene, omerf_scene_info *out_info /*HOST*/);
+
+/* Test hooks: copy derived structures back to the HOST (synchronous).
+ * level in [0, pyramid_levels): out_min/out_max HOST [nx][ny] float32 with nx = ceil(Mx / 2^level);
+ * *nx, *ny receive the level's size; pass out_min = out_max = NULL to query the size only. */
+int omerf_scene_get_pyramid_level(const omerf_scene *scene, int level, int32_t *nx, int32_t *ny,
+                                  float *out_min /*HOST*/, float *out_max /*HOST*/);
+/* sampler GRID: out_words HOST uint32[(Nx*Ny*Nz+31)/32], bit index ((jx*Ny + jy)*Nz + jz), LSB first. */
+int omerf_scene_get_bitfield(const omerf_scene *scene, uint32_t *out_words /*HOST*/, uint64_t n_words);
+
+void omerf_scene_destroy(omerf_scene *scene); /* NULL is a no-op */
+
+const char *omerf_last_error(void); /* thread-local, static storage; "" if none */
+const char *omerf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OMERF_H */

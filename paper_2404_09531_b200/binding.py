@@ -1,0 +1,239 @@
+"""Thin ctypes binding of include/omerf.h — argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libomerf.so; PyTorch is used for device
+memory and streams.  There is no CPU fallback: a missing library or a missing GPU raises.
+Function names mirror the C-ABI: scene_create / render / render_host / scene_destroy.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libomerf.so")
+
+_f32p = C.POINTER(C.c_float)
+_u8p = C.POINTER(C.c_uint8)
+_u32p = C.POINTER(C.c_uint32)
+
+SAMPLER_PLANE = 0
+SAMPLER_GRID = 1
+
+EXPORTS = (
+    "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_last_launch_count",
+    "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield",
+    "omerf_scene_destroy", "omerf_last_error", "omerf_version",
+)
+
+
+class SceneDesc(C.Structure):
+    _fields_ = [
+        ("box", C.c_float * 3),
+        ("hf_n", C.c_int32 * 2), ("h_lo", _f32p), ("h_up", _f32p),
+        ("grid_n", C.c_int32 * 3), ("grid", _u8p),
+        ("xy_n", C.c_int32 * 2), ("xz_n", C.c_int32 * 2), ("yz_n", C.c_int32 * 2),
+        ("plane_xy", _u8p), ("plane_xz", _u8p), ("plane_yz", _u8p),
+        ("deq_scale", C.c_float), ("deq_bias", C.c_float),
+        ("mlp_in", C.c_int32), ("mlp_hidden", C.c_int32),
+        ("W0", _f32p), ("b0", _f32p), ("W1", _f32p), ("b1", _f32p), ("W2", _f32p), ("b2", _f32p),
+        ("step", C.c_float), ("t_stop", C.c_float), ("bg", C.c_float * 3),
+        ("sampler", C.c_int32), ("occ_n", C.c_int32 * 3),
+    ]
+
+
+class SceneInfo(C.Structure):
+    _fields_ = [("device_bytes", C.c_uint64), ("pyramid_levels", C.c_int32), ("sampler", C.c_int32),
+                ("occ_bits_set", C.c_uint64)]
+
+
+class OmerfError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libomerf.so (built in-tree by paper_2404_09531_b200.build).  Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise OmerfError(f"{LIB_PATH} not found: build it with `python -m paper_2404_09531_b200.build` "
+                         "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    L.omerf_last_error.restype = C.c_char_p
+    L.omerf_version.restype = C.c_char_p
+    L.omerf_scene_create.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
+    L.omerf_render.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.omerf_render_host.argtypes = L.omerf_render.argtypes
+    L.omerf_last_launch_count.argtypes = [C.c_void_p]
+    L.omerf_scene_get_info.argtypes = [C.c_void_p, C.POINTER(SceneInfo)]
+    L.omerf_scene_get_pyramid_level.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                                                C.c_void_p, C.c_void_p]
+    L.omerf_scene_get_bitfield.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
+    L.omerf_scene_destroy.argtypes = [C.c_void_p]
+    L.omerf_scene_destroy.restype = None
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise OmerfError(f"{what} failed ({rc}): {load_library().omerf_last_error().decode()}")
+
+
+def _np(a, dt):
+    return np.ascontiguousarray(a, dtype=dt)
+
+
+def make_desc(scene, sampler: int = SAMPLER_PLANE):
+    """Fill an omerf_scene_desc from an object with synth.Scene's attributes. Returns (desc, keepalive)."""
+    d = SceneDesc()
+    keep = []
+
+    def arr(a, dt, pt):
+        a = _np(a, dt)
+        keep.append(a)
+        return a, a.ctypes.data_as(pt)
+
+    d.box[:] = scene.box
+    lo, d.h_lo = arr(scene.h_lo, np.float32, _f32p)
+    _, d.h_up = arr(scene.h_up, np.float32, _f32p)
+    d.hf_n[:] = lo.shape
+    g, d.grid = arr(scene.grid, np.uint8, _u8p)
+    d.grid_n[:] = g.shape[:3]
+    for nm in ("xy", "xz", "yz"):
+        p, ptr = arr(getattr(scene, "plane_" + nm), np.uint8, _u8p)
+        getattr(d, nm + "_n")[:] = p.shape[:2]
+        setattr(d, "plane_" + nm, ptr)
+    d.deq_scale, d.deq_bias = scene.deq_scale, scene.deq_bias
+    W0 = _np(scene.W0, np.float32)
+    d.mlp_in, d.mlp_hidden = W0.shape[1], W0.shape[0]
+    for nm in ("W0", "b0", "W1", "b1", "W2", "b2"):
+        _, ptr = arr(getattr(scene, nm), np.float32, _f32p)
+        setattr(d, nm, ptr)
+    d.step, d.t_stop = scene.step, scene.t_stop
+    d.bg[:] = scene.bg
+    d.sampler = sampler
+    d.occ_n[:] = scene.occ_n
+    return d, keep
+
+
+class SceneHandle:
+    """Owns one omerf_scene*.  Use scene_create(); free with scene_destroy() or as a context manager."""
+
+    def __init__(self, ptr):
+        self.ptr = ptr
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        scene_destroy(self)
+
+    def __del__(self):
+        try:
+            scene_destroy(self)
+        except Exception:
+            pass
+
+
+def scene_create(scene, sampler: int = SAMPLER_PLANE) -> SceneHandle:
+    """omerf_scene_create: upload + re-layout + pyramid (+ bitfield) on the current CUDA device."""
+    import torch
+    if not torch.cuda.is_available():
+        raise OmerfError("no CUDA device: the renderer has no CPU fallback")
+    torch.cuda.init()
+    torch.cuda.current_stream()          # make sure torch's primary context is current
+    L = load_library()
+    d, keep = make_desc(scene, sampler)
+    out = C.c_void_p()
+    _check(L.omerf_scene_create(C.byref(d), C.byref(out)), "omerf_scene_create")
+    del keep
+    return SceneHandle(out)
+
+
+def scene_destroy(h: SceneHandle):
+    if h is not None and h.ptr:
+        load_library().omerf_scene_destroy(h.ptr)
+        h.ptr = None
+
+
+def _cams(cameras):
+    cams = _np(np.atleast_2d(cameras), np.float32)
+    assert cams.shape[1] == 16, "camera rows are origin,right,up,fwd,fx,fy,cx,cy (16 floats)"
+    return cams
+
+
+def render(h: SceneHandle, cameras, W: int, H: int, out_rgb=None, out_nsamples=None, stream=None):
+    """omerf_render: enqueue on `stream` (default: torch's current stream); DEVICE outputs (torch tensors).
+    Returns (out_rgb float32 [n][H][W][3], out_nsamples int32-viewed uint32 [n][H][W]); asynchronous."""
+    import torch
+    cams = _cams(cameras)
+    n = cams.shape[0]
+    if out_rgb is None:
+        out_rgb = torch.empty((n, H, W, 3), dtype=torch.float32, device="cuda")
+    if out_nsamples is None:
+        out_nsamples = torch.empty((n, H, W), dtype=torch.int32, device="cuda")
+    assert out_rgb.is_cuda and out_rgb.is_contiguous() and out_rgb.dtype == torch.float32 and out_rgb.numel() == n * H * W * 3
+    assert out_nsamples.is_cuda and out_nsamples.is_contiguous() and out_nsamples.element_size() == 4 \
+        and out_nsamples.numel() == n * H * W
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(load_library().omerf_render(h.ptr, cams.ctypes.data, n, W, H, out_rgb.data_ptr(), out_nsamples.data_ptr(),
+                                       st.cuda_stream), "omerf_render")
+    return out_rgb, out_nsamples
+
+
+def render_host(h: SceneHandle, cameras, W: int, H: int, out_rgb=None, out_nsamples=None, stream=None):
+    """omerf_render_host: HOST outputs (numpy arrays or pinned CPU torch tensors); synchronous."""
+    import torch
+    cams = _cams(cameras)
+    n = cams.shape[0]
+    if out_rgb is None:
+        out_rgb = np.empty((n, H, W, 3), dtype=np.float32)
+    if out_nsamples is None:
+        out_nsamples = np.empty((n, H, W), dtype=np.uint32)
+
+    def hptr(a, nbytes):
+        if isinstance(a, np.ndarray):
+            assert a.flags["C_CONTIGUOUS"] and a.nbytes == nbytes
+            return a.ctypes.data
+        assert (not a.is_cuda) and a.is_contiguous() and a.numel() * a.element_size() == nbytes
+        return a.data_ptr()
+
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(load_library().omerf_render_host(h.ptr, cams.ctypes.data, n, W, H, hptr(out_rgb, n * H * W * 12),
+                                            hptr(out_nsamples, n * H * W * 4), st.cuda_stream), "omerf_render_host")
+    return out_rgb, out_nsamples
+
+
+def last_launch_count(h: SceneHandle) -> int:
+    return int(load_library().omerf_last_launch_count(h.ptr))
+
+
+def scene_info(h: SceneHandle) -> dict:
+    info = SceneInfo()
+    _check(load_library().omerf_scene_get_info(h.ptr, C.byref(info)), "omerf_scene_get_info")
+    return {"device_bytes": int(info.device_bytes), "pyramid_levels": int(info.pyramid_levels),
+            "sampler": int(info.sampler), "occ_bits_set": int(info.occ_bits_set)}
+
+
+def pyramid_level(h: SceneHandle, level: int):
+    L = load_library()
+    nx, ny = C.c_int32(), C.c_int32()
+    _check(L.omerf_scene_get_pyramid_level(h.ptr, level, C.byref(nx), C.byref(ny), None, None), "get_pyramid_level")
+    mn = np.empty((nx.value, ny.value), dtype=np.float32)
+    mx = np.empty_like(mn)
+    _check(L.omerf_scene_get_pyramid_level(h.ptr, level, C.byref(nx), C.byref(ny), mn.ctypes.data, mx.ctypes.data),
+           "get_pyramid_level")
+    return mn, mx
+
+
+def bitfield(h: SceneHandle, occ_n) -> np.ndarray:
+    n = (int(np.prod(occ_n)) + 31) // 32
+    out = np.empty(n, dtype=np.uint32)
+    _check(load_library().omerf_scene_get_bitfield(h.ptr, out.ctypes.data, n), "get_bitfield")
+    return out

@@ -1,0 +1,314 @@
+// omerf_api.cu — host side of the C-ABI (include/omerf.h): validation, upload, ownership, errors.
+// No rendering arithmetic lives here; every step of the path runs in the kernels of
+// omerf_build.cu (S0/S1/S10 derivations) and omerf_render.cu (S2..S9).
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "omerf_device.cuh"
+
+static thread_local char g_err[512] = "";
+
+void omerf_set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+int omerf_cuda_fail(cudaError_t e, const char *what)
+{
+    omerf_set_error("CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
+    cudaGetLastError(); // clear the sticky-less error state
+    return e == cudaErrorMemoryAllocation ? OMERF_ERR_NOMEM : OMERF_ERR_CUDA;
+}
+
+extern "C" const char *omerf_last_error(void) { return g_err; }
+extern "C" const char *omerf_version(void) { return "omerf-b200 0.1 (sm_100a)"; }
+
+static int invalid(const char *msg)
+{
+    omerf_set_error("invalid argument: %s", msg);
+    return OMERF_ERR_INVALID;
+}
+
+static int upload(void **dptr, const void *host, size_t bytes, uint64_t *total)
+{
+    OMERF_CUDA(cudaMalloc(dptr, bytes));
+    OMERF_CUDA(cudaMemcpy(*dptr, host, bytes, cudaMemcpyHostToDevice));
+    *total += bytes;
+    return OMERF_OK;
+}
+
+static void free_scene(omerf_scene *s)
+{
+    if (!s) return;
+    cudaFree(s->d_pyr);
+    cudaFree(s->d_grid);
+    cudaFree(s->d_pxy);
+    cudaFree(s->d_pxz);
+    cudaFree(s->d_pyz);
+    cudaFree(s->d_occ);
+    cudaFree(s->d_cams);
+    cudaFree(s->d_scratch_rgb);
+    cudaFree(s->d_scratch_n);
+    if (s->h_cams) cudaFreeHost(s->h_cams);
+    if (s->slot_event) {
+        for (int i = 0; i < OMERF_CAM_SLOTS; i++)
+            if (s->slot_event[i]) cudaEventDestroy(s->slot_event[i]);
+        delete[] s->slot_event;
+    }
+    delete s;
+}
+
+extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_scene)
+{
+    g_err[0] = 0;
+    if (!d || !out_scene) return invalid("null desc/out_scene");
+    *out_scene = nullptr;
+    if (!(d->box[0] > 0 && d->box[1] > 0 && d->box[2] > 0)) return invalid("box must be positive");
+    if (d->hf_n[0] < 2 || d->hf_n[1] < 2) return invalid("hf_n must be >= 2");
+    if (!d->h_lo || !d->h_up) return invalid("null height field");
+    for (int i = 0; i < 3; i++)
+        if (d->grid_n[i] < 1) return invalid("grid_n must be >= 1");
+    for (int i = 0; i < 2; i++)
+        if (d->xy_n[i] < 1 || d->xz_n[i] < 1 || d->yz_n[i] < 1) return invalid("plane sizes must be >= 1");
+    if (!d->grid || !d->plane_xy || !d->plane_xz || !d->plane_yz) return invalid("null feature array");
+    if (d->mlp_in != OMERF_MLP_IN || d->mlp_hidden != OMERF_MLP_HID) return invalid("MLP must be 34 -> 16 -> 16 -> 3");
+    if (!d->W0 || !d->b0 || !d->W1 || !d->b1 || !d->W2 || !d->b2) return invalid("null MLP array");
+    if (!(d->step > 0) || !isfinite(d->step)) return invalid("step must be > 0");
+    if (!(d->t_stop > 0 && d->t_stop < 1)) return invalid("t_stop must be in (0,1)");
+    if (d->sampler != OMERF_SAMPLER_PLANE && d->sampler != OMERF_SAMPLER_GRID) return invalid("unknown sampler");
+    if (d->sampler == OMERF_SAMPLER_GRID)
+        for (int i = 0; i < 3; i++)
+            if (d->occ_n[i] < 1) return invalid("occ_n must be >= 1 for the grid sampler");
+
+    omerf_scene *s = new (std::nothrow) omerf_scene();
+    if (!s) {
+        omerf_set_error("host allocation failed");
+        return OMERF_ERR_NOMEM;
+    }
+    memset(s, 0, sizeof *s);
+    if (cudaGetDevice(&s->device) != cudaSuccess) {
+        int rc = omerf_cuda_fail(cudaGetLastError(), "cudaGetDevice (no CUDA device: there is no CPU fallback)");
+        delete s;
+        return rc;
+    }
+    DevScene &v = s->dev;
+    for (int i = 0; i < 3; i++) v.box[i] = d->box[i];
+    v.Mx = d->hf_n[0];
+    v.My = d->hf_n[1];
+    v.sx = (float)(v.Mx - 1) / d->box[0];
+    v.sy = (float)(v.My - 1) / d->box[1];
+    v.cell_x = d->box[0] / (float)(v.Mx - 1);
+    v.cell_y = d->box[1] / (float)(v.My - 1);
+    for (int i = 0; i < 3; i++) {
+        v.G[i] = d->grid_n[i];
+        v.gs[i] = (float)d->grid_n[i] / d->box[i];
+    }
+    const int ax[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+    const int32_t *pn[3] = {d->xy_n, d->xz_n, d->yz_n};
+    int *vn[3] = {v.xy_n, v.xz_n, v.yz_n};
+    float *vs[3] = {v.xy_s, v.xz_s, v.yz_s};
+    for (int p = 0; p < 3; p++)
+        for (int i = 0; i < 2; i++) {
+            vn[p][i] = pn[p][i];
+            vs[p][i] = (float)pn[p][i] / d->box[ax[p][i]];
+        }
+    v.deq_mul = d->deq_scale / 65536.0f;
+    v.deq_add = 4.0f * d->deq_bias;
+    v.step = d->step;
+    v.inv_step = 1.0f / d->step;
+    v.q_stop = (uint32_t)ceil(-log((double)d->t_stop) * 1048576.0);
+    for (int i = 0; i < 3; i++) v.bg[i] = d->bg[i];
+    v.sampler = d->sampler;
+    memcpy(v.W0, d->W0, sizeof v.W0);
+    memcpy(v.b0, d->b0, sizeof v.b0);
+    memcpy(v.W1, d->W1, sizeof v.W1);
+    memcpy(v.b1, d->b1, sizeof v.b1);
+    memcpy(v.W2, d->W2, sizeof v.W2);
+    memcpy(v.b2, d->b2, sizeof v.b2);
+
+    int rc = OMERF_OK;
+    float *d_lo = nullptr, *d_up = nullptr;
+    uint64_t tmp = 0;
+    size_t hf_bytes = (size_t)v.Mx * v.My * sizeof(float);
+    do {
+        // S0: features.  8 channels per texel -> one 8-byte word; row-major order kept.
+        if ((rc = upload(&s->d_grid, d->grid, (size_t)v.G[0] * v.G[1] * v.G[2] * 8, &s->device_bytes))) break;
+        if ((rc = upload(&s->d_pxy, d->plane_xy, (size_t)v.xy_n[0] * v.xy_n[1] * 8, &s->device_bytes))) break;
+        if ((rc = upload(&s->d_pxz, d->plane_xz, (size_t)v.xz_n[0] * v.xz_n[1] * 8, &s->device_bytes))) break;
+        if ((rc = upload(&s->d_pyz, d->plane_yz, (size_t)v.yz_n[0] * v.yz_n[1] * 8, &s->device_bytes))) break;
+        v.grid = (const uint2 *)s->d_grid;
+        v.pxy = (const uint2 *)s->d_pxy;
+        v.pxz = (const uint2 *)s->d_pxz;
+        v.pyz = (const uint2 *)s->d_pyz;
+        // S1: min/max pyramid of the two height fields, built on the device
+        if ((rc = upload((void **)&d_lo, d->h_lo, hf_bytes, &tmp))) break;
+        if ((rc = upload((void **)&d_up, d->h_up, hf_bytes, &tmp))) break;
+        if ((rc = omerf_launch_pyramid(s, d_lo, d_up, 0))) break;
+        // S10: occupancy bitfield + its mip chain, derived on the device from the slab
+        if (d->sampler == OMERF_SAMPLER_GRID) {
+            for (int i = 0; i < 3; i++) {
+                v.N[i] = d->occ_n[i];
+                v.ns[i] = (float)d->occ_n[i] / d->box[i];
+            }
+            if ((rc = omerf_launch_bitfield(s, 0))) break;
+        }
+        cudaError_t e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) {
+            rc = omerf_cuda_fail(e, "scene build");
+            break;
+        }
+        // camera staging ring
+        s->cam_capacity = 0;
+        s->slot_event = new (std::nothrow) cudaEvent_t[OMERF_CAM_SLOTS]();
+        if (!s->slot_event) {
+            omerf_set_error("host allocation failed");
+            rc = OMERF_ERR_NOMEM;
+            break;
+        }
+        for (int i = 0; i < OMERF_CAM_SLOTS && rc == OMERF_OK; i++) {
+            cudaError_t ee = cudaEventCreateWithFlags(&s->slot_event[i], cudaEventDisableTiming);
+            if (ee != cudaSuccess) rc = omerf_cuda_fail(ee, "cudaEventCreate");
+        }
+    } while (0);
+    cudaFree(d_lo);
+    cudaFree(d_up);
+    if (rc != OMERF_OK) {
+        free_scene(s);
+        return rc;
+    }
+    *out_scene = s;
+    return OMERF_OK;
+}
+
+extern "C" void omerf_scene_destroy(omerf_scene *s)
+{
+    if (!s) return;
+    cudaDeviceSynchronize();
+    free_scene(s);
+}
+
+static int ensure_cams(const omerf_scene *s, int n_views)
+{
+    if (n_views <= s->cam_capacity) return OMERF_OK;
+    cudaDeviceSynchronize();
+    cudaFree(s->d_cams);
+    if (s->h_cams) cudaFreeHost(s->h_cams);
+    s->d_cams = nullptr;
+    s->h_cams = nullptr;
+    s->cam_capacity = 0;
+    int cap = n_views < 16 ? 16 : n_views;
+    size_t bytes = (size_t)cap * OMERF_CAM_SLOTS * sizeof(omerf_camera);
+    OMERF_CUDA(cudaMalloc((void **)&s->d_cams, bytes));
+    OMERF_CUDA(cudaMallocHost((void **)&s->h_cams, bytes));
+    s->cam_capacity = cap;
+    return OMERF_OK;
+}
+
+extern "C" int omerf_render(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
+                            float *out_rgb, uint32_t *out_nsamples, void *stream)
+{
+    if (!s || !cameras || !out_rgb || !out_nsamples) return invalid("null scene/cameras/output");
+    if (n_views < 0 || W <= 0 || H <= 0) return invalid("n_views >= 0, W > 0, H > 0 required");
+    if (((uintptr_t)out_rgb & 3) || ((uintptr_t)out_nsamples & 3)) return invalid("misaligned output");
+    s->last_launches = 0;
+    if (n_views == 0) return OMERF_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ensure_cams(s, n_views);
+    if (rc) return rc;
+    // stage the cameras: user memory -> pinned ring slot -> device ring slot (stream-ordered)
+    int slot = (int)(s->call_index++ % OMERF_CAM_SLOTS);
+    OMERF_CUDA(cudaEventSynchronize(s->slot_event[slot]));
+    omerf_camera *h = s->h_cams + (size_t)slot * s->cam_capacity;
+    omerf_camera *dv = s->d_cams + (size_t)slot * s->cam_capacity;
+    memcpy(h, cameras, (size_t)n_views * sizeof(omerf_camera));
+    OMERF_CUDA(cudaMemcpyAsync(dv, h, (size_t)n_views * sizeof(omerf_camera), cudaMemcpyHostToDevice, st));
+    OMERF_CUDA(cudaEventRecord(s->slot_event[slot], st));
+    int launches = 0;
+    rc = omerf_launch_render(s, dv, n_views, W, H, out_rgb, out_nsamples, st, &launches);
+    s->last_launches = launches;
+    return rc;
+}
+
+extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
+                                 float *out_rgb, uint32_t *out_nsamples, void *stream)
+{
+    if (!s || !cameras || !out_rgb || !out_nsamples) return invalid("null scene/cameras/output");
+    if (n_views < 0 || W <= 0 || H <= 0) return invalid("n_views >= 0, W > 0, H > 0 required");
+    if (n_views == 0) return OMERF_OK;
+    uint64_t px = (uint64_t)n_views * W * H;
+    if (px > s->scratch_pixels) {
+        cudaDeviceSynchronize();
+        cudaFree(s->d_scratch_rgb);
+        cudaFree(s->d_scratch_n);
+        s->d_scratch_rgb = nullptr;
+        s->d_scratch_n = nullptr;
+        s->scratch_pixels = 0;
+        OMERF_CUDA(cudaMalloc((void **)&s->d_scratch_rgb, px * 3 * sizeof(float)));
+        OMERF_CUDA(cudaMalloc((void **)&s->d_scratch_n, px * sizeof(uint32_t)));
+        s->scratch_pixels = px;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = omerf_render(s, cameras, n_views, W, H, s->d_scratch_rgb, s->d_scratch_n, stream);
+    if (rc) return rc;
+    OMERF_CUDA(cudaMemcpyAsync(out_rgb, s->d_scratch_rgb, px * 3 * sizeof(float), cudaMemcpyDeviceToHost, st));
+    OMERF_CUDA(cudaMemcpyAsync(out_nsamples, s->d_scratch_n, px * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    OMERF_CUDA(cudaStreamSynchronize(st));
+    return OMERF_OK;
+}
+
+extern "C" int omerf_last_launch_count(const omerf_scene *s) { return s ? s->last_launches : 0; }
+
+extern "C" int omerf_scene_get_info(const omerf_scene *s, omerf_scene_info *out)
+{
+    if (!s || !out) return invalid("null scene/out_info");
+    out->device_bytes = s->device_bytes;
+    out->pyramid_levels = s->dev.n_levels;
+    out->sampler = s->dev.sampler;
+    out->occ_bits_set = s->occ_bits_set;
+    return OMERF_OK;
+}
+
+extern "C" int omerf_scene_get_pyramid_level(const omerf_scene *s, int level, int32_t *nx, int32_t *ny,
+                                             float *out_min, float *out_max)
+{
+    if (!s || !nx || !ny) return invalid("null scene/nx/ny");
+    if (level < 0 || level >= s->dev.n_levels) return invalid("pyramid level out of range");
+    *nx = s->dev.lvl_nx[level];
+    *ny = s->dev.lvl_ny[level];
+    if (!out_min && !out_max) return OMERF_OK;
+    if (!out_min || !out_max) return invalid("out_min and out_max must both be given");
+    size_t n = (size_t)*nx * *ny;
+    float2 *tmp = new (std::nothrow) float2[n];
+    if (!tmp) {
+        omerf_set_error("host allocation failed");
+        return OMERF_ERR_NOMEM;
+    }
+    cudaError_t e = cudaMemcpy(tmp, s->dev.pyr + s->dev.lvl_off[level], n * sizeof(float2), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) {
+        delete[] tmp;
+        return omerf_cuda_fail(e, "cudaMemcpy pyramid");
+    }
+    for (size_t i = 0; i < n; i++) {
+        out_min[i] = tmp[i].x;
+        out_max[i] = tmp[i].y;
+    }
+    delete[] tmp;
+    return OMERF_OK;
+}
+
+extern "C" int omerf_scene_get_bitfield(const omerf_scene *s, uint32_t *out_words, uint64_t n_words)
+{
+    if (!s || !out_words) return invalid("null scene/out_words");
+    if (s->dev.sampler != OMERF_SAMPLER_GRID) return invalid("scene has no bitfield (sampler is not GRID)");
+    uint64_t need = ((uint64_t)s->dev.N[0] * s->dev.N[1] * s->dev.N[2] + 31) / 32;
+    if (n_words != need) return invalid("n_words does not match (Nx*Ny*Nz+31)/32");
+    OMERF_CUDA(cudaMemcpy(out_words, s->dev.occ, need * 4, cudaMemcpyDeviceToHost));
+    return OMERF_OK;
+}

@@ -1,0 +1,205 @@
+// omerf_build.cu — one-time scene derivations on the device.
+//   S1  min/max pyramid of the occupancy plane: "2D max pooling to obtain multiple low-resolution
+//       occupancy planes"; we min-pool z_min and max-pool z_max (R16).
+//   S10 config-4 comparator: binary occupancy grid derived from the slab (voxel set iff it intersects
+//       [z_min, z_max] of an overlapping cell, R18) and its OR-reduced mip chain — the
+//       "multi-resolution binary grid" PAPER.md:188 says the occupancy plane replaces.
+#include "omerf_device.cuh"
+
+// ------------------------------------------------------------------------------------------ pyramid
+__global__ void pyr_level0_kernel(const float *__restrict__ lo, const float *__restrict__ up,
+                                  float2 *__restrict__ out, int n)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = make_float2(lo[i], up[i]);
+}
+
+__global__ void pyr_reduce_kernel(const float2 *__restrict__ src, int snx, int sny, float2 *__restrict__ dst,
+                                  int dnx, int dny)
+{
+    int j = blockIdx.x * blockDim.x + threadIdx.x; // fast axis = y
+    int i = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= dnx || j >= dny) return;
+    float mn = INFINITY, mx = -INFINITY;
+    for (int a = 0; a < 2; a++)
+        for (int b = 0; b < 2; b++) {
+            int si = 2 * i + a, sj = 2 * j + b;
+            if (si < snx && sj < sny) {
+                float2 v = src[(size_t)si * sny + sj];
+                mn = fminf(mn, v.x);
+                mx = fmaxf(mx, v.y);
+            }
+        }
+    dst[(size_t)i * dny + j] = make_float2(mn, mx);
+}
+
+int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, cudaStream_t st)
+{
+    DevScene &v = s->dev;
+    int nx = v.Mx, ny = v.My, L = 0;
+    size_t total = 0;
+    while (true) {
+        v.lvl_nx[L] = nx;
+        v.lvl_ny[L] = ny;
+        v.lvl_off[L] = (int)total;
+        total += (size_t)nx * ny;
+        L++;
+        if ((nx == 1 && ny == 1) || L == OMERF_MAX_LEVELS) break;
+        nx = (nx + 1) / 2;
+        ny = (ny + 1) / 2;
+    }
+    if (total > 0x7fffffffull) {
+        omerf_set_error("invalid argument: occupancy plane too large");
+        return OMERF_ERR_INVALID;
+    }
+    v.n_levels = L;
+    OMERF_CUDA(cudaMalloc(&s->d_pyr, total * sizeof(float2)));
+    s->device_bytes += total * sizeof(float2);
+    v.pyr = (const float2 *)s->d_pyr;
+    float2 *pyr = (float2 *)s->d_pyr;
+    int n0 = v.Mx * v.My;
+    pyr_level0_kernel<<<(n0 + 255) / 256, 256, 0, st>>>(d_lo, d_up, pyr, n0);
+    for (int l = 1; l < L; l++) {
+        dim3 blk(32, 8), grd((v.lvl_ny[l] + 31) / 32, (v.lvl_nx[l] + 7) / 8);
+        pyr_reduce_kernel<<<grd, blk, 0, st>>>(pyr + v.lvl_off[l - 1], v.lvl_nx[l - 1], v.lvl_ny[l - 1],
+                                               pyr + v.lvl_off[l], v.lvl_nx[l], v.lvl_ny[l]);
+    }
+    OMERF_CUDA(cudaGetLastError());
+    return OMERF_OK;
+}
+
+// ------------------------------------------------------------------------------------------ bitfield
+// Cell i overlaps voxel j along one axis with positive length iff (exact integers)
+//   2 j (M-1) < (2i+1) N   and   (2i-1) N < 2 (j+1) (M-1)
+__device__ __forceinline__ void cell_range(int j, int N, int M, int *i0, int *i1)
+{
+    long long a = 2ll * j * (M - 1), e = 2ll * (j + 1) * (M - 1);
+    // smallest i with (2i+1) N > a  <=>  i > (a/N - 1)/2
+    long long lo = (a / N - 1) / 2 - 1;
+    if (lo < 0) lo = 0;
+    while (lo < M - 1 && !((2 * lo + 1) * N > a)) lo++;
+    long long hi = lo;
+    while (hi + 1 <= M - 1 && (2 * (hi + 1) - 1) * N < e) hi++;
+    *i0 = (int)lo;
+    *i1 = ((2 * lo + 1) * N > a && (2 * lo - 1) * N < e) ? (int)hi : (int)lo - 1;
+}
+
+__global__ void occ_level0_kernel(DevScene sc, uint32_t *__restrict__ out, unsigned long long n_words,
+                                  unsigned long long n_bits)
+{
+    unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_words) return;
+    const int Nx = sc.N[0], Ny = sc.N[1], Nz = sc.N[2];
+    const double Z = (double)sc.box[2];
+    uint32_t word = 0;
+    int cjx = -1, cjy = -1, x0 = 0, x1 = -1, y0 = 0, y1 = -1;
+    for (int b = 0; b < 32; b++) {
+        unsigned long long idx = w * 32 + b;
+        if (idx >= n_bits) break;
+        int jz = (int)(idx % Nz);
+        unsigned long long col = idx / Nz;
+        int jy = (int)(col % Ny), jx = (int)(col / Ny);
+        if (jx != cjx) {
+            cell_range(jx, Nx, sc.Mx, &x0, &x1);
+            cjx = jx;
+        }
+        if (jy != cjy) {
+            cell_range(jy, Ny, sc.My, &y0, &y1);
+            cjy = jy;
+        }
+        double zl = __ddiv_rn(__dmul_rn((double)jz, Z), (double)Nz);
+        double zh = __ddiv_rn(__dmul_rn((double)(jz + 1), Z), (double)Nz);
+        bool set = false;
+        for (int ix = x0; ix <= x1 && !set; ix++)
+            for (int iy = y0; iy <= y1 && !set; iy++) {
+                float2 h = sc.pyr[(size_t)ix * sc.My + iy]; // level 0 = the field itself
+                double lo = (double)h.x, hi = (double)h.y;
+                if (lo <= hi && zl <= hi && zh >= lo) set = true;
+            }
+        if (set) word |= 1u << b;
+    }
+    out[w] = word;
+}
+
+__device__ __forceinline__ bool occ_bit(const uint32_t *bits, int ny, int nz, int jx, int jy, int jz)
+{
+    unsigned long long idx = ((unsigned long long)jx * ny + jy) * nz + jz;
+    return (bits[idx >> 5] >> (idx & 31)) & 1u;
+}
+
+__global__ void occ_reduce_kernel(const uint32_t *__restrict__ src, int snx, int sny, int snz,
+                                  uint32_t *__restrict__ dst, int dnx, int dny, int dnz,
+                                  unsigned long long n_words, unsigned long long n_bits)
+{
+    unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_words) return;
+    uint32_t word = 0;
+    for (int b = 0; b < 32; b++) {
+        unsigned long long idx = w * 32 + b;
+        if (idx >= n_bits) break;
+        int jz = (int)(idx % dnz);
+        unsigned long long col = idx / dnz;
+        int jy = (int)(col % dny), jx = (int)(col / dny);
+        bool set = false;
+        for (int a = 0; a < 2 && !set; a++)
+            for (int c = 0; c < 2 && !set; c++)
+                for (int e = 0; e < 2 && !set; e++) {
+                    int x = 2 * jx + a, y = 2 * jy + c, z = 2 * jz + e;
+                    if (x < snx && y < sny && z < snz) set = occ_bit(src, sny, snz, x, y, z);
+                }
+        if (set) word |= 1u << b;
+    }
+    dst[w] = word;
+}
+
+__global__ void popcount_kernel(const uint32_t *__restrict__ words, unsigned long long n_words,
+                                unsigned long long *__restrict__ total)
+{
+    unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    unsigned long long acc = 0;
+    for (; i < n_words; i += stride) acc += __popc(words[i]);
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0 && acc) atomicAdd(total, acc);
+}
+
+int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st)
+{
+    DevScene &v = s->dev;
+    int nx = v.N[0], ny = v.N[1], nz = v.N[2], L = 0;
+    unsigned long long total_words = 0;
+    while (true) {
+        v.occ_nx[L] = nx;
+        v.occ_ny[L] = ny;
+        v.occ_nz[L] = nz;
+        v.occ_off[L] = total_words;
+        total_words += ((unsigned long long)nx * ny * nz + 31) / 32;
+        L++;
+        if ((nx == 1 && ny == 1 && nz == 1) || L == OMERF_MAX_LEVELS) break;
+        nx = (nx + 1) / 2;
+        ny = (ny + 1) / 2;
+        nz = (nz + 1) / 2;
+    }
+    v.occ_levels = L;
+    OMERF_CUDA(cudaMalloc(&s->d_occ, total_words * 4 + 16));
+    s->device_bytes += total_words * 4;
+    v.occ = (const uint32_t *)s->d_occ;
+    uint32_t *occ = (uint32_t *)s->d_occ;
+    unsigned long long *d_total = (unsigned long long *)(occ + total_words + (total_words & 1));
+    OMERF_CUDA(cudaMemsetAsync(d_total, 0, 8, st));
+    unsigned long long bits0 = (unsigned long long)v.N[0] * v.N[1] * v.N[2];
+    unsigned long long words0 = (bits0 + 31) / 32;
+    occ_level0_kernel<<<(unsigned)((words0 + 127) / 128), 128, 0, st>>>(v, occ, words0, bits0);
+    for (int l = 1; l < L; l++) {
+        unsigned long long nb = (unsigned long long)v.occ_nx[l] * v.occ_ny[l] * v.occ_nz[l];
+        unsigned long long nw = (nb + 31) / 32;
+        occ_reduce_kernel<<<(unsigned)((nw + 127) / 128), 128, 0, st>>>(
+            occ + v.occ_off[l - 1], v.occ_nx[l - 1], v.occ_ny[l - 1], v.occ_nz[l - 1], occ + v.occ_off[l],
+            v.occ_nx[l], v.occ_ny[l], v.occ_nz[l], nw, nb);
+    }
+    popcount_kernel<<<1184, 256, 0, st>>>(occ, words0, d_total);
+    OMERF_CUDA(cudaGetLastError());
+    OMERF_CUDA(cudaMemcpyAsync(&s->occ_bits_set, d_total, 8, cudaMemcpyDeviceToHost, st));
+    OMERF_CUDA(cudaStreamSynchronize(st));
+    return OMERF_OK;
+}

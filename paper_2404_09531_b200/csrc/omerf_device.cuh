@@ -1,0 +1,82 @@
+// omerf_device.cuh — device-side scene description shared by the scene-build and render kernels.
+// Internal to the CUDA path (never included by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/omerf.h"
+
+#define OMERF_MAX_LEVELS 16
+#define OMERF_MLP_IN 34
+#define OMERF_MLP_HID 16
+
+// Everything a render kernel needs, passed by value as a __grid_constant__ kernel parameter so that
+// scalars and the 883 MLP weights are read through the constant bank (no loads in the MLP).
+struct DevScene {
+    float box[3];
+    // occupancy plane P_o and its min/max pyramid ("2D max pooling")
+    int Mx, My;
+    float sx, sy;          // (Mx-1)/X, (My-1)/Y in fp32: the predicate's scale (Eq. 7 nearest grid point)
+    float cell_x, cell_y;  // X/(Mx-1): world size of a cell, proposals only
+    int n_levels;
+    const float2 *pyr;     // all levels, (min of h_lo, max of h_up) per node, [nx][ny] row-major
+    int lvl_off[OMERF_MAX_LEVELS], lvl_nx[OMERF_MAX_LEVELS], lvl_ny[OMERF_MAX_LEVELS];
+    // features: 8 uint8 channels per texel = one uint2
+    int G[3];
+    float gs[3];           // G/box per axis
+    const uint2 *grid;     // [Gx][Gy][Gz]
+    int xy_n[2], xz_n[2], yz_n[2];
+    float xy_s[2], xz_s[2], yz_s[2];
+    const uint2 *pxy, *pxz, *pyz;
+    float deq_mul, deq_add; // scale/65536, 4*bias
+    float step, inv_step;
+    uint32_t q_stop;
+    float bg[3];
+    // sampler GRID (config-4 comparator): multi-resolution binary occupancy grid
+    int sampler;
+    int N[3];
+    float ns[3];           // N/box per axis
+    int occ_levels;
+    const uint32_t *occ;   // all levels; level l has dims ceil(N/2^l), bit index ((jx*ny+jy)*nz+jz)
+    unsigned long long occ_off[OMERF_MAX_LEVELS]; // word offset of each level
+    int occ_nx[OMERF_MAX_LEVELS], occ_ny[OMERF_MAX_LEVELS], occ_nz[OMERF_MAX_LEVELS];
+    // deferred MLP G (Eq. 4)
+    float W0[OMERF_MLP_HID * OMERF_MLP_IN], b0[OMERF_MLP_HID];
+    float W1[OMERF_MLP_HID * OMERF_MLP_HID], b1[OMERF_MLP_HID];
+    float W2[3 * OMERF_MLP_HID], b2[3];
+};
+
+struct omerf_scene {
+    DevScene dev;
+    int device;
+    void *d_pyr, *d_grid, *d_pxy, *d_pxz, *d_pyz, *d_occ;
+    uint64_t device_bytes;
+    uint64_t occ_bits_set;
+    // per-render state (mutable through the const handle: calls must be stream-ordered)
+    mutable omerf_camera *d_cams;
+    mutable omerf_camera *h_cams;      // pinned staging ring
+    mutable cudaEvent_t *slot_event;
+    mutable int cam_capacity;          // views per slot
+    mutable unsigned long long call_index;
+    mutable float *d_scratch_rgb;
+    mutable uint32_t *d_scratch_n;
+    mutable uint64_t scratch_pixels;
+    mutable int last_launches;
+};
+
+#define OMERF_CAM_SLOTS 16
+
+// error plumbing (omerf_api.cu)
+void omerf_set_error(const char *fmt, ...);
+int omerf_cuda_fail(cudaError_t e, const char *what);
+#define OMERF_CUDA(call)                                                     \
+    do {                                                                     \
+        cudaError_t e__ = (call);                                            \
+        if (e__ != cudaSuccess) return omerf_cuda_fail(e__, #call);          \
+    } while (0)
+
+// kernels' host launchers
+int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, cudaStream_t st);
+int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st);
+int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H,
+                        float *out_rgb, uint32_t *out_n, cudaStream_t st, int *launches);

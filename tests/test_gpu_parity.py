@@ -1,0 +1,200 @@
+"""Parity of the CUDA path against the CPU oracle, through the C-ABI (run on the B200 box: -m gpu).
+
+Bar (BASELINE.json north_star): per-pixel sample counts bit-exact; max |dRGB| <= 2e-3 per channel.
+"""
+import numpy as np
+import pytest
+
+import synth
+
+pytestmark = pytest.mark.gpu
+
+RGB_TOL = 2e-3   # north_star: "max |dRGB| <= 2e-3 per channel on [0,1] for the fp32 colour path"
+
+
+@pytest.fixture(scope="module")
+def omerf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2404_09531_b200 as m
+    m.load_library()
+    return m
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    import oracle as o
+    return o
+
+
+def _gpu_render(omerf, scene, cams, W, H, sampler=0, host=False):
+    import torch
+    with omerf.scene_create(scene, sampler=sampler) as h:
+        if host:
+            rgb, ns = omerf.render_host(h, cams, W, H)
+            launches = omerf.last_launch_count(h)
+            return rgb.astype(np.float64), ns, launches
+        rgb, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        launches = omerf.last_launch_count(h)
+        return rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), launches
+
+
+def _assert_parity(got_rgb, got_n, ref, what=""):
+    bad = got_n != ref["nsamples"]
+    assert not bad.any(), f"{what}: {int(bad.sum())} pixels with wrong sample counts, first at {np.argwhere(bad)[:5].tolist()}"
+    err = np.abs(got_rgb - ref["rgb"]).max()
+    assert err <= RGB_TOL, f"{what}: max |dRGB| = {err}"
+
+
+# ----------------------------------------------------------------------------- config 0 (whole image, brute oracle)
+def test_config0_full_image(omerf, oracle):
+    sc, cams = synth.make_scene(0), synth.make_cameras(0)
+    W, H = synth.config_resolution(0)
+    rgb, ns, launches = _gpu_render(omerf, sc, cams, W, H)
+    ref = oracle.OracleScene(sc).render(cams, W, H, mode="brute")
+    assert launches >= 1
+    assert ref["nsamples"].sum() > 50000
+    _assert_parity(rgb, ns, ref, "config 0")
+
+
+def test_config0_host_buffers_and_ragged_sizes(omerf, oracle):
+    sc = synth.make_scene(0)
+    O = oracle.OracleScene(sc)
+    for (W, H) in [(37, 29), (1, 1), (16, 8), (17, 9), (130, 3)]:
+        cam = synth.look_at_camera((10.0, -14.0, 30.0), (32.0, 32.0, 8.0), W, H)
+        rgb, ns, _ = _gpu_render(omerf, sc, cam, W, H, host=True)
+        _assert_parity(rgb, ns, O.render(cam, W, H, mode="clipped"), f"{W}x{H}")
+
+
+# ----------------------------------------------------------------------------- edge cameras, degenerate scenes
+EDGE_CAMS = [
+    ((4.0, 4.0, 2.0), (7.0, 5.0, 2.1)),         # inside the box, near-horizontal
+    ((4.0, -3.0, 1.5), (4.0, 4.0, 1.5)),        # horizontal, entering through a side
+    ((4.0, 4.0, 30.0), (4.0, 4.0001, 0.0)),     # straight down
+    ((-5.0, -5.0, 0.5), (8.0, 8.0, 3.5)),       # upward from below the slab
+    ((4.0, 4.0, 2.0), (4.0, 4.0, 9.0)),         # inside looking up
+    ((4.0, -6.0, 9.0), (4.0, -20.0, 12.0)),     # looking away: pure background
+    ((4.0, 4.0, 2.0), (9.0, 4.0, 2.0)),         # axis-parallel centre ray (d_y = d_z = 0 at the centre)
+]
+
+
+@pytest.mark.parametrize("origin,target", EDGE_CAMS)
+def test_edge_cameras(omerf, oracle, origin, target):
+    rng = np.random.default_rng(12)
+    lo = rng.uniform(0.5, 1.5, (9, 9)).astype(np.float32)
+    hi = (lo + rng.uniform(-0.2, 2.0, (9, 9))).astype(np.float32)      # a few empty columns (h_up < h_lo)
+    sc = synth.custom_scene(h_lo=lo, h_up=hi, seed=5, bias_amp=0.2, bg=(0.2, 0.5, 0.9))
+    cam = synth.look_at_camera(origin, target, 48, 40, vfov_deg=70.0)
+    rgb, ns, _ = _gpu_render(omerf, sc, cam, 48, 40)
+    _assert_parity(rgb, ns, oracle.OracleScene(sc).render(cam, 48, 40, mode="brute"), "edge camera")
+
+
+def test_empty_scene_is_background_exactly(omerf):
+    sc = synth.custom_scene(h_lo=3.0, h_up=1.0, bg=(0.25, 0.5, 0.75))
+    cam = synth.look_at_camera((4.0, -6.0, 9.0), (4.0, 4.0, 2.0), 32, 32)
+    rgb, ns, _ = _gpu_render(omerf, sc, cam, 32, 32)
+    assert ns.sum() == 0
+    assert np.array_equal(rgb.astype(np.float32), np.broadcast_to(np.array(sc.bg, dtype=np.float32), rgb.shape))
+
+
+def test_zero_views_and_batches(omerf, oracle):
+    import torch
+    sc = synth.make_scene(0)
+    W, H = 40, 24
+    cams = np.stack([synth.look_at_camera((32.0 + 30 * np.cos(a), 32.0 + 30 * np.sin(a), 25.0 + 3 * i), (32.0, 32.0, 8.0), W, H)
+                     for i, a in enumerate(np.linspace(0, 5, 7))])
+    with omerf.scene_create(sc) as h:
+        L = omerf.load_library()
+        dummy = torch.zeros(4, device="cuda")
+        assert L.omerf_render(h.ptr, cams.ctypes.data, 0, W, H, dummy.data_ptr(), dummy.data_ptr(), None) == 0
+        assert omerf.last_launch_count(h) == 0
+        rgb, ns = omerf.render(h, cams, W, H)
+        # a second call right behind the first (camera staging ring) on a side stream
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            rgb2, ns2 = omerf.render(h, cams[::-1].copy(), W, H, stream=st)
+        torch.cuda.synchronize()
+    ref = oracle.OracleScene(sc).render(cams, W, H, mode="clipped")
+    _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, "batch")
+    assert np.array_equal(ns2.cpu().numpy()[::-1], ns.cpu().numpy())
+    assert np.array_equal(rgb2.cpu().numpy()[::-1], rgb.cpu().numpy())
+
+
+def test_constant_slab_closed_form_on_gpu(omerf):
+    """The GPU path against the closed form directly (not via the oracle): T = exp(-tau n step)."""
+    import math
+    za, zb, byte, step = 1.0, 3.0, 127, 0.125
+    sc = synth.custom_scene(box=(32.0, 32.0, 4.0), h_lo=za, h_up=zb, fill=byte, step=step)
+    # zero the MLP's last layer: S = sigmoid(0) = 0.5, so rgb = (1-T) sigmoid(pre) + 0.5 + T bg, clamped
+    sc.W2[:] = 0
+    cam = synth.look_at_camera((16.0, 4.0, 14.0), (16.0, 16.0, 2.0), 16, 16, vfov_deg=20.0)
+    rgb, ns, _ = _gpu_render(omerf, sc, cam, 16, 16)
+    pre = 4.0 * (byte * 28.0 / 255.0 - 14.0)
+    tau = math.exp(pre)
+    sig = 1.0 / (1.0 + math.exp(-pre))
+    T = np.exp(-tau * ns * step)
+    expect = np.clip((1 - T) * sig + 0.5 + T * 1.0, 0, 1)
+    assert np.all(ns > 0)
+    c = cam.astype(np.float64)
+    for v in range(16):
+        for u in range(16):
+            g = c[9:12] + ((u + 0.5 - c[14]) / c[12]) * c[3:6] - ((v + 0.5 - c[15]) / c[13]) * c[6:9]
+            L = (zb - za) / abs(g[2] / np.linalg.norm(g))
+            assert abs(ns[0, v, u] * step - L) <= step * 1.001
+    sc.bg = (0.0, 0.0, 0.0)
+    rgb0, _, _ = _gpu_render(omerf, sc, cam, 16, 16)
+    assert np.max(np.abs(rgb0[..., 0] - np.clip((1 - T) * sig + 0.5, 0, 1))) < 1e-4
+    assert np.max(np.abs(rgb[..., 0] - expect)) < 1e-4 or np.all(expect == 1.0)
+
+
+# ----------------------------------------------------------------------------- S1 pyramid
+def test_pyramid_levels(omerf):
+    sc = synth.make_scene(0)
+    with omerf.scene_create(sc) as h:
+        info = omerf.scene_info(h)
+        assert info["pyramid_levels"] == 8                 # 65 -> 33 -> 17 -> 9 -> 5 -> 3 -> 2 -> 1
+        mn, mx = omerf.pyramid_level(h, 0)
+        assert np.array_equal(mn, sc.h_lo) and np.array_equal(mx, sc.h_up)
+        for l in range(1, info["pyramid_levels"]):
+            cmn, cmx = omerf.pyramid_level(h, l)
+            assert cmn.shape == ((mn.shape[0] + 1) // 2, (mn.shape[1] + 1) // 2)
+            pmn = np.pad(mn, ((0, mn.shape[0] % 2), (0, mn.shape[1] % 2)), constant_values=np.inf)
+            pmx = np.pad(mx, ((0, mx.shape[0] % 2), (0, mx.shape[1] % 2)), constant_values=-np.inf)
+            ref_mn = pmn.reshape(cmn.shape[0], 2, cmn.shape[1], 2).min(axis=(1, 3))
+            ref_mx = pmx.reshape(cmx.shape[0], 2, cmx.shape[1], 2).max(axis=(1, 3))
+            assert np.array_equal(cmn, ref_mn) and np.array_equal(cmx, ref_mx)
+            mn, mx = cmn, cmx
+        assert mn.shape == (1, 1) and mn[0, 0] == sc.h_lo.min() and mx[0, 0] == sc.h_up.max()
+        assert info["device_bytes"] >= sc.grid.nbytes + sc.plane_xy.nbytes + sc.plane_xz.nbytes + sc.plane_yz.nbytes
+
+
+# ----------------------------------------------------------------------------- S10 comparator (config 4 at small size)
+@pytest.mark.parametrize("hf_n,occ_n", [((17, 17), (32, 32, 32)), ((9, 12), (20, 23, 7)), ((33, 33), (64, 64, 16))])
+def test_bitfield_matches_oracle(omerf, oracle, hf_n, occ_n):
+    rng = np.random.default_rng(31)
+    lo = (1.0 + 0.5 * rng.random(hf_n)).astype(np.float32)
+    hi = (lo - 0.2 + 1.7 * rng.random(hf_n)).astype(np.float32)
+    sc = synth.custom_scene(box=(16.0, 12.0, 4.0), hf_n=hf_n, h_lo=lo, h_up=hi, occ_n=occ_n)
+    O = oracle.OracleScene(sc, sampler=1)
+    with omerf.scene_create(sc, sampler=1) as h:
+        bits = omerf.bitfield(h, occ_n)
+        info = omerf.scene_info(h)
+    assert np.array_equal(bits, O.bits)
+    assert info["occ_bits_set"] == int(np.unpackbits(O.bits.view(np.uint8)).sum())
+
+
+def test_grid_sampler_parity_and_superset(omerf, oracle):
+    rng = np.random.default_rng(33)
+    m = 33
+    lo = (1.0 + 0.5 * rng.random((m, m))).astype(np.float32)
+    hi = (lo + 0.3 + 1.5 * rng.random((m, m))).astype(np.float32)
+    sc = synth.custom_scene(box=(16.0, 16.0, 4.0), hf_n=(m, m), h_lo=lo, h_up=hi, step=0.125, occ_n=(64, 64, 32), seed=2)
+    cams = np.stack([synth.look_at_camera((8.0, -10.0, 14.0), (8.0, 8.0, 2.0), 64, 48),
+                     synth.look_at_camera((2.0, 3.0, 2.5), (14.0, 12.0, 1.0), 64, 48)])
+    rgb_g, ns_g, _ = _gpu_render(omerf, sc, cams, 64, 48, sampler=1)
+    _assert_parity(rgb_g, ns_g, oracle.OracleScene(sc, sampler=1).render(cams, 64, 48, mode="brute"), "grid sampler")
+    rgb_p, ns_p, _ = _gpu_render(omerf, sc, cams, 64, 48, sampler=0)
+    _assert_parity(rgb_p, ns_p, oracle.OracleScene(sc, sampler=0).render(cams, 64, 48, mode="brute"), "plane sampler")
+    assert ns_g.sum() >= ns_p.sum()
