@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the Oblique-MERF render hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
+
+A *step* is one pass of the whole hot path (S2..S9: ray generation, clip, occupancy-plane march,
+gathers, activations, compositing, deferred MLP, outputs) over one batch = the camera(s) of
+BASELINE.json configs[1] (one 1920x1080 view of the 1000x1000x100 m scene).  Inputs are seeded
+synthetic stand-ins for the paper's baked scenes.
+
+value   = Mpixels/s, whole job (all ranks), scene resident in HBM, device-timed with CUDA events on the
+          launching stream; L2 is flushed between timed steps (the flush is outside the event pairs).
+e2e     = the same through omerf_render_host: cameras from host memory, rgb + counts copied back to pinned
+          host memory inside the timed region.
+roofline= march kernel: algorithmic bytes (168 B per sample + 16 B per pixel) / launch duration
+          against the measured HBM copy rate in MEASURED_PEAKS.json.
+cpu_baseline = the CPU oracle as it stands on this box's host cores, on a bounded sample of the same frame.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402
+
+BYTES_PER_SAMPLE = 168   # 20 texels x 8 B (64 B grid + 96 B planes) + one (z_min, z_max) pair of 8 B
+BYTES_PER_PIXEL = 16     # 12 B rgb + 4 B sample count written
+
+
+def workload_name(cfg: int) -> str:
+    return {0: "configs[0] tiny 128x128", 1: "configs[1] 1080p oblique frame, 1000x1000x100 m scene",
+            2: "configs[2] 16 x 1080p views", 3: "configs[3] 8 x 2160p views, 4000x4000x200 m scene",
+            4: "configs[4] sampling ablation (config-1 scene+camera)"}[cfg]
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md 'clocks' line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+                for nm, val in zip(names, r[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            except (ValueError, IndexError):
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_bounded(scene, cams, W, H, sampler=0, budget_s=15.0):
+    """Time the oracle (clipped loop, OpenMP on all host cores) on every `stride`-th row of view 0."""
+    import oracle
+    O = oracle.OracleScene(scene, sampler=sampler)
+    t0 = time.perf_counter()
+    probe_rows = list(range(0, H, max(H // 8, 1)))[:8]
+    n = 0
+    for v in probe_rows:
+        r = O.render(cams[:1], W, H, mode="clipped", rows=(v, v + 1))
+        n += int(r["nsamples"][0, v].sum())
+    t_probe = time.perf_counter() - t0
+    per_row = t_probe / len(probe_rows)
+    n_rows = int(max(8, min(H, budget_s / max(per_row, 1e-6))))
+    stride = max(H // n_rows, 1)
+    rows = list(range(stride // 2, H, stride))
+    t0 = time.perf_counter()
+    samples = 0
+    threads = 1
+    # contiguous row blocks are cheaper to call; rows are sampled with a stride so sky and ground both count
+    for v in rows:
+        r = O.render(cams[:1], W, H, mode="clipped", rows=(v, v + 1))
+        samples += int(r["nsamples"][0, v].sum())
+        threads = r["threads"]
+    dt = time.perf_counter() - t0
+    px = len(rows) * W
+    return {"mpix_s": px / dt / 1e6, "msamples_s": samples / dt / 1e6, "seconds": dt, "pixels": px, "samples": samples,
+            "cores": threads, "sample": f"{len(rows)} of {H} rows (every {stride}th) of view 0, clipped loop"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, timed on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = args.config
+    scene = synth.make_scene(cfg)
+    cams = synth.make_cameras(cfg)
+    W, H = synth.config_resolution(cfg)
+    budget = 120.0 / max(args.steps + args.warmup, 1)
+    times, res = [], None
+    for i in range(args.warmup + args.steps):
+        res = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=min(budget, 20.0))
+        if i >= args.warmup:
+            times.append(res)
+    mp = float(np.mean([r["mpix_s"] for r in times]))
+    line = {
+        "impl": "reference", "metric": "Mpixels/s", "value": mp, "unit": "Mpixels/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean([r["seconds"] for r in times]) * 1e3),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 decisions / f64 colour",
+        "data": "synthetic", "config": {"workload": workload_name(cfg), "sample_per_step": res["sample"]},
+        "gsamples_s": float(np.mean([r["msamples_s"] for r in times]) / 1e3),
+        "cpu_baseline": {"value": mp, "unit": "Mpixels/s", "cores": res["cores"], "kind": "oracle", "sample": res["sample"]},
+        "e2e": {"value": mp, "unit": "Mpixels/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2404_09531_b200 as omerf
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the renderer has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = args.config
+    scene = synth.make_scene(cfg)
+    cams = synth.make_cameras(cfg)
+    W, H = synth.config_resolution(cfg)
+    n_views = cams.shape[0]
+    sampler = omerf.SAMPLER_GRID if args.sampler == "grid" else omerf.SAMPLER_PLANE
+    h = omerf.scene_create(scene, sampler=sampler)
+    info = omerf.scene_info(h)
+    out_rgb = torch.empty((n_views, H, W, 3), dtype=torch.float32, device="cuda")
+    out_n = torch.empty((n_views, H, W), dtype=torch.int32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")           # > 126 MB L2
+    stream = torch.cuda.current_stream()
+    pixels = n_views * W * H
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(n_steps, do_flush, fn):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_steps)]
+        for a, b in evs:
+            if do_flush:
+                flush.fill_(1)
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    def dev_step():
+        omerf.render(h, cams, W, H, out_rgb, out_n, stream=stream)
+
+    for _ in range(max(args.warmup, 3)):
+        dev_step()
+    barrier()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    ms = timed(args.steps, True, dev_step)                                     # the timed region: K steps
+    barrier()
+    launches_per_step = omerf.last_launch_count(h)
+    ms_warm = timed(args.steps, False, dev_step)                               # extra: L2-warm static camera
+    barrier()
+    clk = clocks.stop() if rank == 0 else None
+    total_ms = float(np.sum(ms))
+    samples = int(out_n.sum(dtype=torch.int64).item())
+
+    # e2e through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    h_rgb = torch.empty((n_views, H, W, 3), dtype=torch.float32).pin_memory()
+    h_n = torch.empty((n_views, H, W), dtype=torch.int32).pin_memory()
+
+    def e2e_step():
+        omerf.render_host(h, cams, W, H, h_rgb, h_n, stream=stream)
+
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    ms_e2e = timed(args.steps, True, e2e_step)
+    barrier()
+    wall_e2e = time.perf_counter() - t0
+    assert int(h_n.sum(dtype=torch.int64).item()) == samples, "host and device outputs disagree"
+
+    # max over ranks of the device time
+    t = torch.tensor([total_ms, float(np.sum(ms_e2e)), float(np.sum(ms_warm))], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, total_e2e_ms, total_warm_ms = (float(x) for x in t.tolist())
+
+    if rank == 0:
+        peaks = {}
+        pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(pk):
+            peaks = json.load(open(pk))
+        hbm = float(peaks.get("hbm_gbs", 6650.0))
+        k = args.steps
+        secs = total_ms / 1e3
+        march_ms = total_ms / k                                  # one launch per step: the fused march kernel
+        alg_bytes = samples * BYTES_PER_SAMPLE + pixels * BYTES_PER_PIXEL
+        achieved = alg_bytes / (march_ms / 1e3) / 1e9
+        cpu = None
+        if not args.no_cpu_baseline:
+            cpu = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=15.0)
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get(f"config{cfg}_{args.sampler}")
+        line = {
+            "metric": "Mpixels/s", "value": world * pixels * k / secs / 1e6, "unit": "Mpixels/s", "n_gpus": world,
+            "steps": k, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32 (u8 features, integer interpolation)",
+            "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "views": n_views, "W": W, "H": H, "sampler": args.sampler,
+                       "scene_device_bytes": info["device_bytes"], "l2": "flushed between timed steps (256 MiB fill, "
+                       "outside the event pairs); scene 296 MiB > L2", "parallelism": f"replicated scene x{world}"},
+            "frames_per_s": world * n_views * k / secs,
+            "gsamples_s": world * samples * k / secs / 1e9,
+            "samples_per_step": samples, "samples_per_ray": samples / pixels,
+            "l2_warm": {"ms_per_step": total_warm_ms / k, "mpixels_s": world * pixels * k / (total_warm_ms / 1e3) / 1e6},
+            "e2e": {"value": world * pixels * k / (total_e2e_ms / 1e3) / 1e6, "unit": "Mpixels/s",
+                    "h2d_bytes_per_step": int(cams.nbytes), "d2h_bytes_per_step": pixels * BYTES_PER_PIXEL,
+                    "ms_per_step": total_e2e_ms / k, "wall_ms_per_step": wall_e2e * 1e3 / k},
+            "gpu_launches": launches_per_step * k,
+            "roofline": {"bound": "hbm", "kernel": "omerf_march_kernel", "achieved": achieved, "peak": hbm,
+                         "unit": "GB/s", "frac": achieved / hbm, "traffic": traffic,
+                         "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "fallback 6650 (of fallback)",
+                         "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": march_ms},
+            "clocks": clk,
+        }
+        if cpu is not None:
+            line["cpu_baseline"] = {"value": cpu["mpix_s"], "unit": "Mpixels/s", "cores": cpu["cores"], "kind": "oracle",
+                                    "sample": cpu["sample"], "msamples_s": cpu["msamples_s"], "seconds": cpu["seconds"]}
+        print(json.dumps(line))
+    omerf.scene_destroy(h)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--sampler", default="plane", choices=["plane", "grid"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,96 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (-m gpu).
+
+The whole frame is rendered on the GPU; the oracle computes sampled pixels one by one (a random subset
+plus whole rows), and properties that hold at any size are checked on the full outputs."""
+import numpy as np
+import pytest
+
+import synth
+
+pytestmark = pytest.mark.gpu
+RGB_TOL = 2e-3
+
+
+@pytest.fixture(scope="module")
+def omerf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2404_09531_b200 as m
+    m.load_library()
+    return m
+
+
+@pytest.fixture(scope="module")
+def city():
+    return synth.make_scene(1)
+
+
+def _sample_pixels(rng, n_views, W, H, n_random, rows):
+    vuv = np.stack([rng.integers(0, n_views, n_random), rng.integers(0, W, n_random), rng.integers(0, H, n_random)], axis=1)
+    extra = [np.stack([np.full(W, v), np.arange(W), np.full(W, r)], axis=1) for v in range(n_views) for r in rows]
+    return np.concatenate([vuv] + extra).astype(np.int32)
+
+
+def _check_sampled(omerf, scene, cams, W, H, sampler, n_random, rows, seed):
+    import torch
+
+    import oracle
+    rng = np.random.default_rng(seed)
+    with omerf.scene_create(scene, sampler=sampler) as h:
+        rgb, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        rgb = rgb.cpu().numpy()
+        ns = ns.cpu().numpy().view(np.uint32)
+    vuv = _sample_pixels(rng, cams.shape[0], W, H, n_random, rows)
+    ref = oracle.OracleScene(scene, sampler=sampler).render_pixels(cams, W, H, vuv, mode="clipped")
+    got_n = ns[vuv[:, 0], vuv[:, 2], vuv[:, 1]]
+    got_rgb = rgb[vuv[:, 0], vuv[:, 2], vuv[:, 1]].astype(np.float64)
+    bad = got_n != ref["nsamples"]
+    assert not bad.any(), f"{int(bad.sum())} of {len(vuv)} sampled pixels have wrong counts, e.g. {vuv[bad][:5].tolist()}"
+    assert np.abs(got_rgb - ref["rgb"]).max() <= RGB_TOL
+    # properties at any size
+    assert np.all(np.isfinite(rgb)) and rgb.min() >= 0.0 and rgb.max() <= 1.0
+    empty = ns == 0
+    assert np.array_equal(rgb[empty], np.broadcast_to(np.array(scene.bg, dtype=np.float32), rgb[empty].shape))
+    assert ref["nsamples"].sum() > 0
+    return rgb, ns
+
+
+def test_config1_1080p(omerf, city):
+    cams = synth.make_cameras(1)
+    W, H = synth.config_resolution(1)
+    rgb, ns = _check_sampled(omerf, city, cams, W, H, 0, 40000, [0, 400, 777, 1079], seed=101)
+    assert 2.0 < ns.mean() < 12.0            # a few samples per ray with a long tail
+
+
+def test_config2_batch_of_16(omerf, city):
+    cams = synth.make_cameras(2)
+    W, H = synth.config_resolution(2)
+    rgb, ns = _check_sampled(omerf, city, cams, W, H, 0, 60000, [3, 540], seed=102)
+    per_view = ns.reshape(16, -1).sum(axis=1)
+    assert np.all(per_view > 0)
+
+
+def test_config4_both_samplers(omerf, city):
+    cams = synth.make_cameras(4)
+    W, H = synth.config_resolution(4)
+    _, ns_p = _check_sampled(omerf, city, cams, W, H, 0, 15000, [600], seed=104)
+    _, ns_g = _check_sampled(omerf, city, cams, W, H, 1, 15000, [600], seed=104)
+    # the grid voxels are a superset of the slab (R18): more samples overall
+    assert ns_g.sum() >= ns_p.sum()
+    with omerf.scene_create(city, sampler=1) as h:
+        ratio = omerf.scene_info(h)["occ_bits_set"] / float(np.prod(city.occ_n))
+    w = np.ones(1025)
+    w[0] = w[-1] = 0.5
+    area = np.outer(w, w)
+    frac = float(((city.h_up - city.h_lo).astype(np.float64) * area).sum() / area.sum() / city.box[2])
+    dz = city.box[2] / city.occ_n[2]
+    assert frac <= ratio <= frac + 2 * dz / city.box[2] + 1e-9
+
+
+def test_config3_large_scene(omerf):
+    scene = synth.make_scene(3)
+    cams = synth.make_cameras(3)
+    W, H = synth.config_resolution(3)
+    _check_sampled(omerf, scene, cams, W, H, 0, 40000, [1080], seed=103)
