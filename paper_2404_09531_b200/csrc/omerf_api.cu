@@ -54,6 +54,7 @@ static void free_scene(omerf_scene *s)
     cudaFree(s->d_pyz);
     cudaFree(s->d_occ);
     cudaFree(s->d_cams);
+    cudaFree(s->d_tile_counter);
     cudaFree(s->d_scratch_rgb);
     cudaFree(s->d_scratch_n);
     if (s->h_cams) cudaFreeHost(s->h_cams);
@@ -156,6 +157,7 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
             for (int i = 0; i < 3; i++) {
                 v.N[i] = d->occ_n[i];
                 v.ns[i] = (float)d->occ_n[i] / d->box[i];
+                v.vox[i] = d->box[i] / (float)d->occ_n[i];
             }
             if ((rc = omerf_launch_bitfield(s, 0))) break;
         }
@@ -163,6 +165,14 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         if (e != cudaSuccess) {
             rc = omerf_cuda_fail(e, "scene build");
             break;
+        }
+        if ((rc = omerf_query_persistent_blocks(d->sampler, &s->persistent_blocks))) break;
+        {
+            cudaError_t ee = cudaMalloc((void **)&s->d_tile_counter, sizeof(unsigned int));
+            if (ee != cudaSuccess) {
+                rc = omerf_cuda_fail(ee, "cudaMalloc tile counter");
+                break;
+            }
         }
         // camera staging ring
         s->cam_capacity = 0;

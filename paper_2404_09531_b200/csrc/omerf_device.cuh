@@ -36,6 +36,7 @@ struct DevScene {
     int sampler;
     int N[3];
     float ns[3];           // N/box per axis
+    float vox[3];          // box/N per axis (proposals only)
     int occ_levels;
     const uint32_t *occ;   // all levels; level l has dims ceil(N/2^l), bit index ((jx*ny+jy)*nz+jz)
     unsigned long long occ_off[OMERF_MAX_LEVELS]; // word offset of each level
@@ -62,6 +63,8 @@ struct omerf_scene {
     mutable uint32_t *d_scratch_n;
     mutable uint64_t scratch_pixels;
     mutable int last_launches;
+    unsigned int *d_tile_counter;     // work queue head of the persistent march kernel
+    int persistent_blocks;            // resident CTAs of the march kernel (SMs x occupancy)
 };
 
 #define OMERF_CAM_SLOTS 16
@@ -80,3 +83,4 @@ int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, c
 int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st);
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H,
                         float *out_rgb, uint32_t *out_n, cudaStream_t st, int *launches);
+int omerf_query_persistent_blocks(int sampler, int *blocks);

@@ -1,13 +1,20 @@
-// omerf_render.cu — S2..S9 of the hot path as one fused kernel per frame batch.
+// omerf_render.cu — S2..S9 of the hot path: one persistent kernel per frame batch.
 //
-// One thread per pixel; a warp owns an 8x4 pixel tile so that neighbouring rays share texels.
-//   S2 ray generation          fp32, one correctly rounded operation per step (bit-exact with the oracle)
-//   S3 box clip                fp32 slab test, padded by 2 lattice indices (conservative; the exact
-//                              per-sample predicate decides membership)
-//   S4 occupancy-plane march   stackless traversal of the min/max pyramid of (z_min, z_max): in empty
-//                              space the ray jumps to the exit of the coarsest empty node or to the start
-//                              of the node's z-interval; every jump is VERIFIED with the
-//                              exact lattice arithmetic, so skipping never changes which samples exist
+// Persistent warps with ray refill.  Each lane owns one ray at a time and is in one of four states:
+//   IDLE -> (refill: S2 ray generation + S3 box clip) -> TRAV -> READY -> (sample) -> TRAV ... -> FIN -> IDLE
+// A warp round runs, in this order and only when enough lanes want it, (1) retire: deferred MLP + store for
+// FIN lanes, (2) refill: IDLE lanes take the next pixels of the warp's current 8x4 tile (tiles come from a
+// global atomic counter), (3) one traversal step for TRAV lanes, (4) one sample for READY lanes.  Rays have
+// very different lengths (about 4 samples on average, a long tail, many sky rays with none), so binding a ray
+// to a lane for the whole kernel leaves two thirds of the lanes idle (measured: 10.5 of 32 lanes active);
+// refill keeps the expensive phases (sample: ~450 instructions, MLP: ~1100) close to full.
+//
+//   S2 ray generation          fp32, one correctly rounded operation per step (bit-exact with the CPU checker)
+//   S3 box clip                fp32 slab test, padded by 2 lattice indices (the exact per-sample predicate decides)
+//   S4 occupancy-plane march   hierarchical DDA over the min/max pyramid of (z_min, z_max): in empty space the
+//                              ray jumps to the exit of the coarsest empty node or to the start of the node's
+//                              z-interval; every jump is VERIFIED with the exact lattice
+//                              arithmetic, so skipping never changes which samples exist
 //   S5 gather                  trilinear grid + 3 bilinear planes, uint8 x 8 channels per 8-byte load,
 //                              8-bit fixed-point weights, exact integer sums (Eq. 2, R9)
 //   S6 activations             exp (exp_q on the decision path), sigmoid (Eq. 3)
@@ -23,8 +30,22 @@
 
 namespace {
 
+enum : int { ST_IDLE = 0, ST_TRAV = 1, ST_READY = 2, ST_FIN = 3 };
+
+// scheduling thresholds (lanes): tuned on B200 with configs[1]
+#ifndef OMERF_RETIRE_T
+#define OMERF_RETIRE_T 12
+#endif
+#ifndef OMERF_REFILL_T
+#define OMERF_REFILL_T 8
+#endif
+#ifndef OMERF_SAMPLE_T
+#define OMERF_SAMPLE_T 20
+#endif
+
 struct Ray {
     float ox, oy, oz, dx, dy, dz;
+    float ix, iy, iz; // reciprocals of d (INF where d == 0), proposals only
 };
 
 __device__ __forceinline__ float exp_q(float x)
@@ -70,72 +91,69 @@ __device__ __forceinline__ int voxel_index(float p, float s, int N)
     return min(max(j, 0), N - 1);
 }
 
-// exit parameter of the ray from the 1D interval [lo, hi]
-__device__ __forceinline__ float axis_exit(float o, float d, float lo, float hi)
-{
-    if (d > 0.0f) return __fdividef(hi - o, d);
-    if (d < 0.0f) return __fdividef(lo - o, d);
-    return INFINITY;
-}
-
 // last lattice index whose parameter is below t_end (proposal only; verified by the caller)
 __device__ __forceinline__ int index_before(float t_end, float inv_step, int k1)
 {
-    float f = ceilf(t_end * inv_step - 0.5f) - 1.0f;
+    float f = ceilf(fmaf(t_end, inv_step, -0.5f)) - 1.0f;
     return f >= (float)k1 ? k1 : (int)f;
 }
 
-// ---------------------------------------------------------------------------------- S4: find the next sample
-// sampler PLANE.  Returns true with k = index of the next occupied lattice sample, false if none is left.
-__device__ __forceinline__ bool next_sample_plane(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl,
-                                                  float &px, float &py, float &pz)
+// ---------------------------------------------------------------------------------- S4: one traversal step
+// sampler PLANE.  Advances (k, lvl); returns ST_READY when lattice sample k passes the predicate (Eq. 7),
+// ST_FIN when no sample is left, ST_TRAV otherwise.
+__device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl)
 {
+    if (k > k1) return ST_FIN;
+    float px, py, pz;
+    lattice_point(r, sc.step, k, px, py, pz);
     const int top = sc.n_levels - 1;
-    while (k <= k1) {
-        lattice_point(r, sc.step, k, px, py, pz);
-        if (!in_box(sc, px, py, pz)) {
+    // cell indices are clamped, so points of the 2-index padding outside the box still address valid nodes;
+    // the box test is only needed where a sample is declared
+    const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
+    const int nx = ix >> lvl, ny = iy >> lvl;
+    const float2 h = __ldg(sc.pyr + sc.lvl_off[lvl] + nx * sc.lvl_ny[lvl] + ny);
+    const bool above = pz > h.y, below = pz < h.x;
+    if (!above && !below) {
+        if (lvl == 0) {
+            if (in_box(sc, px, py, pz)) return ST_READY; // z_min <= z <= z_max at the nearest grid point (Eq. 7)
             k++;
-            continue;
+            return ST_TRAV;
         }
-        const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
-        const int nx = ix >> lvl, ny = iy >> lvl;
-        const float2 h = __ldg(sc.pyr + sc.lvl_off[lvl] + nx * sc.lvl_ny[lvl] + ny);
-        const bool above = pz > h.y, below = pz < h.x;
-        if (!above && !below) {
-            // NaN-free inputs: inside [min,max] of the node (an empty level-0 cell has min > max: both flags set)
-            if (lvl == 0) return true; // Eq. 7: z_min <= z <= z_max at the nearest grid point
-            lvl--;
-            continue;
-        }
-        // outside the node's z-range: propose a jump to the node's xy exit or to where z reaches the range
-        const float x_lo = ((float)(nx << lvl) - 0.5f) * sc.cell_x, x_hi = ((float)((nx + 1) << lvl) - 0.5f) * sc.cell_x;
-        const float y_lo = ((float)(ny << lvl) - 0.5f) * sc.cell_y, y_hi = ((float)((ny + 1) << lvl) - 0.5f) * sc.cell_y;
-        float t_end = fminf(axis_exit(r.ox, r.dx, x_lo, x_hi), axis_exit(r.oy, r.dy, y_lo, y_hi));
-        if (above && !below) {
-            if (r.dz < 0.0f) t_end = fminf(t_end, __fdividef(h.y - r.oz, r.dz));
-        } else if (below && !above) {
-            if (r.dz > 0.0f) t_end = fminf(t_end, __fdividef(h.x - r.oz, r.dz));
-        }
-        int kk = index_before(t_end, sc.inv_step, k1);
-        bool jumped = false;
-#pragma unroll 1
-        for (int attempt = 0; attempt < 2 && kk > k; attempt++, kk--) {
-            float qx, qy, qz;
-            lattice_point(r, sc.step, kk, qx, qy, qz);
-            const int jx = cell_index(qx, sc.sx, sc.Mx) >> lvl, jy = cell_index(qy, sc.sy, sc.My) >> lvl;
-            const bool same_side = (above ? qz > h.y : true) && (below ? qz < h.x : true);
-            if (jx == nx && jy == ny && same_side) {
-                k = kk + 1;
-                lvl = min(lvl + 1, top);
-                jumped = true;
-                break;
-            }
-        }
-        if (jumped) continue;
-        if (lvl > 0) lvl--;
-        else k++; // level 0 and the predicate is false at k
+        lvl--;
+        return ST_TRAV;
     }
-    return false;
+    // outside the node's z-range: propose a jump to the node's xy exit or to where z reaches the range.
+    // The boundary crossed decides the next level: an even boundary index also leaves the parent node.
+    const int bxi = nx + (r.dx > 0.0f ? 1 : 0), byi = ny + (r.dy > 0.0f ? 1 : 0);
+    const float xb = fmaf((float)(bxi << lvl), sc.cell_x, -0.5f * sc.cell_x);
+    const float yb = fmaf((float)(byi << lvl), sc.cell_y, -0.5f * sc.cell_y);
+    const float tx = r.dx != 0.0f ? (xb - r.ox) * r.ix : INFINITY;
+    const float ty = r.dy != 0.0f ? (yb - r.oy) * r.iy : INFINITY;
+    float tz = INFINITY;
+    if (above && !below && r.dz < 0.0f) tz = (h.y - r.oz) * r.iz;
+    if (below && !above && r.dz > 0.0f) tz = (h.x - r.oz) * r.iz;
+    const float t_end = fminf(fminf(tx, ty), tz);
+    const int kk = index_before(t_end, sc.inv_step, k1);
+    if (kk > k) {
+        float qx, qy, qz;
+        lattice_point(r, sc.step, kk, qx, qy, qz);
+        const int jx = cell_index(qx, sc.sx, sc.Mx) >> lvl, jy = cell_index(qy, sc.sy, sc.My) >> lvl;
+        const bool same_side = (above ? qz > h.y : true) && (below ? qz < h.x : true);
+        if (jx == nx && jy == ny && same_side) {
+            k = kk + 1;
+            if (tz <= fminf(tx, ty)) {
+                lvl = max(lvl - 1, 0); // entering the node's z-range: refine
+            } else {
+                const int crossed = tx <= ty ? bxi : byi;
+                const int up = crossed == 0 ? 31 : __ffs(crossed) - 1; // levels whose boundary this also is
+                lvl = min(lvl + min(up, 2), top);
+            }
+            return ST_TRAV;
+        }
+    }
+    if (lvl > 0) lvl--;
+    else k++; // level 0 and the predicate is false at k
+    return ST_TRAV;
 }
 
 __device__ __forceinline__ bool occ_test(const DevScene &sc, int lvl, int jx, int jy, int jz)
@@ -144,61 +162,60 @@ __device__ __forceinline__ bool occ_test(const DevScene &sc, int lvl, int jx, in
     return (__ldg(sc.occ + sc.occ_off[lvl] + (idx >> 5)) >> (idx & 31)) & 1u;
 }
 
-// sampler GRID (config-4 comparator): multi-resolution binary occupancy grid with DDA-style skipping.
-__device__ __forceinline__ bool next_sample_grid(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl,
-                                                 float &px, float &py, float &pz)
+// sampler GRID (config-4 comparator): multi-resolution binary occupancy grid, DDA-style skipping.
+__device__ __forceinline__ int trav_step_grid(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl)
 {
-    const int top = sc.occ_levels - 1;
-    while (k <= k1) {
-        lattice_point(r, sc.step, k, px, py, pz);
-        if (!in_box(sc, px, py, pz)) {
-            k++;
-            continue;
-        }
-        const int nx = voxel_index(px, sc.ns[0], sc.N[0]) >> lvl, ny = voxel_index(py, sc.ns[1], sc.N[1]) >> lvl,
-                  nz = voxel_index(pz, sc.ns[2], sc.N[2]) >> lvl;
-        if (occ_test(sc, lvl, nx, ny, nz)) {
-            if (lvl == 0) return true;
-            lvl--;
-            continue;
-        }
-        const float vx = sc.box[0] / (float)sc.N[0], vy = sc.box[1] / (float)sc.N[1], vz = sc.box[2] / (float)sc.N[2];
-        float t_end = axis_exit(r.ox, r.dx, (float)(nx << lvl) * vx, (float)((nx + 1) << lvl) * vx);
-        t_end = fminf(t_end, axis_exit(r.oy, r.dy, (float)(ny << lvl) * vy, (float)((ny + 1) << lvl) * vy));
-        t_end = fminf(t_end, axis_exit(r.oz, r.dz, (float)(nz << lvl) * vz, (float)((nz + 1) << lvl) * vz));
-        int kk = index_before(t_end, sc.inv_step, k1);
-        bool jumped = false;
-#pragma unroll 1
-        for (int attempt = 0; attempt < 2 && kk > k; attempt++, kk--) {
-            float qx, qy, qz;
-            lattice_point(r, sc.step, kk, qx, qy, qz);
-            if ((voxel_index(qx, sc.ns[0], sc.N[0]) >> lvl) == nx && (voxel_index(qy, sc.ns[1], sc.N[1]) >> lvl) == ny &&
-                (voxel_index(qz, sc.ns[2], sc.N[2]) >> lvl) == nz) {
-                k = kk + 1;
-                lvl = min(lvl + 1, top);
-                jumped = true;
-                break;
-            }
-        }
-        if (jumped) continue;
-        if (lvl > 0) lvl--;
-        else k++;
+    if (k > k1) return ST_FIN;
+    float px, py, pz;
+    lattice_point(r, sc.step, k, px, py, pz);
+    if (!in_box(sc, px, py, pz)) {
+        k++;
+        return ST_TRAV;
     }
-    return false;
+    const int top = sc.occ_levels - 1;
+    const int nx = voxel_index(px, sc.ns[0], sc.N[0]) >> lvl, ny = voxel_index(py, sc.ns[1], sc.N[1]) >> lvl,
+              nz = voxel_index(pz, sc.ns[2], sc.N[2]) >> lvl;
+    if (occ_test(sc, lvl, nx, ny, nz)) {
+        if (lvl == 0) return ST_READY;
+        lvl--;
+        return ST_TRAV;
+    }
+    const int bxi = nx + (r.dx > 0.0f ? 1 : 0), byi = ny + (r.dy > 0.0f ? 1 : 0), bzi = nz + (r.dz > 0.0f ? 1 : 0);
+    const float tx = r.dx != 0.0f ? ((float)(bxi << lvl) * sc.vox[0] - r.ox) * r.ix : INFINITY;
+    const float ty = r.dy != 0.0f ? ((float)(byi << lvl) * sc.vox[1] - r.oy) * r.iy : INFINITY;
+    const float tz = r.dz != 0.0f ? ((float)(bzi << lvl) * sc.vox[2] - r.oz) * r.iz : INFINITY;
+    const float t_end = fminf(fminf(tx, ty), tz);
+    const int kk = index_before(t_end, sc.inv_step, k1);
+    if (kk > k) {
+        float qx, qy, qz;
+        lattice_point(r, sc.step, kk, qx, qy, qz);
+        if ((voxel_index(qx, sc.ns[0], sc.N[0]) >> lvl) == nx && (voxel_index(qy, sc.ns[1], sc.N[1]) >> lvl) == ny &&
+            (voxel_index(qz, sc.ns[2], sc.N[2]) >> lvl) == nz) {
+            k = kk + 1;
+            const int crossed = (tx <= ty && tx <= tz) ? bxi : (ty <= tz ? byi : bzi);
+            const int up = crossed == 0 ? 31 : __ffs(crossed) - 1;
+            lvl = min(lvl + min(up, 2), top);
+            return ST_TRAV;
+        }
+    }
+    if (lvl > 0) lvl--;
+    else k++;
+    return ST_TRAV;
 }
 
 // ---------------------------------------------------------------------------------- S5: gather (Eq. 2)
 __device__ __forceinline__ void axis_tap(float p, float s, int N, int &i0, int &i1, uint32_t &w)
 {
-    float q = __fmaf_rn(p, s, -0.5f);
-    float fl = floorf(q);
-    w = (uint32_t)(int)floorf(__fadd_rn(__fmul_rn(__fsub_rn(q, fl), 256.0f), 0.5f));
-    int i = (int)fl;
+    const float q = __fmaf_rn(p, s, -0.5f);
+    const int i = __float2int_rd(q);
+    // (q - floor q) * 256 is exact, so one fma rounds exactly like the mul followed by the add
+    w = (uint32_t)__float2int_rd(__fmaf_rn(__fsub_rn(q, __int2float_rn(i)), 256.0f, 0.5f));
     i0 = min(max(i, 0), N - 1);
     i1 = min(max(i + 1, 0), N - 1);
 }
 
-__device__ __forceinline__ uint32_t byte_of(uint32_t x, int c) { return (x >> (8 * c)) & 0xffu; }
+// byte c of x, zero-extended: one PRMT
+__device__ __forceinline__ uint32_t byte_of(uint32_t x, int c) { return __byte_perm(x, 0u, 0x4440u + (uint32_t)c); }
 
 // out[c] (+)= sum over the 2x2 footprint of w_ab * texel_ab[c]; exact integers <= 255 * 2^16
 template <bool ACCUM>
@@ -266,7 +283,7 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
     bilinear8<true>(sc.pyz, sc.yz_n[1], a0, a1, wa, b0, b1, wb, I);
 }
 
-__device__ __forceinline__ float sigmoid_fast(float x) { return __frcp_rn(1.0f + __expf(-x)); }
+__device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
 
 // ---------------------------------------------------------------------------------- S8: deferred MLP (Eq. 4)
 __device__ __forceinline__ void deferred_mlp(const DevScene &sc, const float acc[7], const Ray &r, float S[3])
@@ -313,110 +330,189 @@ __device__ __forceinline__ void deferred_mlp(const DevScene &sc, const float acc
     }
 }
 
-// ---------------------------------------------------------------------------------- the fused kernel
+// ---------------------------------------------------------------------------------- S2 + S3: new ray for a lane
+// Returns false when the ray cannot have samples (misses the padded box).
+__device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera &cam, int u, int v, Ray &r, int &k,
+                                          int &k1)
+{
+    // S2 (R19): every step one correctly rounded fp32 operation
+    const float a = __fdiv_rn(__fsub_rn(__fadd_rn(__int2float_rn(u), 0.5f), cam.cx), cam.fx);
+    const float b = -__fdiv_rn(__fsub_rn(__fadd_rn(__int2float_rn(v), 0.5f), cam.cy), cam.fy);
+    const float gx = __fmaf_rn(a, cam.right[0], __fmaf_rn(b, cam.up[0], cam.fwd[0]));
+    const float gy = __fmaf_rn(a, cam.right[1], __fmaf_rn(b, cam.up[1], cam.fwd[1]));
+    const float gz = __fmaf_rn(a, cam.right[2], __fmaf_rn(b, cam.up[2], cam.fwd[2]));
+    const float len2 = __fmaf_rn(gx, gx, __fmaf_rn(gy, gy, __fmul_rn(gz, gz)));
+    const float inv = __fdiv_rn(1.0f, __fsqrt_rn(len2));
+    r.ox = cam.origin[0];
+    r.oy = cam.origin[1];
+    r.oz = cam.origin[2];
+    r.dx = __fmul_rn(gx, inv);
+    r.dy = __fmul_rn(gy, inv);
+    r.dz = __fmul_rn(gz, inv);
+    r.ix = r.dx != 0.0f ? __fdividef(1.0f, r.dx) : INFINITY; // proposals only: approximate is fine
+    r.iy = r.dy != 0.0f ? __fdividef(1.0f, r.dy) : INFINITY;
+    r.iz = r.dz != 0.0f ? __fdividef(1.0f, r.dz) : INFINITY;
+    // S3: slab test against the box; padded by 2 lattice indices on both sides
+    float t0 = 0.0f, t1 = INFINITY;
+    bool miss = false;
+    const float o[3] = {r.ox, r.oy, r.oz}, d[3] = {r.dx, r.dy, r.dz}, id[3] = {r.ix, r.iy, r.iz};
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        if (d[i] == 0.0f) {
+            if (o[i] < 0.0f || o[i] > sc.box[i]) miss = true;
+        } else {
+            const float ta = (0.0f - o[i]) * id[i], tb = (sc.box[i] - o[i]) * id[i];
+            t0 = fmaxf(t0, fminf(ta, tb));
+            t1 = fminf(t1, fmaxf(ta, tb));
+        }
+    }
+    if (miss || !(t0 <= t1 * 1.0001f + 1e-3f)) return false; // slack far below the 2-index padding
+    const float fa = floorf(t0 * sc.inv_step - 0.5f) - 2.0f;
+    const float fb = ceilf(t1 * sc.inv_step - 0.5f) + 2.0f;
+    k = fa > 0.0f ? (int)fminf(fa, 1.0e9f) : 0;
+    k1 = (int)fminf(fb, 1.0e9f);
+    return k <= k1;
+}
+
+// ---------------------------------------------------------------------------------- the persistent kernel
 template <int SAMPLER>
 __global__ void __launch_bounds__(128)
-omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__restrict__ cams, int W, int H,
-                   float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
+omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__restrict__ cams, int n_views, int W, int H,
+                   float *__restrict__ out_rgb, uint32_t *__restrict__ out_n, unsigned int *__restrict__ tile_counter)
 {
-    // block = 16x8 pixels, warp = 8x4 tile
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int u = blockIdx.x * 16 + (warp & 1) * 8 + (lane & 7);
-    const int v = blockIdx.y * 8 + (warp >> 1) * 4 + (lane >> 3);
-    const int view = blockIdx.z;
-    const bool valid = u < W && v < H;
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const int tiles_x = (W + 7) >> 3, tiles_y = (H + 3) >> 2;
+    const unsigned tiles_per_view = (unsigned)tiles_x * tiles_y;
+    const unsigned total_tiles = tiles_per_view * (unsigned)n_views;
+    const int start_lvl = (SAMPLER == OMERF_SAMPLER_PLANE ? sc.n_levels : sc.occ_levels) - 1;
 
-    // S2: ray (R19) — every step one correctly rounded fp32 operation
-    const omerf_camera cam = cams[view];
+    // lane state
+    int status = ST_IDLE;
     Ray r;
-    {
-        const float a = __fdiv_rn(__fsub_rn(__fadd_rn(__int2float_rn(u), 0.5f), cam.cx), cam.fx);
-        const float b = -__fdiv_rn(__fsub_rn(__fadd_rn(__int2float_rn(v), 0.5f), cam.cy), cam.fy);
-        const float gx = __fmaf_rn(a, cam.right[0], __fmaf_rn(b, cam.up[0], cam.fwd[0]));
-        const float gy = __fmaf_rn(a, cam.right[1], __fmaf_rn(b, cam.up[1], cam.fwd[1]));
-        const float gz = __fmaf_rn(a, cam.right[2], __fmaf_rn(b, cam.up[2], cam.fwd[2]));
-        const float len2 = __fmaf_rn(gx, gx, __fmaf_rn(gy, gy, __fmul_rn(gz, gz)));
-        const float inv = __fdiv_rn(1.0f, __fsqrt_rn(len2));
-        r.ox = cam.origin[0];
-        r.oy = cam.origin[1];
-        r.oz = cam.origin[2];
-        r.dx = __fmul_rn(gx, inv);
-        r.dy = __fmul_rn(gy, inv);
-        r.dz = __fmul_rn(gz, inv);
-    }
+    int k = 0, k1 = -1, lvl = 0;
+    uint32_t Q = 0, n = 0;
+    float acc[7];
+    size_t pix = 0;
+    // warp state
+    unsigned tile = 0;
+    int tpos = 32;
+    bool more = true;
 
-    // S3: clip to the box, padded by 2 lattice indices on both sides (the exact predicate decides)
-    int k = 0, k1 = -1;
-    {
-        float t0 = 0.0f, t1 = INFINITY;
-        bool miss = false;
-        const float o[3] = {r.ox, r.oy, r.oz}, d[3] = {r.dx, r.dy, r.dz};
-#pragma unroll
-        for (int i = 0; i < 3; i++) {
-            if (d[i] == 0.0f) {
-                if (o[i] < 0.0f || o[i] > sc.box[i]) miss = true;
-            } else {
-                float a = (0.0f - o[i]) / d[i], b = (sc.box[i] - o[i]) / d[i];
-                t0 = fmaxf(t0, fminf(a, b));
-                t1 = fminf(t1, fmaxf(a, b));
+    while (true) {
+        unsigned m_fin = __ballot_sync(FULL, status == ST_FIN);
+        unsigned m_busy = __ballot_sync(FULL, status == ST_TRAV || status == ST_READY);
+        // (1) retire: deferred MLP + outputs for finished rays (S8, S9)
+        if (m_fin && (__popc(m_fin) >= OMERF_RETIRE_T || !m_busy)) {
+            if (status == ST_FIN) {
+                float S[3];
+                deferred_mlp(sc, acc, r, S);
+                const float T_end = __expf(-(float)Q * (1.0f / 1048576.0f));
+                out_rgb[pix * 3 + 0] = __saturatef(acc[0] + S[0] + T_end * sc.bg[0]);
+                out_rgb[pix * 3 + 1] = __saturatef(acc[1] + S[1] + T_end * sc.bg[1]);
+                out_rgb[pix * 3 + 2] = __saturatef(acc[2] + S[2] + T_end * sc.bg[2]);
+                out_n[pix] = n;
+                status = ST_IDLE;
             }
         }
-        // relative slack for the fp32 slab test, far below the 2-index padding
-        if (!miss && t0 <= t1 * 1.0001f + 1e-3f && valid) {
-            float fa = floorf(t0 * sc.inv_step - 0.5f) - 2.0f;
-            float fb = ceilf(t1 * sc.inv_step - 0.5f) + 2.0f;
-            k = fa > 0.0f ? (int)fminf(fa, 1.0e9f) : 0;
-            k1 = (int)fminf(fb, 1.0e9f);
+        // (2) refill: idle lanes take the next pixels of the current 8x4 tile
+        unsigned m_idle = __ballot_sync(FULL, status == ST_IDLE);
+        if (more && (__popc(m_idle) >= OMERF_REFILL_T || !m_busy)) {
+            while (true) {
+                if (tpos >= 32) {
+                    unsigned t = 0;
+                    if (lane == 0) t = atomicAdd(tile_counter, 1u);
+                    tile = __shfl_sync(FULL, t, 0);
+                    tpos = 0;
+                    if (tile >= total_tiles) {
+                        more = false;
+                        break;
+                    }
+                }
+                m_idle = __ballot_sync(FULL, status == ST_IDLE);
+                if (!m_idle) break;
+                const int slot = tpos + __popc(m_idle & lt_mask);
+                const bool take = status == ST_IDLE && slot < 32;
+                if (take) {
+                    const unsigned view = tile / tiles_per_view, tv = tile - view * tiles_per_view;
+                    const int ty = (int)(tv / (unsigned)tiles_x), tx = (int)(tv - (unsigned)ty * tiles_x);
+                    const int u = tx * 8 + (slot & 7), v = ty * 4 + (slot >> 3);
+                    if (u < W && v < H) {
+                        const omerf_camera cam = cams[view];
+                        pix = ((size_t)view * H + v) * W + u;
+                        if (setup_ray(sc, cam, u, v, r, k, k1)) {
+                            status = ST_TRAV;
+                            lvl = start_lvl;
+                            Q = 0;
+                            n = 0;
+#pragma unroll
+                            for (int c = 0; c < 7; c++) acc[c] = 0.0f;
+                        } else { // cannot hit the box: background (R14)
+                            out_rgb[pix * 3 + 0] = sc.bg[0];
+                            out_rgb[pix * 3 + 1] = sc.bg[1];
+                            out_rgb[pix * 3 + 2] = sc.bg[2];
+                            out_n[pix] = 0;
+                        }
+                    }
+                }
+                tpos += min(__popc(m_idle), 32 - tpos);
+            }
+        }
+        if (!__any_sync(FULL, status != ST_IDLE)) {
+            if (!more) break;
+            continue;
+        }
+        // (3) one traversal step for rays in empty space / between samples (S4)
+        if (status == ST_TRAV) {
+            status = SAMPLER == OMERF_SAMPLER_PLANE ? trav_step_plane(sc, r, k, k1, lvl) : trav_step_grid(sc, r, k, k1, lvl);
+            if (status == ST_FIN && n == 0) { // no sample at all: background exactly, MLP skipped (R14)
+                out_rgb[pix * 3 + 0] = sc.bg[0];
+                out_rgb[pix * 3 + 1] = sc.bg[1];
+                out_rgb[pix * 3 + 2] = sc.bg[2];
+                out_n[pix] = 0;
+                status = ST_IDLE;
+            }
+        }
+        // (4) one sample for rays that stand on an occupied lattice point (S5, S6, S7)
+        const unsigned m_ready = __ballot_sync(FULL, status == ST_READY);
+        const unsigned m_trav = __ballot_sync(FULL, status == ST_TRAV);
+        if (m_ready && (__popc(m_ready) >= OMERF_SAMPLE_T || !m_trav)) {
+            if (status == ST_READY) {
+                float px, py, pz;
+                lattice_point(r, sc.step, k, px, py, pz);
+                uint32_t I[8];
+                gather_features(sc, px, py, pz, I);
+                float t[8];
+#pragma unroll
+                for (int c = 0; c < 8; c++) t[c] = __fmaf_rn(__uint2float_rn(I[c]), sc.deq_mul, sc.deq_add);
+                const float tau = exp_q(t[0]); // decision path
+                const float od = __fmul_rn(tau, sc.step);
+                const uint32_t qk = (uint32_t)rintf(fminf(__fmul_rn(od, 1048576.0f), (float)sc.q_stop));
+                const float T = __expf(-(float)Q * (1.0f / 1048576.0f)); // colour path: fast math
+                const float wgt = T * (1.0f - __expf(-od));
+#pragma unroll
+                for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, sigmoid_fast(t[1 + c]), acc[c]);
+                Q += qk;
+                n += 1;
+                k += 1;
+                if (Q >= sc.q_stop) {
+                    status = ST_FIN; // early stop (R7)
+                } else {
+                    // inside the slab the next lattice point is usually occupied too: test it here (level 0)
+                    // instead of paying a traversal round for it
+                    status = ST_TRAV;
+                    lvl = 0;
+                    if (SAMPLER == OMERF_SAMPLER_PLANE && k <= k1) {
+                        lattice_point(r, sc.step, k, px, py, pz);
+                        const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
+                        const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
+                        if (h.x <= pz && pz <= h.y && in_box(sc, px, py, pz)) status = ST_READY;
+                    }
+                }
+            }
         }
     }
-
-    uint32_t Q = 0, n = 0;
-    float acc[7] = {0, 0, 0, 0, 0, 0, 0};
-    int lvl = (SAMPLER == OMERF_SAMPLER_PLANE ? sc.n_levels : sc.occ_levels) - 1;
-    bool alive = k <= k1;
-    while (true) {
-        float px, py, pz;
-        bool have = false;
-        if (alive) {
-            have = SAMPLER == OMERF_SAMPLER_PLANE ? next_sample_plane(sc, r, k, k1, lvl, px, py, pz)
-                                                  : next_sample_grid(sc, r, k, k1, lvl, px, py, pz);
-            alive = have;
-        }
-        if (!__any_sync(0xffffffffu, have)) break;
-        if (have) {
-            uint32_t I[8];
-            gather_features(sc, px, py, pz, I);                                  // S5
-            float t[8];
-#pragma unroll
-            for (int c = 0; c < 8; c++) t[c] = __fmaf_rn(__uint2float_rn(I[c]), sc.deq_mul, sc.deq_add);
-            const float tau = exp_q(t[0]);                                        // S6, decision path
-            const float od = __fmul_rn(tau, sc.step);
-            const uint32_t qk = (uint32_t)rintf(fminf(__fmul_rn(od, 1048576.0f), (float)sc.q_stop));
-            const float T = __expf(-(float)Q * (1.0f / 1048576.0f));              // S7 (colour path: fast math)
-            const float wgt = T * (1.0f - __expf(-od));
-#pragma unroll
-            for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, sigmoid_fast(t[1 + c]), acc[c]);
-            Q += qk;
-            n += 1;
-            k += 1;
-            if (Q >= sc.q_stop) alive = false;                                    // early stop (R7)
-        }
-    }
-
-    if (!valid) return;
-    float rgb[3] = {sc.bg[0], sc.bg[1], sc.bg[2]};
-    if (n > 0) {
-        float S[3];
-        deferred_mlp(sc, acc, r, S);                                              // S8
-        const float T_end = __expf(-(float)Q * (1.0f / 1048576.0f));
-#pragma unroll
-        for (int c = 0; c < 3; c++) rgb[c] = __saturatef(acc[c] + S[c] + T_end * sc.bg[c]);
-    }
-    const size_t pix = ((size_t)view * H + v) * W + u;                            // S9
-    out_rgb[pix * 3 + 0] = rgb[0];
-    out_rgb[pix * 3 + 1] = rgb[1];
-    out_rgb[pix * 3 + 2] = rgb[2];
-    out_n[pix] = n;
 }
 
 } // namespace
@@ -424,16 +520,33 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H, float *out_rgb,
                         uint32_t *out_n, cudaStream_t st, int *launches)
 {
-    dim3 blk(128), grd((W + 15) / 16, (H + 7) / 8, n_views);
-    if (grd.y > 65535u || grd.z > 65535u) {
+    if ((long long)((W + 7) / 8) * ((H + 3) / 4) * n_views > 0x7fffffffll) {
         omerf_set_error("invalid argument: image or batch too large");
         return OMERF_ERR_INVALID;
     }
+    OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, sizeof(unsigned int), st));
+    const int grid = s->persistent_blocks;
     if (s->dev.sampler == OMERF_SAMPLER_PLANE)
-        omerf_march_kernel<OMERF_SAMPLER_PLANE><<<grd, blk, 0, st>>>(s->dev, d_cams, W, H, out_rgb, out_n);
+        omerf_march_kernel<OMERF_SAMPLER_PLANE><<<grid, 128, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,
+                                                                       s->d_tile_counter);
     else
-        omerf_march_kernel<OMERF_SAMPLER_GRID><<<grd, blk, 0, st>>>(s->dev, d_cams, W, H, out_rgb, out_n);
+        omerf_march_kernel<OMERF_SAMPLER_GRID><<<grid, 128, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,
+                                                                      s->d_tile_counter);
     *launches = 1;
     OMERF_CUDA(cudaGetLastError());
+    return OMERF_OK;
+}
+
+// resident blocks of the march kernel on this device: the persistent grid size
+int omerf_query_persistent_blocks(int sampler, int *blocks)
+{
+    int dev = 0, sms = 0, per_sm = 0;
+    OMERF_CUDA(cudaGetDevice(&dev));
+    OMERF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (sampler == OMERF_SAMPLER_PLANE)
+        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_PLANE>, 128, 0));
+    else
+        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_GRID>, 128, 0));
+    *blocks = sms * (per_sm > 0 ? per_sm : 1);
     return OMERF_OK;
 }
