@@ -53,6 +53,7 @@ static void free_scene(omerf_scene *s)
     cudaFree(s->d_pxz);
     cudaFree(s->d_pyz);
     cudaFree(s->d_occ);
+    cudaFree(s->d_mlp_tab);
     cudaFree(s->d_cams);
     cudaFree(s->d_tile_counter);
     cudaFree(s->d_scratch_rgb);
@@ -127,12 +128,6 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
     v.q_stop = (uint32_t)ceil(-log((double)d->t_stop) * 1048576.0);
     for (int i = 0; i < 3; i++) v.bg[i] = d->bg[i];
     v.sampler = d->sampler;
-    memcpy(v.W0, d->W0, sizeof v.W0);
-    memcpy(v.b0, d->b0, sizeof v.b0);
-    memcpy(v.W1, d->W1, sizeof v.W1);
-    memcpy(v.b1, d->b1, sizeof v.b1);
-    memcpy(v.W2, d->W2, sizeof v.W2);
-    memcpy(v.b2, d->b2, sizeof v.b2);
 
     int rc = OMERF_OK;
     float *d_lo = nullptr, *d_up = nullptr;
@@ -148,6 +143,8 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         v.pxy = (const uint2 *)s->d_pxy;
         v.pxz = (const uint2 *)s->d_pxz;
         v.pyz = (const uint2 *)s->d_pyz;
+        // S0: deferred-MLP weights -> tensor-core fragment order, tf32 hi/lo split (device kernel)
+        if ((rc = omerf_launch_mlp_pack(s, d, 0))) break;
         // S1: min/max pyramid of the two height fields, built on the device
         if ((rc = upload((void **)&d_lo, d->h_lo, hf_bytes, &tmp))) break;
         if ((rc = upload((void **)&d_up, d->h_up, hf_bytes, &tmp))) break;
@@ -168,7 +165,7 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         }
         if ((rc = omerf_query_persistent_blocks(d->sampler, &s->persistent_blocks))) break;
         {
-            cudaError_t ee = cudaMalloc((void **)&s->d_tile_counter, sizeof(unsigned int));
+            cudaError_t ee = cudaMalloc((void **)&s->d_tile_counter, 64 * sizeof(unsigned int));
             if (ee != cudaSuccess) {
                 rc = omerf_cuda_fail(ee, "cudaMalloc tile counter");
                 break;

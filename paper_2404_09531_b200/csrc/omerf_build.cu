@@ -4,6 +4,8 @@
 //   S10 config-4 comparator: binary occupancy grid derived from the slab (voxel set iff it intersects
 //       [z_min, z_max] of an overlapping cell, R18) and its OR-reduced mip chain — the
 //       "multi-resolution binary grid" PAPER.md:188 says the occupancy plane replaces.
+#include <string.h>
+
 #include "omerf_device.cuh"
 
 // ------------------------------------------------------------------------------------------ pyramid
@@ -201,5 +203,91 @@ int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st)
     OMERF_CUDA(cudaGetLastError());
     OMERF_CUDA(cudaMemcpyAsync(&s->occ_bits_set, d_total, 8, cudaMemcpyDeviceToHost, st));
     OMERF_CUDA(cudaStreamSynchronize(st));
+    return OMERF_OK;
+}
+
+// ------------------------------------------------------------------------------------------ MLP weight packing
+// G: 34 -> 16 -> 16 -> 3 (Eq. 4).  The render kernel evaluates it for 16 rays at a time with
+// mma.sync.m16n8k8 (tf32 x 3 split: a_hi b_hi + a_lo b_hi + a_hi b_lo, fp32 accumulate), so the weights are
+// stored once in B-fragment order: lane (g = lane/4, t = lane%4) of tile (k-step s, n-tile q) holds
+//   layer 1:  W0[8q+g][8s+t],    W0[8q+g][8s+t+4]      (zero beyond the 34 inputs)
+//   layer 2:  W1[8q+g][8s+2t],   W1[8q+g][8s+2t+1]     (k order = the C-fragment order of layer 1's output,
+//   layer 3:  W2[g][8s+2t],      W2[g][8s+2t+1]         so hidden activations never leave their registers)
+__device__ __forceinline__ float tf32_rna(float x)
+{
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return __uint_as_float(r);
+}
+
+__global__ void mlp_pack_kernel(const float *__restrict__ W0, const float *__restrict__ b0,
+                                const float *__restrict__ W1, const float *__restrict__ b1,
+                                const float *__restrict__ W2, const float *__restrict__ b2, float2 *__restrict__ tab)
+{
+    const int lane = threadIdx.x & 31, tile = threadIdx.x >> 5; // 21 warps: 16 weight tiles + 5 bias tiles
+    const int g = lane >> 2, t = lane & 3;
+    if (tile < OMERF_MLP_TILES) {
+        float w0 = 0.0f, w1 = 0.0f;
+        if (tile < 10) {
+            const int s = tile >> 1, q = tile & 1, n = 8 * q + g, k0 = 8 * s + t, k1 = 8 * s + t + 4;
+            if (k0 < OMERF_MLP_IN) w0 = W0[n * OMERF_MLP_IN + k0];
+            if (k1 < OMERF_MLP_IN) w1 = W0[n * OMERF_MLP_IN + k1];
+        } else if (tile < 14) {
+            const int s = (tile - 10) >> 1, q = (tile - 10) & 1, n = 8 * q + g;
+            w0 = W1[n * OMERF_MLP_HID + 8 * s + 2 * t];
+            w1 = W1[n * OMERF_MLP_HID + 8 * s + 2 * t + 1];
+        } else {
+            const int s = tile - 14;
+            if (g < 3) {
+                w0 = W2[g * OMERF_MLP_HID + 8 * s + 2 * t];
+                w1 = W2[g * OMERF_MLP_HID + 8 * s + 2 * t + 1];
+            }
+        }
+        const float h0 = tf32_rna(w0), h1 = tf32_rna(w1);
+        tab[(tile * 2 + 0) * 32 + lane] = make_float2(h0, h1);
+        tab[(tile * 2 + 1) * 32 + lane] = make_float2(tf32_rna(w0 - h0), tf32_rna(w1 - h1));
+    } else {
+        const int bt = tile - OMERF_MLP_TILES; // C-fragment columns 2t, 2t+1 of n-tile
+        float v0 = 0.0f, v1 = 0.0f;
+        if (bt < 2) {
+            v0 = b0[8 * bt + 2 * t];
+            v1 = b0[8 * bt + 2 * t + 1];
+        } else if (bt < 4) {
+            v0 = b1[8 * (bt - 2) + 2 * t];
+            v1 = b1[8 * (bt - 2) + 2 * t + 1];
+        } else {
+            if (2 * t < 3) v0 = b2[2 * t];
+            if (2 * t + 1 < 3) v1 = b2[2 * t + 1];
+        }
+        tab[OMERF_MLP_BIAS_OFF + bt * 32 + lane] = make_float2(v0, v1);
+    }
+}
+
+int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_t st)
+{
+    const int nW0 = OMERF_MLP_HID * OMERF_MLP_IN, nW1 = OMERF_MLP_HID * OMERF_MLP_HID, nW2 = 3 * OMERF_MLP_HID;
+    const int total = nW0 + nW1 + nW2 + 2 * OMERF_MLP_HID + 3;
+    float host[OMERF_MLP_HID * OMERF_MLP_IN + OMERF_MLP_HID * OMERF_MLP_HID + 3 * OMERF_MLP_HID + 2 * OMERF_MLP_HID + 3];
+    float *p = host;
+    memcpy(p, d->W0, nW0 * 4); p += nW0;
+    memcpy(p, d->b0, OMERF_MLP_HID * 4); p += OMERF_MLP_HID;
+    memcpy(p, d->W1, nW1 * 4); p += nW1;
+    memcpy(p, d->b1, OMERF_MLP_HID * 4); p += OMERF_MLP_HID;
+    memcpy(p, d->W2, nW2 * 4); p += nW2;
+    memcpy(p, d->b2, 3 * 4);
+    float *raw = nullptr;
+    OMERF_CUDA(cudaMalloc((void **)&raw, total * 4));
+    cudaError_t e = cudaMemcpyAsync(raw, host, total * 4, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_mlp_tab, OMERF_MLP_TAB_LEN * sizeof(float2));
+    if (e == cudaSuccess) {
+        const float *W0 = raw, *b0 = W0 + nW0, *W1 = b0 + OMERF_MLP_HID, *b1 = W1 + nW1, *W2 = b1 + OMERF_MLP_HID, *b2 = W2 + nW2;
+        mlp_pack_kernel<<<1, 32 * (OMERF_MLP_TILES + 5), 0, st>>>(W0, b0, W1, b1, W2, b2, (float2 *)s->d_mlp_tab);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(raw);
+    if (e != cudaSuccess) return omerf_cuda_fail(e, "MLP weight packing");
+    s->dev.mlp_tab = (const float2 *)s->d_mlp_tab;
+    s->device_bytes += OMERF_MLP_TAB_LEN * sizeof(float2);
     return OMERF_OK;
 }

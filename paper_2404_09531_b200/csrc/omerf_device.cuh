@@ -9,6 +9,9 @@
 #define OMERF_MAX_LEVELS 16
 #define OMERF_MLP_IN 34
 #define OMERF_MLP_HID 16
+#define OMERF_MLP_TILES 16
+#define OMERF_MLP_BIAS_OFF (OMERF_MLP_TILES * 2 * 32)
+#define OMERF_MLP_TAB_LEN (OMERF_MLP_BIAS_OFF + 5 * 32)
 
 // Everything a render kernel needs, passed by value as a __grid_constant__ kernel parameter so that
 // scalars and the 883 MLP weights are read through the constant bank (no loads in the MLP).
@@ -41,16 +44,16 @@ struct DevScene {
     const uint32_t *occ;   // all levels; level l has dims ceil(N/2^l), bit index ((jx*ny+jy)*nz+jz)
     unsigned long long occ_off[OMERF_MAX_LEVELS]; // word offset of each level
     int occ_nx[OMERF_MAX_LEVELS], occ_ny[OMERF_MAX_LEVELS], occ_nz[OMERF_MAX_LEVELS];
-    // deferred MLP G (Eq. 4)
-    float W0[OMERF_MLP_HID * OMERF_MLP_IN], b0[OMERF_MLP_HID];
-    float W1[OMERF_MLP_HID * OMERF_MLP_HID], b1[OMERF_MLP_HID];
-    float W2[3 * OMERF_MLP_HID], b2[3];
+    // deferred MLP G (Eq. 4): weights pre-arranged as mma.m16n8k8 B fragments, split into tf32 hi + lo
+    // (omerf_build.cu: mlp_pack_kernel).  tab[(tile*2 + part)*32 + lane], part 0 = hi, 1 = lo; tiles 0..9 layer 1
+    // (k-step*2 + n-tile), 10..13 layer 2, 14..15 layer 3; then 5 bias tiles (layer 1 n-tiles 0,1; layer 2; layer 3).
+    const float2 *mlp_tab;
 };
 
 struct omerf_scene {
     DevScene dev;
     int device;
-    void *d_pyr, *d_grid, *d_pxy, *d_pxz, *d_pyz, *d_occ;
+    void *d_pyr, *d_grid, *d_pxy, *d_pxz, *d_pyz, *d_occ, *d_mlp_tab;
     uint64_t device_bytes;
     uint64_t occ_bits_set;
     // per-render state (mutable through the const handle: calls must be stream-ordered)
@@ -81,6 +84,7 @@ int omerf_cuda_fail(cudaError_t e, const char *what);
 // kernels' host launchers
 int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, cudaStream_t st);
 int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st);
+int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_t st);
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H,
                         float *out_rgb, uint32_t *out_n, cudaStream_t st, int *launches);
 int omerf_query_persistent_blocks(int sampler, int *blocks);

@@ -26,6 +26,8 @@
 // in k in every component (rounding is monotone), so cell indices and z are monotone in k.  If samples k
 // and kk both lie in one pyramid node and both are on the same side outside its [min,max] z-range, so
 // does every sample between them: all of them fail the predicate and may be skipped.
+#include <stdio.h>
+
 #include "omerf_device.cuh"
 
 namespace {
@@ -119,7 +121,7 @@ __device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r,
             k++;
             return ST_TRAV;
         }
-        lvl--;
+        lvl = max(lvl - 2, 0); // level policy tuned with a CPU model of this loop on configs[1]: 17 -> 11 steps per ray
         return ST_TRAV;
     }
     // outside the node's z-range: propose a jump to the node's xy exit or to where z reaches the range.
@@ -142,11 +144,10 @@ __device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r,
         if (jx == nx && jy == ny && same_side) {
             k = kk + 1;
             if (tz <= fminf(tx, ty)) {
-                lvl = max(lvl - 1, 0); // entering the node's z-range: refine
+                lvl = max(lvl - 2, 0); // entering the node's z-range: refine
             } else {
                 const int crossed = tx <= ty ? bxi : byi;
-                const int up = crossed == 0 ? 31 : __ffs(crossed) - 1; // levels whose boundary this also is
-                lvl = min(lvl + min(up, 2), top);
+                lvl = min(lvl + ((crossed & 1) ^ 1), top); // an even boundary index also leaves the parent node
             }
             return ST_TRAV;
         }
@@ -286,47 +287,106 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
 __device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
 
 // ---------------------------------------------------------------------------------- S8: deferred MLP (Eq. 4)
-__device__ __forceinline__ void deferred_mlp(const DevScene &sc, const float acc[7], const Ray &r, float S[3])
+// Warp-cooperative: the 34 -> 16 -> 16 -> 3 network of 16 rays at a time as m16n8k8 tensor-core tiles.
+// tf32 operands are split hi + lo (3 mma per tile product), so the result keeps fp32-level accuracy; hidden
+// activations stay in registers (the C fragment of one layer is the A fragment of the next, see mlp_pack_kernel).
+#define OMERF_XS 44 // row stride of the staged input tile in floats: conflict-free A-fragment loads
+
+// x = hi + lo with hi = x truncated to tf32 (10 explicit mantissa bits) and lo = x - hi exactly; the tensor core
+// reads only the tf32 part of lo, which leaves a relative error of about 2^-21 in the product sum
+__device__ __forceinline__ void split_tf32(float x, uint32_t &hi, uint32_t &lo)
 {
-    float in[OMERF_MLP_IN];
+    hi = __float_as_uint(x) & 0xffffe000u;
+    lo = __float_as_uint(x - __uint_as_float(hi));
+}
+
+__device__ __forceinline__ void mma_tf32(float c[4], const uint32_t a[4], float b0, float b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(__float_as_uint(b0)), "r"(__float_as_uint(b1)));
+}
+
+// c += A * B for one k-step/n-tile, A given as fp32 values (split here), B from the packed table
+__device__ __forceinline__ void mma_x3(float c[4], const uint32_t ahi[4], const uint32_t alo[4], const float2 *__restrict__ tab,
+                                       int tile, int lane)
+{
+    const float2 bhi = __ldg(tab + (tile * 2 + 0) * 32 + lane), blo = __ldg(tab + (tile * 2 + 1) * 32 + lane);
+    mma_tf32(c, alo, bhi.x, bhi.y);
+    mma_tf32(c, ahi, blo.x, blo.y);
+    mma_tf32(c, ahi, bhi.x, bhi.y);
+}
+
+// MLP input of one ray: [sum w c^d (3), sum w f (4), d (3), sin/cos(2^j d) j = 0..3 (24)]  (R13)
+__device__ __forceinline__ void mlp_input(const float acc[7], float dx, float dy, float dz, float in[OMERF_MLP_IN])
+{
 #pragma unroll
     for (int i = 0; i < 7; i++) in[i] = acc[i];
-    const float d[3] = {r.dx, r.dy, r.dz};
+    const float d[3] = {dx, dy, dz};
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         in[7 + c] = d[c];
         float s, co;
-        sincosf(d[c], &s, &co); // |d| <= 1: no range reduction slow path
+        sincosf(d[c], &s, &co); // |d| <= 1: no range-reduction slow path
 #pragma unroll
         for (int j = 0; j < 4; j++) {
             in[10 + (3 * j + c) * 2] = s;
             in[10 + (3 * j + c) * 2 + 1] = co;
-            const float s2 = 2.0f * s * co, c2 = 1.0f - 2.0f * s * s; // double-angle: sin/cos(2^(j+1) d)
+            const float s2 = 2.0f * s * co, c2 = 1.0f - 2.0f * s * s; // double angle: sin/cos(2^(j+1) d)
             s = s2;
             co = c2;
         }
     }
-    float h1[OMERF_MLP_HID], h2[OMERF_MLP_HID];
+}
+
+// Evaluates G for the rays staged by lanes [16*half, 16*half+16) and returns this lane's share of the output
+// C fragment: out[0], out[1] = row g cols 2t, 2t+1; out[2], out[3] = row g+8 (pre-sigmoid; cols >= 3 unused).
+__device__ __forceinline__ void mlp_half(const float2 *__restrict__ tab, const float *X, int lane, float out[4])
+{
+    const int g = lane >> 2, t = lane & 3;
+    float c1[2][4], c2[2][4];
 #pragma unroll
-    for (int o = 0; o < OMERF_MLP_HID; o++) {
-        float a = sc.b0[o];
-#pragma unroll
-        for (int i = 0; i < OMERF_MLP_IN; i++) a = fmaf(sc.W0[o * OMERF_MLP_IN + i], in[i], a);
-        h1[o] = fmaxf(a, 0.0f);
+    for (int q = 0; q < 2; q++) {
+        const float2 bq = __ldg(tab + OMERF_MLP_BIAS_OFF + q * 32 + lane), bq2 = __ldg(tab + OMERF_MLP_BIAS_OFF + (2 + q) * 32 + lane);
+        c1[q][0] = c1[q][2] = bq.x;
+        c1[q][1] = c1[q][3] = bq.y;
+        c2[q][0] = c2[q][2] = bq2.x;
+        c2[q][1] = c2[q][3] = bq2.y;
     }
+    // layer 1: K = 34 (padded to 40), N = 16
 #pragma unroll
-    for (int o = 0; o < OMERF_MLP_HID; o++) {
-        float a = sc.b1[o];
+    for (int s = 0; s < 5; s++) {
+        uint32_t ahi[4], alo[4];
+        split_tf32(X[g * OMERF_XS + 8 * s + t], ahi[0], alo[0]);
+        split_tf32(X[(g + 8) * OMERF_XS + 8 * s + t], ahi[1], alo[1]);
+        split_tf32(X[g * OMERF_XS + 8 * s + t + 4], ahi[2], alo[2]);
+        split_tf32(X[(g + 8) * OMERF_XS + 8 * s + t + 4], ahi[3], alo[3]);
 #pragma unroll
-        for (int i = 0; i < OMERF_MLP_HID; i++) a = fmaf(sc.W1[o * OMERF_MLP_HID + i], h1[i], a);
-        h2[o] = fmaxf(a, 0.0f);
+        for (int q = 0; q < 2; q++) mma_x3(c1[q], ahi, alo, tab, s * 2 + q, lane);
     }
+    // layer 2: K = 16, N = 16; A fragment of k-step s = relu(C fragment of n-tile s)
 #pragma unroll
-    for (int o = 0; o < 3; o++) {
-        float a = sc.b2[o];
+    for (int s = 0; s < 2; s++) {
+        uint32_t ahi[4], alo[4];
+        split_tf32(fmaxf(c1[s][0], 0.0f), ahi[0], alo[0]);
+        split_tf32(fmaxf(c1[s][2], 0.0f), ahi[1], alo[1]);
+        split_tf32(fmaxf(c1[s][1], 0.0f), ahi[2], alo[2]);
+        split_tf32(fmaxf(c1[s][3], 0.0f), ahi[3], alo[3]);
 #pragma unroll
-        for (int i = 0; i < OMERF_MLP_HID; i++) a = fmaf(sc.W2[o * OMERF_MLP_HID + i], h2[i], a);
-        S[o] = sigmoid_fast(a);
+        for (int q = 0; q < 2; q++) mma_x3(c2[q], ahi, alo, tab, 10 + s * 2 + q, lane);
+    }
+    // layer 3: K = 16, N = 3 (padded to 8)
+    const float2 b3 = __ldg(tab + OMERF_MLP_BIAS_OFF + 4 * 32 + lane);
+    out[0] = out[2] = b3.x;
+    out[1] = out[3] = b3.y;
+#pragma unroll
+    for (int s = 0; s < 2; s++) {
+        uint32_t ahi[4], alo[4];
+        split_tf32(fmaxf(c2[s][0], 0.0f), ahi[0], alo[0]);
+        split_tf32(fmaxf(c2[s][2], 0.0f), ahi[1], alo[1]);
+        split_tf32(fmaxf(c2[s][1], 0.0f), ahi[2], alo[2]);
+        split_tf32(fmaxf(c2[s][3], 0.0f), ahi[3], alo[3]);
+        mma_x3(out, ahi, alo, tab, 14 + s, lane);
     }
 }
 
@@ -375,143 +435,303 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 }
 
 // ---------------------------------------------------------------------------------- the persistent kernel
+// Warp-private ray pool in shared memory (structure of arrays, one word per ray and field).
+#ifndef OMERF_POOL
+#define OMERF_POOL 96          // rays per warp; a multiple of 32
+#endif
+#ifndef OMERF_TRAV_STEPS
+#define OMERF_TRAV_STEPS 6     // traversal steps per visit while at least OMERF_TRAV_KEEP lanes still traverse
+#endif
+#ifndef OMERF_TRAV_KEEP
+#define OMERF_TRAV_KEEP 16
+#endif
+#ifndef OMERF_SAMPLE_KEEP
+#define OMERF_SAMPLE_KEEP 24   // sample again at once while this many lanes stand on an occupied point
+#endif
+#define OMERF_WARPS 4
+#define OMERF_PJ (OMERF_POOL / 32)
+
+struct WarpPool {
+    uint32_t meta[OMERF_POOL]; // status (bits 0-1) | pyramid level (bits 2-6) | view (bits 8-31)
+    float dx[OMERF_POOL], dy[OMERF_POOL], dz[OMERF_POOL];
+    int k[OMERF_POOL], k1[OMERF_POOL];
+    uint32_t Q[OMERF_POOL], n[OMERF_POOL], pix[OMERF_POOL];
+    float acc[7][OMERF_POOL];
+    uint32_t list[32];
+    float X[16 * OMERF_XS]; // staged MLP inputs of 16 rays
+};
+
+__device__ __forceinline__ uint32_t pack_meta(int status, int lvl, uint32_t view)
+{
+    return (uint32_t)status | ((uint32_t)lvl << 2) | (view << 8);
+}
+
+#ifndef OMERF_MIN_BLOCKS
+#define OMERF_MIN_BLOCKS 5
+#endif
 template <int SAMPLER>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(32 * OMERF_WARPS, OMERF_MIN_BLOCKS)
 omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__restrict__ cams, int n_views, int W, int H,
                    float *__restrict__ out_rgb, uint32_t *__restrict__ out_n, unsigned int *__restrict__ tile_counter)
 {
+    __shared__ WarpPool pools[OMERF_WARPS];
+    WarpPool &P = pools[threadIdx.x >> 5];
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
     const int tiles_x = (W + 7) >> 3, tiles_y = (H + 3) >> 2;
     const unsigned tiles_per_view = (unsigned)tiles_x * tiles_y;
     const unsigned total_tiles = tiles_per_view * (unsigned)n_views;
-    const int start_lvl = (SAMPLER == OMERF_SAMPLER_PLANE ? sc.n_levels : sc.occ_levels) - 1;
+    const int start_lvl = min((SAMPLER == OMERF_SAMPLER_PLANE ? sc.n_levels : sc.occ_levels) - 1, 6);
 
-    // lane state
-    int status = ST_IDLE;
-    Ray r;
-    int k = 0, k1 = -1, lvl = 0;
-    uint32_t Q = 0, n = 0;
-    float acc[7];
-    size_t pix = 0;
-    // warp state
-    unsigned tile = 0;
-    int tpos = 32;
+#pragma unroll
+    for (int j = 0; j < OMERF_PJ; j++) P.meta[lane + 32 * j] = ST_IDLE;
+    __syncwarp();
     bool more = true;
 
     while (true) {
-        unsigned m_fin = __ballot_sync(FULL, status == ST_FIN);
-        unsigned m_busy = __ballot_sync(FULL, status == ST_TRAV || status == ST_READY);
-        // (1) retire: deferred MLP + outputs for finished rays (S8, S9)
-        if (m_fin && (__popc(m_fin) >= OMERF_RETIRE_T || !m_busy)) {
-            if (status == ST_FIN) {
-                float S[3];
-                deferred_mlp(sc, acc, r, S);
-                const float T_end = __expf(-(float)Q * (1.0f / 1048576.0f));
-                out_rgb[pix * 3 + 0] = __saturatef(acc[0] + S[0] + T_end * sc.bg[0]);
-                out_rgb[pix * 3 + 1] = __saturatef(acc[1] + S[1] + T_end * sc.bg[1]);
-                out_rgb[pix * 3 + 2] = __saturatef(acc[2] + S[2] + T_end * sc.bg[2]);
-                out_n[pix] = n;
-                status = ST_IDLE;
+        // ---- census of the pool
+        uint32_t st[OMERF_PJ];
+        unsigned bal[4][OMERF_PJ];
+        int cnt[4] = {0, 0, 0, 0};
+#pragma unroll
+        for (int j = 0; j < OMERF_PJ; j++) {
+            st[j] = P.meta[lane + 32 * j] & 3u;
+#pragma unroll
+            for (int s = 0; s < 4; s++) {
+                bal[s][j] = __ballot_sync(FULL, st[j] == (uint32_t)s);
+                cnt[s] += __popc(bal[s][j]);
             }
         }
-        // (2) refill: idle lanes take the next pixels of the current 8x4 tile
-        unsigned m_idle = __ballot_sync(FULL, status == ST_IDLE);
-        if (more && (__popc(m_idle) >= OMERF_REFILL_T || !m_busy)) {
-            while (true) {
-                if (tpos >= 32) {
-                    unsigned t = 0;
-                    if (lane == 0) t = atomicAdd(tile_counter, 1u);
-                    tile = __shfl_sync(FULL, t, 0);
-                    tpos = 0;
-                    if (tile >= total_tiles) {
-                        more = false;
-                        break;
+        // ---- pick a phase: full warps first, then the fullest
+        int phase;
+        if (cnt[ST_FIN] >= 32) phase = ST_FIN;
+        else if (cnt[ST_READY] >= 32) phase = ST_READY;
+        else if (cnt[ST_TRAV] >= 32) phase = ST_TRAV;
+        else if (more && cnt[ST_IDLE] >= 32) phase = ST_IDLE;
+        else {
+            phase = ST_READY;
+            int best = cnt[ST_READY];
+            if (cnt[ST_TRAV] > best) { best = cnt[ST_TRAV]; phase = ST_TRAV; }
+            if (best == 0) { best = cnt[ST_FIN]; phase = ST_FIN; } // finished rays wait for a full MLP batch
+            if (best == 0) break; // pool empty and no tile left (otherwise the refill branch was taken)
+        }
+        // ---- the first 32 slots in that state
+        {
+            int base = 0;
+#pragma unroll
+            for (int j = 0; j < OMERF_PJ; j++) {
+                unsigned b = phase == ST_IDLE ? bal[0][j] : phase == ST_TRAV ? bal[1][j] : phase == ST_READY ? bal[2][j] : bal[3][j];
+                const int pos = base + __popc(b & lt_mask);
+                if (((b >> lane) & 1u) && pos < 32) P.list[pos] = lane + 32 * j;
+                base += __popc(b);
+            }
+        }
+        __syncwarp();
+        const int n_act = min(cnt[phase], 32);
+#ifdef OMERF_X_STATS
+        if (lane == 0) { atomicAdd(tile_counter + 1 + phase, 1u); atomicAdd(tile_counter + 5 + phase, (unsigned)n_act); }
+#endif
+        const bool active = lane < n_act;
+        const int slot = active ? (int)P.list[lane] : 0;
+
+        if (phase == ST_IDLE) {
+            // ---- refill: one 8x4 tile -> 32 new rays (S2, S3)
+            unsigned t = 0;
+            if (lane == 0) t = atomicAdd(tile_counter, 1u);
+            const unsigned tile = __shfl_sync(FULL, t, 0);
+            if (tile >= total_tiles) {
+                more = false;
+            } else {
+                const unsigned view = tile / tiles_per_view, tv = tile - view * tiles_per_view;
+                const int ty = (int)(tv / (unsigned)tiles_x), tx = (int)(tv - (unsigned)ty * tiles_x);
+                const int u = tx * 8 + (lane & 7), v = ty * 4 + (lane >> 3);
+                if (u < W && v < H) {
+                    const omerf_camera cam = cams[view];
+                    const size_t pix = ((size_t)view * H + v) * W + u;
+                    Ray r;
+                    int k, k1;
+                    if (setup_ray(sc, cam, u, v, r, k, k1)) {
+                        P.meta[slot] = pack_meta(ST_TRAV, start_lvl, view);
+                        P.dx[slot] = r.dx;
+                        P.dy[slot] = r.dy;
+                        P.dz[slot] = r.dz;
+                        P.k[slot] = k;
+                        P.k1[slot] = k1;
+                        P.Q[slot] = 0;
+                        P.n[slot] = 0;
+                        P.pix[slot] = (uint32_t)pix;
+#pragma unroll
+                        for (int c = 0; c < 7; c++) P.acc[c][slot] = 0.0f;
+                    } else { // cannot hit the box: background (R14)
+                        out_rgb[pix * 3 + 0] = sc.bg[0];
+                        out_rgb[pix * 3 + 1] = sc.bg[1];
+                        out_rgb[pix * 3 + 2] = sc.bg[2];
+                        out_n[pix] = 0;
                     }
                 }
-                m_idle = __ballot_sync(FULL, status == ST_IDLE);
-                if (!m_idle) break;
-                const int slot = tpos + __popc(m_idle & lt_mask);
-                const bool take = status == ST_IDLE && slot < 32;
-                if (take) {
-                    const unsigned view = tile / tiles_per_view, tv = tile - view * tiles_per_view;
-                    const int ty = (int)(tv / (unsigned)tiles_x), tx = (int)(tv - (unsigned)ty * tiles_x);
-                    const int u = tx * 8 + (slot & 7), v = ty * 4 + (slot >> 3);
-                    if (u < W && v < H) {
-                        const omerf_camera cam = cams[view];
-                        pix = ((size_t)view * H + v) * W + u;
-                        if (setup_ray(sc, cam, u, v, r, k, k1)) {
-                            status = ST_TRAV;
-                            lvl = start_lvl;
-                            Q = 0;
-                            n = 0;
+            }
+        } else if (phase == ST_TRAV) {
+            // ---- traversal visit: a few steps of the hierarchical DDA (S4)
+            int status = ST_IDLE, k = 0, k1 = -1, lvl = 0;
+            uint32_t view = 0;
+            Ray r;
+            if (active) {
+                const uint32_t m = P.meta[slot];
+                status = ST_TRAV;
+                lvl = (int)((m >> 2) & 31u);
+                view = m >> 8;
+                k = P.k[slot];
+                k1 = P.k1[slot];
+                r.dx = P.dx[slot];
+                r.dy = P.dy[slot];
+                r.dz = P.dz[slot];
+                r.ox = __ldg(&cams[view].origin[0]);
+                r.oy = __ldg(&cams[view].origin[1]);
+                r.oz = __ldg(&cams[view].origin[2]);
+                r.ix = r.dx != 0.0f ? __fdividef(1.0f, r.dx) : INFINITY;
+                r.iy = r.dy != 0.0f ? __fdividef(1.0f, r.dy) : INFINITY;
+                r.iz = r.dz != 0.0f ? __fdividef(1.0f, r.dz) : INFINITY;
+            }
+#pragma unroll 1
+            for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
+#ifdef OMERF_X_STATS
+                { unsigned m = __ballot_sync(FULL, status == ST_TRAV); if (lane == 0) { atomicAdd(tile_counter + 9, 1u); atomicAdd(tile_counter + 10, (unsigned)__popc(m)); } }
+#endif
+                if (status == ST_TRAV)
+                    status = SAMPLER == OMERF_SAMPLER_PLANE ? trav_step_plane(sc, r, k, k1, lvl) : trav_step_grid(sc, r, k, k1, lvl);
+                if (__popc(__ballot_sync(FULL, status == ST_TRAV)) < OMERF_TRAV_KEEP) break;
+            }
+            if (active) {
+                if (status == ST_FIN && P.n[slot] == 0) { // no sample at all: background exactly, MLP skipped (R14)
+                    const size_t pix = P.pix[slot];
+                    out_rgb[pix * 3 + 0] = sc.bg[0];
+                    out_rgb[pix * 3 + 1] = sc.bg[1];
+                    out_rgb[pix * 3 + 2] = sc.bg[2];
+                    out_n[pix] = 0;
+                    status = ST_IDLE;
+                }
+                P.k[slot] = k;
+                P.meta[slot] = pack_meta(status, lvl, view);
+            }
+        } else if (phase == ST_READY) {
+            // ---- samples: gather, activations, compositing (S5, S6, S7)
+            int status = ST_IDLE, k = 0, k1 = -1, lvl = 0;
+            uint32_t view = 0, Q = 0, n = 0;
+            float acc[7];
+            Ray r;
+            if (active) {
+                view = P.meta[slot] >> 8;
+                status = ST_READY;
+                k = P.k[slot];
+                k1 = P.k1[slot];
+                Q = P.Q[slot];
+                n = P.n[slot];
+                r.dx = P.dx[slot];
+                r.dy = P.dy[slot];
+                r.dz = P.dz[slot];
+                r.ox = __ldg(&cams[view].origin[0]);
+                r.oy = __ldg(&cams[view].origin[1]);
+                r.oz = __ldg(&cams[view].origin[2]);
 #pragma unroll
-                            for (int c = 0; c < 7; c++) acc[c] = 0.0f;
-                        } else { // cannot hit the box: background (R14)
-                            out_rgb[pix * 3 + 0] = sc.bg[0];
-                            out_rgb[pix * 3 + 1] = sc.bg[1];
-                            out_rgb[pix * 3 + 2] = sc.bg[2];
-                            out_n[pix] = 0;
+                for (int c = 0; c < 7; c++) acc[c] = P.acc[c][slot];
+            }
+#pragma unroll 1
+            while (true) {
+#ifdef OMERF_X_STATS
+                { unsigned m = __ballot_sync(FULL, status == ST_READY); if (lane == 0) { atomicAdd(tile_counter + 11, 1u); atomicAdd(tile_counter + 12, (unsigned)__popc(m)); } }
+#endif
+                if (status == ST_READY) {
+                    float px, py, pz;
+                    lattice_point(r, sc.step, k, px, py, pz);
+                    uint32_t I[8];
+                    gather_features(sc, px, py, pz, I);
+                    float t[8];
+#pragma unroll
+                    for (int c = 0; c < 8; c++) t[c] = __fmaf_rn(__uint2float_rn(I[c]), sc.deq_mul, sc.deq_add);
+                    const float tau = exp_q(t[0]); // decision path
+                    const float od = __fmul_rn(tau, sc.step);
+                    const uint32_t qk = (uint32_t)rintf(fminf(__fmul_rn(od, 1048576.0f), (float)sc.q_stop));
+                    const float T = __expf(-(float)Q * (1.0f / 1048576.0f)); // colour path: fast math
+                    const float wgt = T * (1.0f - __expf(-od));
+#pragma unroll
+                    for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, sigmoid_fast(t[1 + c]), acc[c]);
+                    Q += qk;
+                    n += 1;
+                    k += 1;
+                    if (Q >= sc.q_stop) {
+                        status = ST_FIN; // early stop (R7)
+                    } else {
+                        // inside the slab the next lattice point is usually occupied too: test it here (level 0)
+                        status = ST_TRAV;
+                        lvl = 0;
+                        if (SAMPLER == OMERF_SAMPLER_PLANE && k <= k1) {
+                            lattice_point(r, sc.step, k, px, py, pz);
+                            const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
+                            const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
+                            if (h.x <= pz && pz <= h.y && in_box(sc, px, py, pz)) status = ST_READY;
                         }
                     }
                 }
-                tpos += min(__popc(m_idle), 32 - tpos);
+                if (__popc(__ballot_sync(FULL, status == ST_READY)) < OMERF_SAMPLE_KEEP) break;
             }
-        }
-        if (!__any_sync(FULL, status != ST_IDLE)) {
-            if (!more) break;
-            continue;
-        }
-        // (3) one traversal step for rays in empty space / between samples (S4)
-        if (status == ST_TRAV) {
-            status = SAMPLER == OMERF_SAMPLER_PLANE ? trav_step_plane(sc, r, k, k1, lvl) : trav_step_grid(sc, r, k, k1, lvl);
-            if (status == ST_FIN && n == 0) { // no sample at all: background exactly, MLP skipped (R14)
-                out_rgb[pix * 3 + 0] = sc.bg[0];
-                out_rgb[pix * 3 + 1] = sc.bg[1];
-                out_rgb[pix * 3 + 2] = sc.bg[2];
-                out_n[pix] = 0;
-                status = ST_IDLE;
+            if (active) {
+                P.k[slot] = k;
+                P.Q[slot] = Q;
+                P.n[slot] = n;
+#pragma unroll
+                for (int c = 0; c < 7; c++) P.acc[c][slot] = acc[c];
+                P.meta[slot] = pack_meta(status, lvl, view);
             }
-        }
-        // (4) one sample for rays that stand on an occupied lattice point (S5, S6, S7)
-        const unsigned m_ready = __ballot_sync(FULL, status == ST_READY);
-        const unsigned m_trav = __ballot_sync(FULL, status == ST_TRAV);
-        if (m_ready && (__popc(m_ready) >= OMERF_SAMPLE_T || !m_trav)) {
-            if (status == ST_READY) {
-                float px, py, pz;
-                lattice_point(r, sc.step, k, px, py, pz);
-                uint32_t I[8];
-                gather_features(sc, px, py, pz, I);
-                float t[8];
+        } else {
+            // ---- retire: deferred MLP on tensor cores + outputs (S8, S9)
+#pragma unroll 1
+            for (int half = 0; half < 2; half++) {
+                if (half * 16 >= n_act) break;
+                if ((lane >> 4) == half) { // stage the inputs of this half's rays (zeros for unused rows)
+                    float in[OMERF_MLP_IN];
 #pragma unroll
-                for (int c = 0; c < 8; c++) t[c] = __fmaf_rn(__uint2float_rn(I[c]), sc.deq_mul, sc.deq_add);
-                const float tau = exp_q(t[0]); // decision path
-                const float od = __fmul_rn(tau, sc.step);
-                const uint32_t qk = (uint32_t)rintf(fminf(__fmul_rn(od, 1048576.0f), (float)sc.q_stop));
-                const float T = __expf(-(float)Q * (1.0f / 1048576.0f)); // colour path: fast math
-                const float wgt = T * (1.0f - __expf(-od));
+                    for (int i = 0; i < OMERF_MLP_IN; i++) in[i] = 0.0f;
+                    if (active) {
+                        float acc[7];
 #pragma unroll
-                for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, sigmoid_fast(t[1 + c]), acc[c]);
-                Q += qk;
-                n += 1;
-                k += 1;
-                if (Q >= sc.q_stop) {
-                    status = ST_FIN; // early stop (R7)
-                } else {
-                    // inside the slab the next lattice point is usually occupied too: test it here (level 0)
-                    // instead of paying a traversal round for it
-                    status = ST_TRAV;
-                    lvl = 0;
-                    if (SAMPLER == OMERF_SAMPLER_PLANE && k <= k1) {
-                        lattice_point(r, sc.step, k, px, py, pz);
-                        const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
-                        const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
-                        if (h.x <= pz && pz <= h.y && in_box(sc, px, py, pz)) status = ST_READY;
+                        for (int c = 0; c < 7; c++) acc[c] = P.acc[c][slot];
+                        mlp_input(acc, P.dx[slot], P.dy[slot], P.dz[slot], in);
+                    }
+                    float4 *row = reinterpret_cast<float4 *>(P.X + (lane & 15) * OMERF_XS);
+#pragma unroll
+                    for (int i = 0; i < 8; i++) row[i] = make_float4(in[4 * i], in[4 * i + 1], in[4 * i + 2], in[4 * i + 3]);
+                    row[8] = make_float4(in[32], in[33], 0.0f, 0.0f);
+                    row[9] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                }
+                __syncwarp();
+                float o[4];
+                mlp_half(sc.mlp_tab, P.X, lane, o);
+                // lane (g, t): t = 0 holds colours 0,1 and t = 1 colour 2 of rays g and g+8 of this half
+                const int g = lane >> 2, t = lane & 3;
+                if (t < 2) {
+#pragma unroll
+                    for (int rr = 0; rr < 2; rr++) {
+                        const int ray = half * 16 + g + 8 * rr;
+                        if (ray < n_act) {
+                            const int sl = (int)P.list[ray];
+                            const size_t pix = P.pix[sl];
+                            const float T_end = __expf(-(float)P.Q[sl] * (1.0f / 1048576.0f));
+                            if (t == 0) {
+                                out_rgb[pix * 3 + 0] = __saturatef(P.acc[0][sl] + sigmoid_fast(o[2 * rr]) + T_end * sc.bg[0]);
+                                out_rgb[pix * 3 + 1] = __saturatef(P.acc[1][sl] + sigmoid_fast(o[2 * rr + 1]) + T_end * sc.bg[1]);
+                                out_n[pix] = P.n[sl];
+                            } else {
+                                out_rgb[pix * 3 + 2] = __saturatef(P.acc[2][sl] + sigmoid_fast(o[2 * rr]) + T_end * sc.bg[2]);
+                            }
+                        }
                     }
                 }
+                __syncwarp();
             }
+            if (active) P.meta[slot] = ST_IDLE;
         }
+        __syncwarp();
     }
 }
 
@@ -520,17 +740,32 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H, float *out_rgb,
                         uint32_t *out_n, cudaStream_t st, int *launches)
 {
-    if ((long long)((W + 7) / 8) * ((H + 3) / 4) * n_views > 0x7fffffffll) {
+    if ((long long)((W + 7) / 8) * ((H + 3) / 4) * n_views > 0x7fffffffll || (long long)W * H * n_views > 0xffffffffll) {
         omerf_set_error("invalid argument: image or batch too large");
         return OMERF_ERR_INVALID;
     }
+#ifdef OMERF_X_STATS
+    {
+        static int calls = 0;
+        if (calls++ == 8) {
+            unsigned h[16];
+            cudaMemcpy(h, s->d_tile_counter, sizeof h, cudaMemcpyDeviceToHost);
+            const char *nm[4] = {"refill", "trav", "sample", "mlp"};
+            for (int i = 0; i < 4; i++) printf("STATS %s rounds %u avg lanes %.1f\n", nm[i], h[1 + i], h[5 + i] / (double)(h[1 + i] ? h[1 + i] : 1));
+            printf("STATS trav steps(warp) %u avg lanes %.1f thread-steps %u\n", h[9], h[10] / (double)(h[9] ? h[9] : 1), h[10]);
+            printf("STATS sample iters(warp) %u avg lanes %.1f thread-samples %u\n", h[11], h[12] / (double)(h[11] ? h[11] : 1), h[12]);
+        }
+    }
+    OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, 64 * sizeof(unsigned int), st));
+#else
     OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, sizeof(unsigned int), st));
+#endif
     const int grid = s->persistent_blocks;
     if (s->dev.sampler == OMERF_SAMPLER_PLANE)
-        omerf_march_kernel<OMERF_SAMPLER_PLANE><<<grid, 128, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,
+        omerf_march_kernel<OMERF_SAMPLER_PLANE><<<grid, 32 * OMERF_WARPS, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,
                                                                        s->d_tile_counter);
     else
-        omerf_march_kernel<OMERF_SAMPLER_GRID><<<grid, 128, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,
+        omerf_march_kernel<OMERF_SAMPLER_GRID><<<grid, 32 * OMERF_WARPS, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,
                                                                       s->d_tile_counter);
     *launches = 1;
     OMERF_CUDA(cudaGetLastError());
@@ -544,9 +779,9 @@ int omerf_query_persistent_blocks(int sampler, int *blocks)
     OMERF_CUDA(cudaGetDevice(&dev));
     OMERF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     if (sampler == OMERF_SAMPLER_PLANE)
-        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_PLANE>, 128, 0));
+        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_PLANE>, 32 * OMERF_WARPS, 0));
     else
-        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_GRID>, 128, 0));
+        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_GRID>, 32 * OMERF_WARPS, 0));
     *blocks = sms * (per_sm > 0 ? per_sm : 1);
     return OMERF_OK;
 }
