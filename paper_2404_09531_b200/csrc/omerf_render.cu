@@ -449,6 +449,12 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 #define OMERF_SAMPLE_KEEP 24   // sample again at once while this many lanes stand on an occupied point
 #endif
 #define OMERF_WARPS 4
+#ifndef OMERF_ENDGAME_WARPS
+#define OMERF_ENDGAME_WARPS 2   // endgame starts when fewer than this many tiles per warp are left
+#endif
+#ifndef OMERF_ENDGAME_BUSY
+#define OMERF_ENDGAME_BUSY 32   // in the endgame a warp takes a new tile only with at most this many rays in flight
+#endif
 #define OMERF_PJ (OMERF_POOL / 32)
 
 struct WarpPool {
@@ -487,48 +493,67 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 #pragma unroll
     for (int j = 0; j < OMERF_PJ; j++) P.meta[lane + 32 * j] = ST_IDLE;
     __syncwarp();
+#ifdef OMERF_X_TIMELINE
+    unsigned long long *tl = reinterpret_cast<unsigned long long *>(tile_counter + 64);
+    if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 3 + 0] = t; }
+#endif
     bool more = true;
+    // Endgame: a warp's pool holds about three tiles of work, which would all drain at falling utilisation once the
+    // tile counter runs out.  For the last tiles, warps refill only when (nearly) empty, so the remaining work
+    // spreads over all warps and they finish together.
+    bool endgame = false;
+    const unsigned endgame_tiles = OMERF_ENDGAME_WARPS * gridDim.x * OMERF_WARPS;
 
     while (true) {
-        // ---- census of the pool
-        uint32_t st[OMERF_PJ];
+        // ---- census of the pool (idle = the rest)
         unsigned bal[4][OMERF_PJ];
-        int cnt[4] = {0, 0, 0, 0};
+        int cnt[4] = {OMERF_POOL, 0, 0, 0};
 #pragma unroll
         for (int j = 0; j < OMERF_PJ; j++) {
-            st[j] = P.meta[lane + 32 * j] & 3u;
+            const uint32_t st = P.meta[lane + 32 * j] & 3u;
 #pragma unroll
-            for (int s = 0; s < 4; s++) {
-                bal[s][j] = __ballot_sync(FULL, st[j] == (uint32_t)s);
+            for (int s = 1; s < 4; s++) {
+                bal[s][j] = __ballot_sync(FULL, st == (uint32_t)s);
                 cnt[s] += __popc(bal[s][j]);
             }
+            bal[0][j] = ~(bal[1][j] | bal[2][j] | bal[3][j]);
         }
-        // ---- pick a phase: full warps first, then the fullest
-        int phase;
-        if (cnt[ST_FIN] >= 32) phase = ST_FIN;
-        else if (cnt[ST_READY] >= 32) phase = ST_READY;
-        else if (cnt[ST_TRAV] >= 32) phase = ST_TRAV;
-        else if (more && cnt[ST_IDLE] >= 32) phase = ST_IDLE;
+        cnt[0] -= cnt[1] + cnt[2] + cnt[3];
+        // ---- pick a phase: full warps first, then the fullest (all warp-uniform)
+        int phase, n_sel;
+        unsigned b[OMERF_PJ];
+#define OMERF_PICK(S)                                           \
+    {                                                           \
+        phase = (S);                                            \
+        n_sel = cnt[S];                                         \
+        _Pragma("unroll") for (int j = 0; j < OMERF_PJ; j++) b[j] = bal[S][j]; \
+    }
+        if (cnt[ST_FIN] >= 32) OMERF_PICK(ST_FIN)
+        else if (cnt[ST_READY] >= 32) OMERF_PICK(ST_READY)
+        else if (cnt[ST_TRAV] >= 32) OMERF_PICK(ST_TRAV)
+        else if (more && cnt[ST_IDLE] >= (endgame ? OMERF_POOL - OMERF_ENDGAME_BUSY : 32)) OMERF_PICK(ST_IDLE)
+        else if (cnt[ST_READY] > 0 && cnt[ST_READY] >= cnt[ST_TRAV]) OMERF_PICK(ST_READY)
+        else if (cnt[ST_TRAV] > 0) OMERF_PICK(ST_TRAV)
+        else if (cnt[ST_FIN] > 0) OMERF_PICK(ST_FIN) // finished rays wait for a full MLP batch unless nothing else is left
         else {
-            phase = ST_READY;
-            int best = cnt[ST_READY];
-            if (cnt[ST_TRAV] > best) { best = cnt[ST_TRAV]; phase = ST_TRAV; }
-            if (best == 0) { best = cnt[ST_FIN]; phase = ST_FIN; } // finished rays wait for a full MLP batch
-            if (best == 0) break; // pool empty and no tile left (otherwise the refill branch was taken)
+#ifdef OMERF_X_TIMELINE
+            if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 3 + 2] = t; }
+#endif
+            break; // pool empty and no tile left (otherwise the refill branch was taken)
         }
+#undef OMERF_PICK
         // ---- the first 32 slots in that state
         {
             int base = 0;
 #pragma unroll
             for (int j = 0; j < OMERF_PJ; j++) {
-                unsigned b = phase == ST_IDLE ? bal[0][j] : phase == ST_TRAV ? bal[1][j] : phase == ST_READY ? bal[2][j] : bal[3][j];
-                const int pos = base + __popc(b & lt_mask);
-                if (((b >> lane) & 1u) && pos < 32) P.list[pos] = lane + 32 * j;
-                base += __popc(b);
+                const int pos = base + __popc(b[j] & lt_mask);
+                if (((b[j] >> lane) & 1u) && pos < 32) P.list[pos] = lane + 32 * j;
+                base += __popc(b[j]);
             }
         }
         __syncwarp();
-        const int n_act = min(cnt[phase], 32);
+        const int n_act = min(n_sel, 32);
 #ifdef OMERF_X_STATS
         if (lane == 0) { atomicAdd(tile_counter + 1 + phase, 1u); atomicAdd(tile_counter + 5 + phase, (unsigned)n_act); }
 #endif
@@ -540,8 +565,12 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             unsigned t = 0;
             if (lane == 0) t = atomicAdd(tile_counter, 1u);
             const unsigned tile = __shfl_sync(FULL, t, 0);
+            if (tile + endgame_tiles >= total_tiles) endgame = true;
             if (tile >= total_tiles) {
                 more = false;
+#ifdef OMERF_X_TIMELINE
+                if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 3 + 1] = t; }
+#endif
             } else {
                 const unsigned view = tile / tiles_per_view, tv = tile - view * tiles_per_view;
                 const int ty = (int)(tv / (unsigned)tiles_x), tx = (int)(tv - (unsigned)ty * tiles_x);
@@ -744,6 +773,28 @@ int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_
         omerf_set_error("invalid argument: image or batch too large");
         return OMERF_ERR_INVALID;
     }
+#ifdef OMERF_X_TIMELINE
+    {
+        static int calls = 0;
+        if (calls++ == 8) {
+            int nw = s->persistent_blocks * OMERF_WARPS;
+            unsigned long long *h = new unsigned long long[nw * 3];
+            cudaMemcpy(h, s->d_tile_counter + 64, sizeof(unsigned long long) * nw * 3, cudaMemcpyDeviceToHost);
+            unsigned long long t0 = ~0ull;
+            for (int i = 0; i < nw; i++) if (h[i * 3] < t0) t0 = h[i * 3];
+            double sum[3] = {0, 0, 0}, mx[3] = {0, 0, 0}, mn[3] = {1e30, 1e30, 1e30};
+            for (int i = 0; i < nw; i++) for (int c = 0; c < 3; c++) { double v = (double)(h[i * 3 + c] - t0) * 1e-3; sum[c] += v; if (v > mx[c]) mx[c] = v; if (v < mn[c]) mn[c] = v; }
+            for (int c = 0; c < 3; c++) printf("TIMELINE %s us: min %.1f mean %.1f max %.1f\n", c == 0 ? "start" : c == 1 ? "exhausted" : "finish", mn[c], sum[c] / nw, mx[c]);
+            // histogram of finish times
+            int hist[16] = {0};
+            for (int i = 0; i < nw; i++) { int b = (int)((double)(h[i * 3 + 2] - t0) * 1e-3 / 100.0); if (b > 15) b = 15; hist[b]++; }
+            printf("TIMELINE finish histogram (100 us bins):");
+            for (int b = 0; b < 16; b++) printf(" %d", hist[b]);
+            printf("\n");
+            delete[] h;
+        }
+    }
+#endif
 #ifdef OMERF_X_STATS
     {
         static int calls = 0;
