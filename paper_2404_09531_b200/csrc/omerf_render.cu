@@ -215,73 +215,124 @@ __device__ __forceinline__ void axis_tap(float p, float s, int N, int &i0, int &
     i1 = min(max(i + 1, 0), N - 1);
 }
 
-// byte c of x, zero-extended: one PRMT
-__device__ __forceinline__ uint32_t byte_of(uint32_t x, int c) { return __byte_perm(x, 0u, 0x4440u + (uint32_t)c); }
+// Bilinear footprints as 16-bit x 8-bit dot products (IDP.2A, fma pipe, full rate): the four weights
+// w_ab = (256 - w_a | w_a)(256 - w_b | w_b) are packed as two u16 pairs, the texel bytes of one channel of two
+// texels are brought side by side with one PRMT per two channels.  Only w_00 can reach 2^16 (w_a = w_b = 0, after
+// weight 256 has been folded into the neighbour index); then tap b1 is redirected to b0 and one unit of w_00 moves
+// to w_01, which multiplies the same texel: the sum stays the exact integer of R9.
+struct BiW {
+    uint32_t w0, w1; // (w00 | w01 << 16), (w10 | w11 << 16): pairs along axis b for rows a0 and a1
+};
 
-// out[c] (+)= sum over the 2x2 footprint of w_ab * texel_ab[c]; exact integers <= 255 * 2^16
-template <bool ACCUM>
-__device__ __forceinline__ void bilinear8(const uint2 *__restrict__ tex, int Nb, int a0, int a1, uint32_t wa, int b0,
-                                          int b1, uint32_t wb, uint32_t out[8])
+// fold weight 256 into the index (w in [0,255] afterwards)
+__device__ __forceinline__ void fold_tap(int &i0, int i1, uint32_t &w)
 {
-    const uint2 t00 = __ldg(tex + (size_t)a0 * Nb + b0);
-    const uint2 t01 = __ldg(tex + (size_t)a0 * Nb + b1);
-    const uint2 t10 = __ldg(tex + (size_t)a1 * Nb + b0);
-    const uint2 t11 = __ldg(tex + (size_t)a1 * Nb + b1);
-    const uint32_t w00 = (256u - wa) * (256u - wb), w10 = wa * (256u - wb), w01 = (256u - wa) * wb, w11 = wa * wb;
-#pragma unroll
-    for (int c = 0; c < 4; c++) {
-        uint32_t lo = w00 * byte_of(t00.x, c) + w10 * byte_of(t10.x, c) + w01 * byte_of(t01.x, c) + w11 * byte_of(t11.x, c);
-        uint32_t hi = w00 * byte_of(t00.y, c) + w10 * byte_of(t10.y, c) + w01 * byte_of(t01.y, c) + w11 * byte_of(t11.y, c);
-        if (ACCUM) {
-            out[c] += lo;
-            out[4 + c] += hi;
-        } else {
-            out[c] = lo;
-            out[4 + c] = hi;
-        }
+    if (w == 256u) {
+        i0 = i1;
+        w = 0u;
     }
+}
+
+__device__ __forceinline__ BiW bilinear_weights(uint32_t wa, uint32_t wb, int b0, int &b1)
+{
+    if (wb == 0u) b1 = b0; // weight of column b1 is zero: point it at b0 so that it can carry the overflow unit
+    const uint32_t ua = 256u - wa, ub = 256u - wb;
+    const uint32_t w00 = ua * ub, c = w00 >> 16;
+    BiW r;
+    r.w0 = (w00 - c) + ((ua * wb + c) << 16);
+    r.w1 = wa * ub + ((wa * wb) << 16);
+    return r;
+}
+
+// acc[0..7] += sum over the 2x2 footprint of w_ab * texel_ab[c]
+__device__ __forceinline__ void bilinear8_dp(const uint2 t00, const uint2 t01, const uint2 t10, const uint2 t11, const BiW w,
+                                             uint32_t acc[8])
+{
+    uint32_t p, q;
+    p = __byte_perm(t00.x, t01.x, 0x5140);
+    q = __byte_perm(t10.x, t11.x, 0x5140);
+    acc[0] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[0]));
+    acc[1] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[1]));
+    p = __byte_perm(t00.x, t01.x, 0x7362);
+    q = __byte_perm(t10.x, t11.x, 0x7362);
+    acc[2] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[2]));
+    acc[3] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[3]));
+    p = __byte_perm(t00.y, t01.y, 0x5140);
+    q = __byte_perm(t10.y, t11.y, 0x5140);
+    acc[4] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[4]));
+    acc[5] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[5]));
+    p = __byte_perm(t00.y, t01.y, 0x7362);
+    q = __byte_perm(t10.y, t11.y, 0x7362);
+    acc[6] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[6]));
+    acc[7] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[7]));
+}
+
+__device__ __forceinline__ void plane_taps(const uint2 *__restrict__ tex, int Nb, int a0, int a1, int b0, int b1, uint2 t[4])
+{
+    const uint2 *r0 = tex + (size_t)a0 * Nb, *r1 = tex + (size_t)a1 * Nb;
+    t[0] = __ldg(r0 + b0);
+    t[1] = __ldg(r0 + b1);
+    t[2] = __ldg(r1 + b0);
+    t[3] = __ldg(r1 + b1);
 }
 
 __device__ __forceinline__ void gather_features(const DevScene &sc, float px, float py, float pz, uint32_t I[8])
 {
+    // taps and weights of all four sources first, then all 20 loads, then the arithmetic
     int x0, x1, y0, y1, z0, z1;
     uint32_t wx, wy, wz;
-    // low-res voxel grid V: bilinear in (x,y) on two z-slices, then the z lerp with rounding (R9)
     axis_tap(px, sc.gs[0], sc.G[0], x0, x1, wx);
     axis_tap(py, sc.gs[1], sc.G[1], y0, y1, wy);
     axis_tap(pz, sc.gs[2], sc.G[2], z0, z1, wz);
+    fold_tap(x0, x1, wx);
+    fold_tap(y0, y1, wy);
+    const BiW wg = bilinear_weights(wx, wy, y0, y1);
+    uint2 ga[4], gb[4];
     {
+        // low-res voxel grid V: bilinear in (x,y) on the z-slices z0 and z1
         const int Gy = sc.G[1], Gz = sc.G[2];
         const uint2 *g = sc.grid;
-        const size_t r00 = ((size_t)x0 * Gy + y0) * Gz, r10 = ((size_t)x1 * Gy + y0) * Gz;
-        const size_t r01 = ((size_t)x0 * Gy + y1) * Gz, r11 = ((size_t)x1 * Gy + y1) * Gz;
-        const uint2 a00 = __ldg(g + r00 + z0), b00 = __ldg(g + r00 + z1);
-        const uint2 a10 = __ldg(g + r10 + z0), b10 = __ldg(g + r10 + z1);
-        const uint2 a01 = __ldg(g + r01 + z0), b01 = __ldg(g + r01 + z1);
-        const uint2 a11 = __ldg(g + r11 + z0), b11 = __ldg(g + r11 + z1);
-        const uint32_t w00 = (256u - wx) * (256u - wy), w10 = wx * (256u - wy), w01 = (256u - wx) * wy, w11 = wx * wy;
-#pragma unroll
-        for (int c = 0; c < 4; c++) {
-            uint32_t A = w00 * byte_of(a00.x, c) + w10 * byte_of(a10.x, c) + w01 * byte_of(a01.x, c) + w11 * byte_of(a11.x, c);
-            uint32_t B = w00 * byte_of(b00.x, c) + w10 * byte_of(b10.x, c) + w01 * byte_of(b01.x, c) + w11 * byte_of(b11.x, c);
-            I[c] = ((256u - wz) * A + wz * B + 128u) >> 8;
-            A = w00 * byte_of(a00.y, c) + w10 * byte_of(a10.y, c) + w01 * byte_of(a01.y, c) + w11 * byte_of(a11.y, c);
-            B = w00 * byte_of(b00.y, c) + w10 * byte_of(b10.y, c) + w01 * byte_of(b01.y, c) + w11 * byte_of(b11.y, c);
-            I[4 + c] = ((256u - wz) * A + wz * B + 128u) >> 8;
-        }
+        const uint2 *r00 = g + ((size_t)x0 * Gy + y0) * Gz, *r01 = g + ((size_t)x0 * Gy + y1) * Gz;
+        const uint2 *r10 = g + ((size_t)x1 * Gy + y0) * Gz, *r11 = g + ((size_t)x1 * Gy + y1) * Gz;
+        ga[0] = __ldg(r00 + z0); gb[0] = __ldg(r00 + z1);
+        ga[1] = __ldg(r01 + z0); gb[1] = __ldg(r01 + z1);
+        ga[2] = __ldg(r10 + z0); gb[2] = __ldg(r10 + z1);
+        ga[3] = __ldg(r11 + z0); gb[3] = __ldg(r11 + z1);
     }
     // triplanes: xy sampled with (x,y), xz with (x,z), yz with (y,z)
     int a0, a1, b0, b1;
     uint32_t wa, wb;
+    uint2 t1[4], t2[4], t3[4];
     axis_tap(px, sc.xy_s[0], sc.xy_n[0], a0, a1, wa);
     axis_tap(py, sc.xy_s[1], sc.xy_n[1], b0, b1, wb);
-    bilinear8<true>(sc.pxy, sc.xy_n[1], a0, a1, wa, b0, b1, wb, I);
+    fold_tap(a0, a1, wa);
+    fold_tap(b0, b1, wb);
+    const BiW w1 = bilinear_weights(wa, wb, b0, b1);
+    plane_taps(sc.pxy, sc.xy_n[1], a0, a1, b0, b1, t1);
     axis_tap(px, sc.xz_s[0], sc.xz_n[0], a0, a1, wa);
     axis_tap(pz, sc.xz_s[1], sc.xz_n[1], b0, b1, wb);
-    bilinear8<true>(sc.pxz, sc.xz_n[1], a0, a1, wa, b0, b1, wb, I);
+    fold_tap(a0, a1, wa);
+    fold_tap(b0, b1, wb);
+    const BiW w2 = bilinear_weights(wa, wb, b0, b1);
+    plane_taps(sc.pxz, sc.xz_n[1], a0, a1, b0, b1, t2);
     axis_tap(py, sc.yz_s[0], sc.yz_n[0], a0, a1, wa);
     axis_tap(pz, sc.yz_s[1], sc.yz_n[1], b0, b1, wb);
-    bilinear8<true>(sc.pyz, sc.yz_n[1], a0, a1, wa, b0, b1, wb, I);
+    fold_tap(a0, a1, wa);
+    fold_tap(b0, b1, wb);
+    const BiW w3 = bilinear_weights(wa, wb, b0, b1);
+    plane_taps(sc.pyz, sc.yz_n[1], a0, a1, b0, b1, t3);
+
+    uint32_t A[8], B[8];
+#pragma unroll
+    for (int c = 0; c < 8; c++) A[c] = B[c] = 0u;
+    bilinear8_dp(ga[0], ga[1], ga[2], ga[3], wg, A);
+    bilinear8_dp(gb[0], gb[1], gb[2], gb[3], wg, B);
+    // the z lerp rounds once (R9): (256 - wz) A + wz B < 2^32
+#pragma unroll
+    for (int c = 0; c < 8; c++) I[c] = ((256u - wz) * A[c] + wz * B[c] + 128u) >> 8;
+    bilinear8_dp(t1[0], t1[1], t1[2], t1[3], w1, I);
+    bilinear8_dp(t2[0], t2[1], t2[2], t2[3], w2, I);
+    bilinear8_dp(t3[0], t3[1], t3[2], t3[3], w3, I);
 }
 
 __device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
