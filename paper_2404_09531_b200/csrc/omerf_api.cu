@@ -79,6 +79,11 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         if (d->grid_n[i] < 1) return invalid("grid_n must be >= 1");
     for (int i = 0; i < 2; i++)
         if (d->xy_n[i] < 1 || d->xz_n[i] < 1 || d->yz_n[i] < 1) return invalid("plane sizes must be >= 1");
+    // the gather addresses texels with 32-bit indices
+    if ((unsigned long long)d->grid_n[0] * d->grid_n[1] * d->grid_n[2] > 0xffffffffull ||
+        (unsigned long long)d->xy_n[0] * d->xy_n[1] > 0xffffffffull || (unsigned long long)d->xz_n[0] * d->xz_n[1] > 0xffffffffull ||
+        (unsigned long long)d->yz_n[0] * d->yz_n[1] > 0xffffffffull)
+        return invalid("a feature array has more than 2^32 - 1 texels");
     if (!d->grid || !d->plane_xy || !d->plane_xz || !d->plane_yz) return invalid("null feature array");
     if (d->mlp_in != OMERF_MLP_IN || d->mlp_hidden != OMERF_MLP_HID) return invalid("MLP must be 34 -> 16 -> 16 -> 3");
     if (!d->W0 || !d->b0 || !d->W1 || !d->b1 || !d->W2 || !d->b2) return invalid("null MLP array");

@@ -211,8 +211,9 @@ __device__ __forceinline__ void axis_tap(float p, float s, int N, int &i0, int &
     const int i = __float2int_rd(q);
     // (q - floor q) * 256 is exact, so one fma rounds exactly like the mul followed by the add
     w = (uint32_t)__float2int_rd(__fmaf_rn(__fsub_rn(q, __int2float_rn(i)), 256.0f, 0.5f));
-    i0 = min(max(i, 0), N - 1);
-    i1 = min(max(i + 1, 0), N - 1);
+    // the point is inside the box (checked before every sample), so -1 <= i <= N-1: one clamp per tap suffices
+    i0 = max(i, 0);
+    i1 = min(i + 1, N - 1);
 }
 
 // Bilinear footprints as 16-bit x 8-bit dot products (IDP.2A, fma pipe, full rate): the four weights
@@ -269,11 +270,12 @@ __device__ __forceinline__ void bilinear8_dp(const uint2 t00, const uint2 t01, c
 
 __device__ __forceinline__ void plane_taps(const uint2 *__restrict__ tex, int Nb, int a0, int a1, int b0, int b1, uint2 t[4])
 {
-    const uint2 *r0 = tex + (size_t)a0 * Nb, *r1 = tex + (size_t)a1 * Nb;
-    t[0] = __ldg(r0 + b0);
-    t[1] = __ldg(r0 + b1);
-    t[2] = __ldg(r1 + b0);
-    t[3] = __ldg(r1 + b1);
+    // 32-bit texel indices (every source has fewer than 2^32 texels; checked at scene creation)
+    const uint32_t r0 = (uint32_t)a0 * (uint32_t)Nb, r1 = (uint32_t)a1 * (uint32_t)Nb;
+    t[0] = __ldg(tex + (r0 + (uint32_t)b0));
+    t[1] = __ldg(tex + (r0 + (uint32_t)b1));
+    t[2] = __ldg(tex + (r1 + (uint32_t)b0));
+    t[3] = __ldg(tex + (r1 + (uint32_t)b1));
 }
 
 __device__ __forceinline__ void gather_features(const DevScene &sc, float px, float py, float pz, uint32_t I[8])
@@ -290,14 +292,15 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
     uint2 ga[4], gb[4];
     {
         // low-res voxel grid V: bilinear in (x,y) on the z-slices z0 and z1
-        const int Gy = sc.G[1], Gz = sc.G[2];
+        const uint32_t Gy = (uint32_t)sc.G[1], Gz = (uint32_t)sc.G[2];
         const uint2 *g = sc.grid;
-        const uint2 *r00 = g + ((size_t)x0 * Gy + y0) * Gz, *r01 = g + ((size_t)x0 * Gy + y1) * Gz;
-        const uint2 *r10 = g + ((size_t)x1 * Gy + y0) * Gz, *r11 = g + ((size_t)x1 * Gy + y1) * Gz;
-        ga[0] = __ldg(r00 + z0); gb[0] = __ldg(r00 + z1);
-        ga[1] = __ldg(r01 + z0); gb[1] = __ldg(r01 + z1);
-        ga[2] = __ldg(r10 + z0); gb[2] = __ldg(r10 + z1);
-        ga[3] = __ldg(r11 + z0); gb[3] = __ldg(r11 + z1);
+        const uint32_t c0 = (uint32_t)x0 * Gy, c1 = (uint32_t)x1 * Gy;
+        const uint32_t r00 = (c0 + (uint32_t)y0) * Gz, r01 = (c0 + (uint32_t)y1) * Gz;
+        const uint32_t r10 = (c1 + (uint32_t)y0) * Gz, r11 = (c1 + (uint32_t)y1) * Gz;
+        ga[0] = __ldg(g + (r00 + (uint32_t)z0)); gb[0] = __ldg(g + (r00 + (uint32_t)z1));
+        ga[1] = __ldg(g + (r01 + (uint32_t)z0)); gb[1] = __ldg(g + (r01 + (uint32_t)z1));
+        ga[2] = __ldg(g + (r10 + (uint32_t)z0)); gb[2] = __ldg(g + (r10 + (uint32_t)z1));
+        ga[3] = __ldg(g + (r11 + (uint32_t)z0)); gb[3] = __ldg(g + (r11 + (uint32_t)z1));
     }
     // triplanes: xy sampled with (x,y), xz with (x,z), yz with (y,z)
     int a0, a1, b0, b1;
