@@ -231,6 +231,9 @@ def run_ours(args):
     total_ms = float(np.sum(ms))
     samples = int(out_n.sum(dtype=torch.int64).item())
 
+    # gather calibration: the same frame's 20 texel loads per sample replayed with no arithmetic
+    probe = omerf.gather_probe(h, cams[0], W, H, repeats=10, flush_l2=True) if rank == 0 else None
+
     # e2e through the C-ABI with HOST buffers (pinned), copies inside the timed region
     h_rgb = torch.empty((n_views, H, W, 3), dtype=torch.float32).pin_memory()
     h_n = torch.empty((n_views, H, W), dtype=torch.int32).pin_memory()
@@ -297,6 +300,14 @@ def run_ours(args):
                               "algorithmic_bytes_per_launch": alg_bytes},
             "clocks": clk,
         }
+        if probe and probe["samples"]:
+            ceil_gs = probe["samples"] / probe["ms_frame_order"] / 1e6           # Gsamples/s, gather only, frame order
+            view0 = probe["samples"] / (march_ms / n_views) / 1e6 if n_views == 1 else world * samples * k / secs / 1e9 / world
+            line["gather_calibrated"] = {
+                "what": "omerf_gather_probe: 20 x 8-byte loads per sample of view 0, no arithmetic, L2 flushed",
+                "ceiling_gsamples_s": ceil_gs, "ceiling_gbs": ceil_gs * 160,
+                "scattered_gsamples_s": probe["samples"] / probe["ms_scattered"] / 1e6,
+                "march_gsamples_s": view0, "frac": view0 / ceil_gs}
         if cpu is not None:
             line["cpu_baseline"] = {"value": cpu["mpix_s"], "unit": "Mpixels/s", "cores": cpu["cores"], "kind": "oracle",
                                     "sample": cpu["sample"], "msamples_s": cpu["msamples_s"], "seconds": cpu["seconds"]}

@@ -92,6 +92,20 @@ int omerf_render(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/,
 int omerf_render_host(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W,
                       int H, float *out_rgb /*HOST*/, uint32_t *out_nsamples /*HOST*/, void *stream);
 
+/* Gather calibration (SURVEY.md 8(d) "L2/L1 gather rate": the builder must calibrate the achievable rate of the
+ * same load width over the same footprint).  Renders one frame of `camera` while logging every sample taken, then
+ * times a kernel that only replays the 20 eight-byte texel loads of Eq. 2 for those samples - no
+ * filtering, activations or compositing - once in frame order (pixel-coherent addresses) and once in a scattered
+ * order.  160 B are requested per sample.  flush_l2 != 0 overwrites a 256 MiB buffer before every timed launch.
+ * Synchronous (device-wide); owns and frees its scratch.  HOST pointers. */
+typedef struct {
+    uint64_t samples;       /* samples of the frame (= sum of out_nsamples) */
+    double ms_frame_order;  /* mean duration of one replay launch, frame order */
+    double ms_scattered;    /* mean duration of one replay launch, scattered order */
+} omerf_gather_probe_result;
+int omerf_gather_probe(const omerf_scene *scene, const omerf_camera *camera /*HOST, one view*/, int W, int H,
+                       int repeats, int flush_l2, omerf_gather_probe_result *out /*HOST*/);
+
 /* Number of kernels of this library the last omerf_render / omerf_render_host on this scene launched. */
 int omerf_last_launch_count(const omerf_scene *scene);
 

@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     OmerfError,
     SceneHandle,
     bitfield,
+    gather_probe,
     last_launch_count,
     load_library,
     pyramid_level,

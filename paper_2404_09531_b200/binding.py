@@ -22,7 +22,7 @@ SAMPLER_PLANE = 0
 SAMPLER_GRID = 1
 
 EXPORTS = (
-    "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_last_launch_count",
+    "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_gather_probe", "omerf_last_launch_count",
     "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield",
     "omerf_scene_destroy", "omerf_last_error", "omerf_version",
 )
@@ -48,6 +48,10 @@ class SceneInfo(C.Structure):
                 ("occ_bits_set", C.c_uint64)]
 
 
+class GatherProbeResult(C.Structure):
+    _fields_ = [("samples", C.c_uint64), ("ms_frame_order", C.c_double), ("ms_scattered", C.c_double)]
+
+
 class OmerfError(RuntimeError):
     pass
 
@@ -69,6 +73,8 @@ def load_library() -> C.CDLL:
     L.omerf_scene_create.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
     L.omerf_render.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
     L.omerf_render_host.argtypes = L.omerf_render.argtypes
+    L.omerf_gather_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
+                                     C.POINTER(GatherProbeResult)]
     L.omerf_last_launch_count.argtypes = [C.c_void_p]
     L.omerf_scene_get_info.argtypes = [C.c_void_p, C.POINTER(SceneInfo)]
     L.omerf_scene_get_pyramid_level.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
@@ -208,6 +214,16 @@ def render_host(h: SceneHandle, cameras, W: int, H: int, out_rgb=None, out_nsamp
     _check(load_library().omerf_render_host(h.ptr, cams.ctypes.data, n, W, H, hptr(out_rgb, n * H * W * 12),
                                             hptr(out_nsamples, n * H * W * 4), st.cuda_stream), "omerf_render_host")
     return out_rgb, out_nsamples
+
+
+def gather_probe(h: SceneHandle, camera, W: int, H: int, repeats: int = 10, flush_l2: bool = True) -> dict:
+    """omerf_gather_probe: gather-only replay of one frame's samples (calibration of the gather ceiling)."""
+    cams = _cams(camera)
+    res = GatherProbeResult()
+    _check(load_library().omerf_gather_probe(h.ptr, cams.ctypes.data, W, H, repeats, int(flush_l2), C.byref(res)),
+           "omerf_gather_probe")
+    return {"samples": int(res.samples), "ms_frame_order": float(res.ms_frame_order),
+            "ms_scattered": float(res.ms_scattered)}
 
 
 def last_launch_count(h: SceneHandle) -> int:

@@ -275,6 +275,85 @@ extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *camer
     return OMERF_OK;
 }
 
+
+// Gather calibration: logs the samples of one frame, then times kernels that only replay their
+// 20 texel loads, in frame order and in a scattered order.  Synchronous; allocates and frees its own buffers.
+extern "C" int omerf_gather_probe(const omerf_scene *s, const omerf_camera *camera, int W, int H, int repeats,
+                                  int flush_l2, omerf_gather_probe_result *out)
+{
+    if (!s || !camera || !out) return invalid("null scene/camera/out");
+    if (W <= 0 || H <= 0 || repeats <= 0) return invalid("W > 0, H > 0, repeats > 0 required");
+    memset(out, 0, sizeof *out);
+    const uint64_t px = (uint64_t)W * H;
+    int rc = ensure_cams(s, 1);
+    if (rc) return rc;
+    OMERF_CUDA(cudaDeviceSynchronize());
+    omerf_camera *dv = s->d_cams; // slot 0 of the ring; nothing is in flight after the synchronise
+    OMERF_CUDA(cudaMemcpy(dv, camera, sizeof(omerf_camera), cudaMemcpyHostToDevice));
+    float *rgb = nullptr;
+    uint32_t *cnt = nullptr, *sink = nullptr;
+    uint2 *log = nullptr;
+    char *flush = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    const size_t flush_bytes = (size_t)256 << 20;
+    unsigned int cap = (unsigned int)(px * 8 < 0xffffffffull ? px * 8 : 0xffffffffull), n = 0;
+    do {
+        cudaError_t e;
+#define PROBE_CUDA(call)                                       \
+    if ((e = (call)) != cudaSuccess) {                         \
+        rc = omerf_cuda_fail(e, #call);                        \
+        break;                                                 \
+    }
+        PROBE_CUDA(cudaMalloc((void **)&rgb, px * 3 * sizeof(float)));
+        PROBE_CUDA(cudaMalloc((void **)&cnt, px * sizeof(uint32_t)));
+        for (int attempt = 0; attempt < 2 && rc == OMERF_OK; attempt++) {
+            PROBE_CUDA(cudaMalloc((void **)&log, (size_t)cap * sizeof(uint2)));
+            int launches = 0;
+            if ((rc = omerf_launch_render(s, dv, 1, W, H, rgb, cnt, 0, &launches, log, cap))) break;
+            PROBE_CUDA(cudaMemcpy(&n, s->d_tile_counter + 32, sizeof n, cudaMemcpyDeviceToHost));
+            if (n <= cap) break;
+            cudaFree(log); // more samples than the first guess: size the log exactly and log again
+            log = nullptr;
+            cap = n;
+        }
+        if (rc) break;
+        out->samples = n;
+        if (n == 0) break;
+        PROBE_CUDA(cudaMalloc((void **)&sink, (size_t)n * sizeof(uint32_t)));
+        if (flush_l2) PROBE_CUDA(cudaMalloc((void **)&flush, flush_bytes));
+        PROBE_CUDA(cudaEventCreate(&e0));
+        PROBE_CUDA(cudaEventCreate(&e1));
+        // a multiplier coprime with n permutes the log; 1 keeps frame order
+        unsigned int mult = 2654435761u % n;
+        if (mult < 2) mult = 1;
+        auto gcd = [](unsigned a, unsigned b) { while (b) { unsigned t = a % b; a = b; b = t; } return a; };
+        while (mult > 1 && gcd(mult, n) != 1) mult--;
+        for (int order = 0; order < 2 && rc == OMERF_OK; order++) {
+            double total = 0.0;
+            for (int it = -1; it < repeats && rc == OMERF_OK; it++) { // it = -1: warm-up
+                if (flush) PROBE_CUDA(cudaMemsetAsync(flush, it & 0xff, flush_bytes, 0));
+                PROBE_CUDA(cudaEventRecord(e0, 0));
+                if ((rc = omerf_launch_gather_probe(s, dv, W, log, n, order ? mult : 1u, sink, 0))) break;
+                PROBE_CUDA(cudaEventRecord(e1, 0));
+                PROBE_CUDA(cudaEventSynchronize(e1));
+                float ms = 0.f;
+                PROBE_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+                if (it >= 0) total += ms;
+            }
+            (order ? out->ms_scattered : out->ms_frame_order) = total / repeats;
+        }
+#undef PROBE_CUDA
+    } while (0);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(rgb);
+    cudaFree(cnt);
+    cudaFree(log);
+    cudaFree(sink);
+    cudaFree(flush);
+    return rc;
+}
+
 extern "C" int omerf_last_launch_count(const omerf_scene *s) { return s ? s->last_launches : 0; }
 
 extern "C" int omerf_scene_get_info(const omerf_scene *s, omerf_scene_info *out)

@@ -86,5 +86,8 @@ int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, c
 int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st);
 int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_t st);
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H,
-                        float *out_rgb, uint32_t *out_n, cudaStream_t st, int *launches);
+                        float *out_rgb, uint32_t *out_n, cudaStream_t st, int *launches, uint2 *sample_log = nullptr,
+                        unsigned int log_capacity = 0);
+int omerf_launch_gather_probe(const omerf_scene *s, const omerf_camera *d_cam, int W, const uint2 *sample_log,
+                              unsigned int n, unsigned int mult, uint32_t *sink, cudaStream_t st);
 int omerf_query_persistent_blocks(int sampler, int *blocks);

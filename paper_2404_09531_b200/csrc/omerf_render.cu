@@ -445,11 +445,9 @@ __device__ __forceinline__ void mlp_half(const float2 *__restrict__ tab, const f
 }
 
 // ---------------------------------------------------------------------------------- S2 + S3: new ray for a lane
-// Returns false when the ray cannot have samples (misses the padded box).
-__device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera &cam, int u, int v, Ray &r, int &k,
-                                          int &k1)
+// S2 (R19): every step one correctly rounded fp32 operation
+__device__ __forceinline__ void ray_direction(const omerf_camera &cam, int u, int v, float &dx, float &dy, float &dz)
 {
-    // S2 (R19): every step one correctly rounded fp32 operation
     const float a = __fdiv_rn(__fsub_rn(__fadd_rn(__int2float_rn(u), 0.5f), cam.cx), cam.fx);
     const float b = -__fdiv_rn(__fsub_rn(__fadd_rn(__int2float_rn(v), 0.5f), cam.cy), cam.fy);
     const float gx = __fmaf_rn(a, cam.right[0], __fmaf_rn(b, cam.up[0], cam.fwd[0]));
@@ -457,12 +455,19 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
     const float gz = __fmaf_rn(a, cam.right[2], __fmaf_rn(b, cam.up[2], cam.fwd[2]));
     const float len2 = __fmaf_rn(gx, gx, __fmaf_rn(gy, gy, __fmul_rn(gz, gz)));
     const float inv = __fdiv_rn(1.0f, __fsqrt_rn(len2));
+    dx = __fmul_rn(gx, inv);
+    dy = __fmul_rn(gy, inv);
+    dz = __fmul_rn(gz, inv);
+}
+
+// Returns false when the ray cannot have samples (misses the padded box).
+__device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera &cam, int u, int v, Ray &r, int &k,
+                                          int &k1)
+{
+    ray_direction(cam, u, v, r.dx, r.dy, r.dz);
     r.ox = cam.origin[0];
     r.oy = cam.origin[1];
     r.oz = cam.origin[2];
-    r.dx = __fmul_rn(gx, inv);
-    r.dy = __fmul_rn(gy, inv);
-    r.dz = __fmul_rn(gz, inv);
     r.ix = r.dx != 0.0f ? __fdividef(1.0f, r.dx) : INFINITY; // proposals only: approximate is fine
     r.iy = r.dy != 0.0f ? __fdividef(1.0f, r.dy) : INFINITY;
     r.iz = r.dz != 0.0f ? __fdividef(1.0f, r.dz) : INFINITY;
@@ -529,10 +534,12 @@ __device__ __forceinline__ uint32_t pack_meta(int status, int lvl, uint32_t view
 #ifndef OMERF_MIN_BLOCKS
 #define OMERF_MIN_BLOCKS 5
 #endif
-template <int SAMPLER>
+// LOG (gather calibration only): every sample taken is appended to sample_log as (pixel, lattice index).
+template <int SAMPLER, bool LOG>
 __global__ void __launch_bounds__(32 * OMERF_WARPS, OMERF_MIN_BLOCKS)
 omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__restrict__ cams, int n_views, int W, int H,
-                   float *__restrict__ out_rgb, uint32_t *__restrict__ out_n, unsigned int *__restrict__ tile_counter)
+                   float *__restrict__ out_rgb, uint32_t *__restrict__ out_n, unsigned int *__restrict__ tile_counter,
+                   uint2 *__restrict__ sample_log, unsigned int log_capacity)
 {
     __shared__ WarpPool pools[OMERF_WARPS];
     WarpPool &P = pools[threadIdx.x >> 5];
@@ -727,6 +734,10 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                 if (status == ST_READY) {
                     float px, py, pz;
                     lattice_point(r, sc.step, k, px, py, pz);
+                    if (LOG) {
+                        const unsigned at = atomicAdd(tile_counter + 32, 1u);
+                        if (at < log_capacity) sample_log[at] = make_uint2(P.pix[slot], (uint32_t)k);
+                    }
                     uint32_t I[8];
                     gather_features(sc, px, py, pz, I);
                     float t[8];
@@ -818,10 +829,69 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
     }
 }
 
+// ---------------------------------------------------------------------------------- gather calibration
+// Replays the 20 feature loads (8 grid + 3 x 4 plane texels, 8 bytes each) of logged samples with no filtering,
+// activation or compositing: one sample per thread, every lane busy, full occupancy.  The rate it reaches is the
+// gather ceiling of this scene, camera and load width on this GPU; `order` selects frame order (the order the
+// march kernel took the samples) or a scattered order (multiplicative permutation of the log).
+__global__ void __launch_bounds__(256)
+omerf_gather_probe_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__restrict__ cam, int W,
+                          const uint2 *__restrict__ sample_log, unsigned int n, unsigned int mult, uint32_t *__restrict__ sink)
+{
+    const unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const unsigned int j = (unsigned int)(((unsigned long long)i * mult) % n);
+    const uint2 e = __ldg(sample_log + j);
+    const int v = (int)(e.x / (unsigned)W), u = (int)(e.x - (unsigned)v * (unsigned)W);
+    Ray r;
+    ray_direction(*cam, u, v, r.dx, r.dy, r.dz);
+    r.ox = cam->origin[0];
+    r.oy = cam->origin[1];
+    r.oz = cam->origin[2];
+    float px, py, pz;
+    lattice_point(r, sc.step, (int)e.y, px, py, pz);
+    int x0, x1, y0, y1, z0, z1, a0, a1, b0, b1;
+    uint32_t w;
+    axis_tap(px, sc.gs[0], sc.G[0], x0, x1, w);
+    axis_tap(py, sc.gs[1], sc.G[1], y0, y1, w);
+    axis_tap(pz, sc.gs[2], sc.G[2], z0, z1, w);
+    const uint32_t Gy = (uint32_t)sc.G[1], Gz = (uint32_t)sc.G[2];
+    const uint32_t c0 = (uint32_t)x0 * Gy, c1 = (uint32_t)x1 * Gy;
+    const uint32_t r00 = (c0 + (uint32_t)y0) * Gz, r01 = (c0 + (uint32_t)y1) * Gz;
+    const uint32_t r10 = (c1 + (uint32_t)y0) * Gz, r11 = (c1 + (uint32_t)y1) * Gz;
+    uint2 t[20];
+    t[0] = __ldg(sc.grid + (r00 + (uint32_t)z0)); t[1] = __ldg(sc.grid + (r00 + (uint32_t)z1));
+    t[2] = __ldg(sc.grid + (r01 + (uint32_t)z0)); t[3] = __ldg(sc.grid + (r01 + (uint32_t)z1));
+    t[4] = __ldg(sc.grid + (r10 + (uint32_t)z0)); t[5] = __ldg(sc.grid + (r10 + (uint32_t)z1));
+    t[6] = __ldg(sc.grid + (r11 + (uint32_t)z0)); t[7] = __ldg(sc.grid + (r11 + (uint32_t)z1));
+    axis_tap(px, sc.xy_s[0], sc.xy_n[0], a0, a1, w);
+    axis_tap(py, sc.xy_s[1], sc.xy_n[1], b0, b1, w);
+    plane_taps(sc.pxy, sc.xy_n[1], a0, a1, b0, b1, t + 8);
+    axis_tap(px, sc.xz_s[0], sc.xz_n[0], a0, a1, w);
+    axis_tap(pz, sc.xz_s[1], sc.xz_n[1], b0, b1, w);
+    plane_taps(sc.pxz, sc.xz_n[1], a0, a1, b0, b1, t + 12);
+    axis_tap(py, sc.yz_s[0], sc.yz_n[0], a0, a1, w);
+    axis_tap(pz, sc.yz_s[1], sc.yz_n[1], b0, b1, w);
+    plane_taps(sc.pyz, sc.yz_n[1], a0, a1, b0, b1, t + 16);
+    uint32_t x = 0;
+#pragma unroll
+    for (int q = 0; q < 20; q++) x ^= t[q].x + t[q].y;
+    sink[i] = x;
+}
+
 } // namespace
 
+int omerf_launch_gather_probe(const omerf_scene *s, const omerf_camera *d_cam, int W, const uint2 *sample_log,
+                              unsigned int n, unsigned int mult, uint32_t *sink, cudaStream_t st)
+{
+    if (n == 0) return OMERF_OK;
+    omerf_gather_probe_kernel<<<(n + 255) / 256, 256, 0, st>>>(s->dev, d_cam, W, sample_log, n, mult, sink);
+    OMERF_CUDA(cudaGetLastError());
+    return OMERF_OK;
+}
+
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H, float *out_rgb,
-                        uint32_t *out_n, cudaStream_t st, int *launches)
+                        uint32_t *out_n, cudaStream_t st, int *launches, uint2 *sample_log, unsigned int log_capacity)
 {
     if ((long long)((W + 7) / 8) * ((H + 3) / 4) * n_views > 0x7fffffffll || (long long)W * H * n_views > 0xffffffffll) {
         omerf_set_error("invalid argument: image or batch too large");
@@ -863,15 +933,20 @@ int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_
     }
     OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, 64 * sizeof(unsigned int), st));
 #else
-    OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, sizeof(unsigned int), st));
+    OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, (sample_log ? 64 : 1) * sizeof(unsigned int), st));
 #endif
     const int grid = s->persistent_blocks;
-    if (s->dev.sampler == OMERF_SAMPLER_PLANE)
-        omerf_march_kernel<OMERF_SAMPLER_PLANE><<<grid, 32 * OMERF_WARPS, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,
-                                                                       s->d_tile_counter);
-    else
-        omerf_march_kernel<OMERF_SAMPLER_GRID><<<grid, 32 * OMERF_WARPS, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,
-                                                                      s->d_tile_counter);
+#define OMERF_LAUNCH(SAMPLER, LOG)                                                                                          \
+    omerf_march_kernel<SAMPLER, LOG><<<grid, 32 * OMERF_WARPS, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,      \
+                                                                         s->d_tile_counter, sample_log, log_capacity)
+    if (s->dev.sampler == OMERF_SAMPLER_PLANE) {
+        if (sample_log) OMERF_LAUNCH(OMERF_SAMPLER_PLANE, true);
+        else OMERF_LAUNCH(OMERF_SAMPLER_PLANE, false);
+    } else {
+        if (sample_log) OMERF_LAUNCH(OMERF_SAMPLER_GRID, true);
+        else OMERF_LAUNCH(OMERF_SAMPLER_GRID, false);
+    }
+#undef OMERF_LAUNCH
     *launches = 1;
     OMERF_CUDA(cudaGetLastError());
     return OMERF_OK;
@@ -884,9 +959,9 @@ int omerf_query_persistent_blocks(int sampler, int *blocks)
     OMERF_CUDA(cudaGetDevice(&dev));
     OMERF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     if (sampler == OMERF_SAMPLER_PLANE)
-        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_PLANE>, 32 * OMERF_WARPS, 0));
+        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_PLANE, false>, 32 * OMERF_WARPS, 0));
     else
-        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_GRID>, 32 * OMERF_WARPS, 0));
+        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_GRID, false>, 32 * OMERF_WARPS, 0));
     *blocks = sms * (per_sm > 0 ? per_sm : 1);
     return OMERF_OK;
 }

@@ -198,3 +198,38 @@ def test_grid_sampler_parity_and_superset(omerf, oracle):
     rgb_p, ns_p, _ = _gpu_render(omerf, sc, cams, 64, 48, sampler=0)
     _assert_parity(rgb_p, ns_p, oracle.OracleScene(sc, sampler=0).render(cams, 64, 48, mode="brute"), "plane sampler")
     assert ns_g.sum() >= ns_p.sum()
+
+
+# ----------------------------------------------------------------------------- interpolation-weight corner cases
+def test_texel_centre_and_weight_256_taps(omerf, oracle):
+    """Samples exactly on texel centres (all four bilinear weights collapse to w00 = 2^16) and a hair below a
+    centre (fractional weight rounds to 256): the packed-u16 dot-product path of the gather must stay exact (R9)."""
+    sc = synth.custom_scene(box=(16.0, 16.0, 8.0), hf_n=(17, 17), h_lo=1.0, h_up=6.0, grid_n=(16, 16, 8),
+                            xy_n=(64, 64), xz_n=(64, 32), yz_n=(64, 32), seed=5, step=0.25, smooth=False)
+    cams = []
+    for dx, dy in ((0.0, 0.0), (-0.25 / 1024, 0.0), (0.0, -0.25 / 1024), (-0.25 / 1024, -0.25 / 1024), (0.125, 0.0)):
+        # principal ray straight down through a texel centre of the 0.25-spaced planes (and the shifted variants);
+        # z samples fall on texel centres of the xz / yz planes as well: 12 - (k + 1/2)/4 = (j + 1/2)/4
+        row = np.array([5.125 + dx, 7.375 + dy, 12.0, 1, 0, 0, 0, 1, 0, 0, 0, -1, 40.0, 40.0, 1.5, 1.5], dtype=np.float32)
+        cams.append(row)
+    cams = np.stack(cams)
+    rgb, ns, _ = _gpu_render(omerf, sc, cams, 3, 3)
+    ref = oracle.OracleScene(sc).render(cams, 3, 3, mode="brute")
+    assert ref["nsamples"][:, 1, 1].min() >= 1
+    _assert_parity(rgb, ns, ref, "texel-centre taps")
+
+
+def test_gather_probe_replays_every_sample(omerf):
+    import torch
+    sc, cams = synth.make_scene(0), synth.make_cameras(0)
+    W, H = synth.config_resolution(0)
+    with omerf.scene_create(sc) as h:
+        _, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        res = omerf.gather_probe(h, cams[0], W, H, repeats=2, flush_l2=False)
+        assert res["samples"] == int(ns.sum().item())
+        assert res["ms_frame_order"] > 0 and res["ms_scattered"] > 0
+        # the probe must leave the scene usable
+        _, ns2 = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        assert torch.equal(ns, ns2)
