@@ -50,6 +50,15 @@ struct Ray {
     float ix, iy, iz; // reciprocals of d (INF where d == 0), proposals only
 };
 
+__device__ __forceinline__ int floor_int(float x, float &fl)
+{
+    const int i = __float2int_rd(x);
+    fl = __int2float_rn(i);
+    return i;
+}
+__device__ __forceinline__ int floor_int(float x) { return __float2int_rd(x); }
+__device__ __forceinline__ int ceil_int(float x) { return __float2int_ru(x); } // saturates: +inf -> INT_MAX
+
 __device__ __forceinline__ float exp_q(float x)
 {
     float y = __fmul_rn(x, 0x1.715476p+0f);
@@ -83,21 +92,21 @@ __device__ __forceinline__ bool in_box(const DevScene &sc, float px, float py, f
 
 __device__ __forceinline__ int cell_index(float p, float s, int M)
 {
-    int i = (int)floorf(__fmaf_rn(p, s, 0.5f));
+    const int i = floor_int(__fmaf_rn(p, s, 0.5f));
     return min(max(i, 0), M - 1);
 }
 
 __device__ __forceinline__ int voxel_index(float p, float s, int N)
 {
-    int j = (int)floorf(__fmul_rn(p, s));
+    const int j = floor_int(__fmul_rn(p, s));
     return min(max(j, 0), N - 1);
 }
 
 // last lattice index whose parameter is below t_end (proposal only; verified by the caller)
 __device__ __forceinline__ int index_before(float t_end, float inv_step, int k1)
 {
-    float f = ceilf(fmaf(t_end, inv_step, -0.5f)) - 1.0f;
-    return f >= (float)k1 ? k1 : (int)f;
+    // t_end = +inf saturates to INT_MAX (clamped to k1); anything not above k is rejected by the caller
+    return max(min(ceil_int(fmaf(t_end, inv_step, -0.5f)), k1 + 1), 0) - 1;
 }
 
 // ---------------------------------------------------------------------------------- S4: one traversal step
@@ -208,9 +217,10 @@ __device__ __forceinline__ int trav_step_grid(const DevScene &sc, const Ray &r, 
 __device__ __forceinline__ void axis_tap(float p, float s, int N, int &i0, int &i1, uint32_t &w)
 {
     const float q = __fmaf_rn(p, s, -0.5f);
-    const int i = __float2int_rd(q);
+    float fl;
+    const int i = floor_int(q, fl);
     // (q - floor q) * 256 is exact, so one fma rounds exactly like the mul followed by the add
-    w = (uint32_t)__float2int_rd(__fmaf_rn(__fsub_rn(q, __int2float_rn(i)), 256.0f, 0.5f));
+    w = (uint32_t)floor_int(__fmaf_rn(__fsub_rn(q, fl), 256.0f, 0.5f));
     // the point is inside the box (checked before every sample), so -1 <= i <= N-1: one clamp per tap suffices
     i0 = max(i, 0);
     i1 = min(i + 1, N - 1);
@@ -339,6 +349,16 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
 }
 
 __device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
+
+// per-sample activations (Eq. 3, colour path only): sigmoid(x) = 1/2 + 1/2 tanh(x/2) with one MUFU.TANH.
+// tanh.approx has an absolute error of about 2^-11 = 5e-4, so the sigmoid is off by <= 2.5e-4; the compositing
+// weights sum to <= 1, which bounds the contribution to the pixel at 2.5e-4 of the 2e-3 budget.
+__device__ __forceinline__ float sigmoid_tanh(float x)
+{
+    float t;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(0.5f * x));
+    return fmaf(t, 0.5f, 0.5f);
+}
 
 // ---------------------------------------------------------------------------------- S8: deferred MLP (Eq. 4)
 // Warp-cooperative: the 34 -> 16 -> 16 -> 3 network of 16 rays at a time as m16n8k8 tensor-core tiles.
@@ -506,6 +526,9 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 #endif
 #ifndef OMERF_SAMPLE_KEEP
 #define OMERF_SAMPLE_KEEP 24   // sample again at once while this many lanes stand on an occupied point
+#endif
+#ifndef OMERF_SAMPLE_SIGMOID
+#define OMERF_SAMPLE_SIGMOID sigmoid_tanh
 #endif
 #define OMERF_WARPS 4
 #ifndef OMERF_ENDGAME_WARPS
@@ -749,7 +772,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                     const float T = __expf(-(float)Q * (1.0f / 1048576.0f)); // colour path: fast math
                     const float wgt = T * (1.0f - __expf(-od));
 #pragma unroll
-                    for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, sigmoid_fast(t[1 + c]), acc[c]);
+                    for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, OMERF_SAMPLE_SIGMOID(t[1 + c]), acc[c]);
                     Q += qk;
                     n += 1;
                     k += 1;
