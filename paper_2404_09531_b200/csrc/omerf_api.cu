@@ -126,6 +126,7 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
             vn[p][i] = pn[p][i];
             vs[p][i] = (float)pn[p][i] / d->box[ax[p][i]];
         }
+    v.shared_taps = d->xy_n[0] == d->xz_n[0] && d->xy_n[1] == d->yz_n[0] && d->xz_n[1] == d->yz_n[1];
     v.deq_mul = d->deq_scale / 65536.0f;
     v.deq_add = 4.0f * d->deq_bias;
     v.step = d->step;

@@ -31,6 +31,7 @@ struct DevScene {
     int xy_n[2], xz_n[2], yz_n[2];
     float xy_s[2], xz_s[2], yz_s[2];
     const uint2 *pxy, *pxz, *pyz;
+    int shared_taps;       // xy_n[0] == xz_n[0], xy_n[1] == yz_n[0], xz_n[1] == yz_n[1]: three taps serve the six plane axes
     float deq_mul, deq_add; // scale/65536, 4*bias
     float step, inv_step;
     uint32_t q_stop;

@@ -312,28 +312,38 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
         ga[2] = __ldg(g + (r10 + (uint32_t)z0)); gb[2] = __ldg(g + (r10 + (uint32_t)z1));
         ga[3] = __ldg(g + (r11 + (uint32_t)z0)); gb[3] = __ldg(g + (r11 + (uint32_t)z1));
     }
-    // triplanes: xy sampled with (x,y), xz with (x,z), yz with (y,z)
-    int a0, a1, b0, b1;
-    uint32_t wa, wb;
+    // triplanes: xy sampled with (x,y), xz with (x,z), yz with (y,z).  When the planes share their resolution per
+    // world axis (every config: xy A x A, xz and yz A x B) a tap computed for one plane is the other plane's tap too
+    // (same scale, same arithmetic), so three taps serve all six plane axes.
     uint2 t1[4], t2[4], t3[4];
-    axis_tap(px, sc.xy_s[0], sc.xy_n[0], a0, a1, wa);
-    axis_tap(py, sc.xy_s[1], sc.xy_n[1], b0, b1, wb);
-    fold_tap(a0, a1, wa);
-    fold_tap(b0, b1, wb);
-    const BiW w1 = bilinear_weights(wa, wb, b0, b1);
-    plane_taps(sc.pxy, sc.xy_n[1], a0, a1, b0, b1, t1);
-    axis_tap(px, sc.xz_s[0], sc.xz_n[0], a0, a1, wa);
-    axis_tap(pz, sc.xz_s[1], sc.xz_n[1], b0, b1, wb);
-    fold_tap(a0, a1, wa);
-    fold_tap(b0, b1, wb);
-    const BiW w2 = bilinear_weights(wa, wb, b0, b1);
-    plane_taps(sc.pxz, sc.xz_n[1], a0, a1, b0, b1, t2);
-    axis_tap(py, sc.yz_s[0], sc.yz_n[0], a0, a1, wa);
-    axis_tap(pz, sc.yz_s[1], sc.yz_n[1], b0, b1, wb);
-    fold_tap(a0, a1, wa);
-    fold_tap(b0, b1, wb);
-    const BiW w3 = bilinear_weights(wa, wb, b0, b1);
-    plane_taps(sc.pyz, sc.yz_n[1], a0, a1, b0, b1, t3);
+    int xa0, xa1, ya0, ya1, za0, za1;
+    uint32_t xw, yw, zw;
+    axis_tap(px, sc.xy_s[0], sc.xy_n[0], xa0, xa1, xw);
+    axis_tap(py, sc.xy_s[1], sc.xy_n[1], ya0, ya1, yw);
+    axis_tap(pz, sc.xz_s[1], sc.xz_n[1], za0, za1, zw);
+    fold_tap(xa0, xa1, xw);
+    fold_tap(ya0, ya1, yw);
+    fold_tap(za0, za1, zw);
+    int xb0 = xa0, xb1 = xa1, yb0 = ya0, yb1 = ya1, zb0 = za0, zb1 = za1; // taps of xz axis 0, yz axis 0, yz axis 1
+    uint32_t xbw = xw, ybw = yw, zbw = zw;
+    if (!sc.shared_taps) {
+        axis_tap(px, sc.xz_s[0], sc.xz_n[0], xb0, xb1, xbw);
+        axis_tap(py, sc.yz_s[0], sc.yz_n[0], yb0, yb1, ybw);
+        axis_tap(pz, sc.yz_s[1], sc.yz_n[1], zb0, zb1, zbw);
+        fold_tap(xb0, xb1, xbw);
+        fold_tap(yb0, yb1, ybw);
+        fold_tap(zb0, zb1, zbw);
+    }
+    int b1;
+    b1 = ya1;
+    const BiW w1 = bilinear_weights(xw, yw, ya0, b1);
+    plane_taps(sc.pxy, sc.xy_n[1], xa0, xa1, ya0, b1, t1);
+    b1 = za1;
+    const BiW w2 = bilinear_weights(xbw, zw, za0, b1);
+    plane_taps(sc.pxz, sc.xz_n[1], xb0, xb1, za0, b1, t2);
+    b1 = zb1;
+    const BiW w3 = bilinear_weights(ybw, zbw, zb0, b1);
+    plane_taps(sc.pyz, sc.yz_n[1], yb0, yb1, zb0, b1, t3);
 
     uint32_t A[8], B[8];
 #pragma unroll
@@ -761,6 +771,16 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                         const unsigned at = atomicAdd(tile_counter + 32, 1u);
                         if (at < log_capacity) sample_log[at] = make_uint2(P.pix[slot], (uint32_t)k);
                     }
+                    // Inside the slab the next lattice point is usually occupied too: test it here (level 0).  The test
+                    // does not depend on the features, so its pyramid load is in flight together with the gather.
+                    bool next_ready = false;
+                    if (SAMPLER == OMERF_SAMPLER_PLANE) {
+                        float qx, qy, qz;
+                        lattice_point(r, sc.step, k + 1, qx, qy, qz);
+                        const int ix = cell_index(qx, sc.sx, sc.Mx), iy = cell_index(qy, sc.sy, sc.My);
+                        const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
+                        next_ready = k < k1 && h.x <= qz && qz <= h.y && in_box(sc, qx, qy, qz);
+                    }
                     uint32_t I[8];
                     gather_features(sc, px, py, pz, I);
                     float t[8];
@@ -779,15 +799,8 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                     if (Q >= sc.q_stop) {
                         status = ST_FIN; // early stop (R7)
                     } else {
-                        // inside the slab the next lattice point is usually occupied too: test it here (level 0)
-                        status = ST_TRAV;
+                        status = next_ready ? ST_READY : ST_TRAV;
                         lvl = 0;
-                        if (SAMPLER == OMERF_SAMPLER_PLANE && k <= k1) {
-                            lattice_point(r, sc.step, k, px, py, pz);
-                            const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
-                            const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
-                            if (h.x <= pz && pz <= h.y && in_box(sc, px, py, pz)) status = ST_READY;
-                        }
                     }
                 }
                 if (__popc(__ballot_sync(FULL, status == ST_READY)) < OMERF_SAMPLE_KEEP) break;

@@ -233,3 +233,19 @@ def test_gather_probe_replays_every_sample(omerf):
         _, ns2 = omerf.render(h, cams, W, H)
         torch.cuda.synchronize()
         assert torch.equal(ns, ns2)
+
+
+def test_planes_with_unrelated_resolutions(omerf, oracle):
+    """Plane resolutions that differ per world axis: the gather may not share taps between planes."""
+    rng = np.random.default_rng(9)
+    m = 21
+    lo = (1.0 + rng.random((m, m))).astype(np.float32)
+    hi = (lo + 0.5 + 2.0 * rng.random((m, m))).astype(np.float32)
+    sc = synth.custom_scene(box=(10.0, 12.0, 5.0), hf_n=(m, m), h_lo=lo, h_up=hi, grid_n=(7, 9, 5), xy_n=(20, 24),
+                            xz_n=(28, 12), yz_n=(36, 10), seed=4, step=0.2, bias_amp=0.3)
+    cams = np.stack([synth.look_at_camera((5.0, -7.0, 11.0), (5.0, 6.0, 2.0), 48, 40),
+                     synth.look_at_camera((1.0, 2.0, 2.2), (9.0, 10.0, 1.5), 48, 40)])
+    rgb, ns, _ = _gpu_render(omerf, sc, cams, 48, 40)
+    ref = oracle.OracleScene(sc).render(cams, 48, 40, mode="brute")
+    assert ref["nsamples"].sum() > 2000
+    _assert_parity(rgb, ns, ref, "unrelated plane resolutions")
