@@ -166,6 +166,47 @@ __device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r,
     return ST_TRAV;
 }
 
+// The same step without branches (selects only): two rays per lane can then be interleaved by the compiler, which
+// doubles the loads in flight of this latency-bound loop, and the warp no longer serialises the inside / jump /
+// descend paths.  Semantics are identical to trav_step_plane (kept above as the readable statement of the step).
+__device__ __forceinline__ int trav_step_plane_bf(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl, int status)
+{
+    const bool run = status == ST_TRAV && k <= k1;
+    float px, py, pz;
+    lattice_point(r, sc.step, k, px, py, pz);
+    const int top = sc.n_levels - 1;
+    const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
+    const int nx = ix >> lvl, ny = iy >> lvl;
+    const float2 h = __ldg(sc.pyr + sc.lvl_off[lvl] + nx * sc.lvl_ny[lvl] + ny);
+    const bool above = pz > h.y, below = pz < h.x, inside = !above && !below;
+    const int bxi = nx + (r.dx > 0.0f ? 1 : 0), byi = ny + (r.dy > 0.0f ? 1 : 0);
+    const float xb = fmaf((float)(bxi << lvl), sc.cell_x, -0.5f * sc.cell_x);
+    const float yb = fmaf((float)(byi << lvl), sc.cell_y, -0.5f * sc.cell_y);
+    const float tx = r.dx != 0.0f ? (xb - r.ox) * r.ix : INFINITY;
+    const float ty = r.dy != 0.0f ? (yb - r.oy) * r.iy : INFINITY;
+    float tz = INFINITY;
+    if (above && !below && r.dz < 0.0f) tz = (h.y - r.oz) * r.iz;
+    if (below && !above && r.dz > 0.0f) tz = (h.x - r.oz) * r.iz;
+    const float txy = fminf(tx, ty);
+    const int kk = index_before(fminf(txy, tz), sc.inv_step, k1);
+    float qx, qy, qz;
+    lattice_point(r, sc.step, kk, qx, qy, qz);
+    const int jx = cell_index(qx, sc.sx, sc.Mx) >> lvl, jy = cell_index(qy, sc.sy, sc.My) >> lvl;
+    const bool same_side = (above ? qz > h.y : true) && (below ? qz < h.x : true);
+    const bool jump = !inside && kk > k && jx == nx && jy == ny && same_side;
+    const bool ready = run && inside && lvl == 0 && in_box(sc, px, py, pz);
+    // next (k, lvl)
+    const int crossed = tx <= ty ? bxi : byi;
+    const int lvl_jump = tz <= txy ? max(lvl - 2, 0) : min(lvl + ((crossed & 1) ^ 1), top);
+    const int lvl_next = inside ? max(lvl - 2, 0) : (jump ? lvl_jump : max(lvl - 1, 0));
+    const int k_next = jump ? kk + 1 : ((lvl == 0 && !ready) ? k + 1 : k); // level 0 and the predicate is false at k
+    if (run) {
+        k = k_next;
+        lvl = lvl_next;
+    }
+    return status != ST_TRAV ? status : (k > k1 && !ready ? ST_FIN : (ready ? ST_READY : ST_TRAV));
+}
+
 __device__ __forceinline__ bool occ_test(const DevScene &sc, int lvl, int jx, int jy, int jz)
 {
     unsigned long long idx = ((unsigned long long)jx * sc.occ_ny[lvl] + jy) * sc.occ_nz[lvl] + jz;
@@ -555,13 +596,80 @@ struct WarpPool {
     int k[OMERF_POOL], k1[OMERF_POOL];
     uint32_t Q[OMERF_POOL], n[OMERF_POOL], pix[OMERF_POOL];
     float acc[7][OMERF_POOL];
-    uint32_t list[32];
+    uint32_t list[32];      // slots picked for this round
     float X[16 * OMERF_XS]; // staged MLP inputs of 16 rays
 };
 
 __device__ __forceinline__ uint32_t pack_meta(int status, int lvl, uint32_t view)
 {
     return (uint32_t)status | ((uint32_t)lvl << 2) | (view << 8);
+}
+
+// ---------------------------------------------------------------------------------- S4: one traversal visit
+// A few steps of the hierarchical DDA for the first min(n_sel, 32 R) listed rays, R rays per lane.
+template <int SAMPLER, int R>
+__device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, const omerf_camera *__restrict__ cams, int lane,
+                                           int n_sel, float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
+{
+                int status[R], k[R], k1[R], lvl[R], sl[R];
+                uint32_t view[R];
+                Ray r[R];
+                const int n_trav = min(n_sel, 32 * R);
+                const unsigned FULL = 0xffffffffu;
+    #pragma unroll
+                for (int q = 0; q < R; q++) {
+                    const bool on = lane + 32 * q < n_trav;
+                    sl[q] = on ? (int)P.list[lane + 32 * q] : -1;
+                    const int s_ = on ? sl[q] : 0; // idle lanes read slot 0 and step nothing
+                    const uint32_t m = P.meta[s_];
+                    status[q] = on ? ST_TRAV : ST_IDLE;
+                    lvl[q] = (int)((m >> 2) & 31u);
+                    view[q] = m >> 8;
+                    k[q] = P.k[s_];
+                    k1[q] = P.k1[s_];
+                    r[q].dx = P.dx[s_];
+                    r[q].dy = P.dy[s_];
+                    r[q].dz = P.dz[s_];
+                    r[q].ox = __ldg(&cams[view[q]].origin[0]);
+                    r[q].oy = __ldg(&cams[view[q]].origin[1]);
+                    r[q].oz = __ldg(&cams[view[q]].origin[2]);
+                    r[q].ix = r[q].dx != 0.0f ? __fdividef(1.0f, r[q].dx) : INFINITY;
+                    r[q].iy = r[q].dy != 0.0f ? __fdividef(1.0f, r[q].dy) : INFINITY;
+                    r[q].iz = r[q].dz != 0.0f ? __fdividef(1.0f, r[q].dz) : INFINITY;
+                }
+                const int keep = n_trav > 32 ? 2 * OMERF_TRAV_KEEP : OMERF_TRAV_KEEP;
+    #pragma unroll 1
+                for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
+                    int left = 0;
+    #pragma unroll
+                    for (int q = 0; q < R; q++) {
+                        if (SAMPLER == OMERF_SAMPLER_PLANE) {
+                            status[q] = trav_step_plane_bf(sc, r[q], k[q], k1[q], lvl[q], status[q]);
+                        } else {
+                            if (status[q] == ST_TRAV) status[q] = trav_step_grid(sc, r[q], k[q], k1[q], lvl[q]);
+                        }
+                    }
+    #pragma unroll
+                    for (int q = 0; q < R; q++) left += __popc(__ballot_sync(FULL, status[q] == ST_TRAV));
+                    if (left < keep) break;
+                }
+    #pragma unroll
+                for (int q = 0; q < R; q++) {
+                    if (sl[q] >= 0) {
+                        const int s_ = sl[q];
+                        int st_ = status[q];
+                        if (st_ == ST_FIN && P.n[s_] == 0) { // no sample at all: background exactly, MLP skipped (R14)
+                            const size_t pix = P.pix[s_];
+                            out_rgb[pix * 3 + 0] = sc.bg[0];
+                            out_rgb[pix * 3 + 1] = sc.bg[1];
+                            out_rgb[pix * 3 + 2] = sc.bg[2];
+                            out_n[pix] = 0;
+                            st_ = ST_IDLE;
+                        }
+                        P.k[s_] = k[q];
+                        P.meta[s_] = pack_meta(st_, lvl[q], view[q]);
+                    }
+                }
 }
 
 #ifndef OMERF_MIN_BLOCKS
@@ -695,48 +803,9 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                 }
             }
         } else if (phase == ST_TRAV) {
-            // ---- traversal visit: a few steps of the hierarchical DDA (S4)
-            int status = ST_IDLE, k = 0, k1 = -1, lvl = 0;
-            uint32_t view = 0;
-            Ray r;
-            if (active) {
-                const uint32_t m = P.meta[slot];
-                status = ST_TRAV;
-                lvl = (int)((m >> 2) & 31u);
-                view = m >> 8;
-                k = P.k[slot];
-                k1 = P.k1[slot];
-                r.dx = P.dx[slot];
-                r.dy = P.dy[slot];
-                r.dz = P.dz[slot];
-                r.ox = __ldg(&cams[view].origin[0]);
-                r.oy = __ldg(&cams[view].origin[1]);
-                r.oz = __ldg(&cams[view].origin[2]);
-                r.ix = r.dx != 0.0f ? __fdividef(1.0f, r.dx) : INFINITY;
-                r.iy = r.dy != 0.0f ? __fdividef(1.0f, r.dy) : INFINITY;
-                r.iz = r.dz != 0.0f ? __fdividef(1.0f, r.dz) : INFINITY;
-            }
-#pragma unroll 1
-            for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
-#ifdef OMERF_X_STATS
-                { unsigned m = __ballot_sync(FULL, status == ST_TRAV); if (lane == 0) { atomicAdd(tile_counter + 9, 1u); atomicAdd(tile_counter + 10, (unsigned)__popc(m)); } }
-#endif
-                if (status == ST_TRAV)
-                    status = SAMPLER == OMERF_SAMPLER_PLANE ? trav_step_plane(sc, r, k, k1, lvl) : trav_step_grid(sc, r, k, k1, lvl);
-                if (__popc(__ballot_sync(FULL, status == ST_TRAV)) < OMERF_TRAV_KEEP) break;
-            }
-            if (active) {
-                if (status == ST_FIN && P.n[slot] == 0) { // no sample at all: background exactly, MLP skipped (R14)
-                    const size_t pix = P.pix[slot];
-                    out_rgb[pix * 3 + 0] = sc.bg[0];
-                    out_rgb[pix * 3 + 1] = sc.bg[1];
-                    out_rgb[pix * 3 + 2] = sc.bg[2];
-                    out_n[pix] = 0;
-                    status = ST_IDLE;
-                }
-                P.k[slot] = k;
-                P.meta[slot] = pack_meta(status, lvl, view);
-            }
+            // ---- traversal visit (S4).  R = 2 rays per lane (interleaved dependency chains) was measured slower on
+            // B200 at every threshold (0.80-0.86 ms against 0.76 ms per configs[1] frame), so one ray per lane it is.
+            trav_visit<SAMPLER, 1>(sc, P, cams, lane, n_sel, out_rgb, out_n);
         } else if (phase == ST_READY) {
             // ---- samples: gather, activations, compositing (S5, S6, S7)
             int status = ST_IDLE, k = 0, k1 = -1, lvl = 0;
