@@ -44,7 +44,8 @@ ALU_PEAK_TOPS = 148 * 128 * 1.965e9 / 1e12   # B200: SMs x fp32/int lanes x max 
 def workload_name(cfg: int) -> str:
     return {0: "configs[0] tiny 128x128", 1: "configs[1] 1080p oblique frame, 1000x1000x100 m scene",
             2: "configs[2] 16 x 1080p views", 3: "configs[3] 8 x 2160p views, 4000x4000x200 m scene",
-            4: "configs[4] sampling ablation (config-1 scene+camera)"}[cfg]
+            4: "configs[4] sampling ablation (config-1 scene+camera)",
+            5: "SURVEY 8(f).4 low-altitude cameras: 4 x 1080p views inside the config-1 box"}[cfg]
 
 
 class ClockSampler:
@@ -323,7 +324,7 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4, 5])
     ap.add_argument("--sampler", default="plane", choices=["plane", "grid"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -30,6 +30,7 @@ class _Scene(C.Structure):
         ("W0", _f32p), ("b0", _f32p), ("W1", _f32p), ("b1", _f32p), ("W2", _f32p), ("b2", _f32p),
         ("step", C.c_float), ("t_stop", C.c_float), ("bg", C.c_float * 3),
         ("sampler", C.c_int32), ("occ_n", C.c_int32 * 3), ("occ_bits", _u32p),
+        ("soft_eps", C.c_float),
     ]
 
 
@@ -40,6 +41,7 @@ def lib():
     global _lib
     if _lib is None:
         L = C.CDLL(_build())
+        L.orc_soft_mask.restype = C.c_double
         L.orc_exp_q.restype = C.c_float
         L.orc_exp_q.argtypes = [C.c_float]
         L.orc_q_stop.restype = C.c_uint32
@@ -69,7 +71,7 @@ def q_stop(t_stop: float) -> int:
 class OracleScene:
     """Holds a synth.Scene (keeps the numpy arrays alive) and its C view."""
 
-    def __init__(self, scene, sampler: int = 0):
+    def __init__(self, scene, sampler: int = 0, soft_eps: float = 0.0):
         self.scene = scene
         s = _Scene()
         self._keep = []
@@ -98,6 +100,7 @@ class OracleScene:
         s.step, s.t_stop = scene.step, scene.t_stop
         s.bg[:] = scene.bg
         s.sampler = sampler
+        s.soft_eps = soft_eps
         s.occ_n[:] = scene.occ_n
         self.c = s
         self.bits = None
@@ -142,6 +145,10 @@ class OracleScene:
         p = np.ascontiguousarray(p, dtype=np.float32)
         f = lib().orc_occupied_plane if self.c.sampler == 0 else lib().orc_occupied_grid
         return bool(f(C.byref(self.c), _ptr(p, _f32p)))
+
+    def soft_mask(self, p) -> float:
+        p = np.ascontiguousarray(p, dtype=np.float32)
+        return float(lib().orc_soft_mask(C.byref(self.c), _ptr(p, _f32p)))
 
     def mlp(self, x):
         x = np.ascontiguousarray(x, dtype=np.float64)

@@ -16,6 +16,7 @@
  *   - tau = exp(t0), c^d = sigmoid(t1..3), f = sigmoid(t4..7)      PAPER.md:74-77 (Eq. 3)
  *   - C = sum_i w_i c_i, w_i = T_i alpha_i, alpha = 1 - e^{-tau d} PAPER.md:65-67 (Eq. 1), :122 (Eq. 8, binary M)
  *   - C = sum w c^d + G([sum w c^d, sum w f], d)                   PAPER.md:79-81 (Eq. 4)
+ *   - optional soft occupancy M of Eq. 6 (q = 2) weighting w_i       PAPER.md:114-122 (Eq. 6-8), SURVEY 8(f).2
  * The occupancy-plane *marching* of PAPER.md:188 is an exact acceleration (it
  * reaches the same samples), so it does NOT appear here: the oracle is the plain
  * definition — every lattice sample tested with the per-sample predicate.
@@ -63,6 +64,7 @@ typedef struct {
     int32_t sampler;                    /* 0 occupancy plane, 1 binary occupancy grid (config 4) */
     int32_t occ_n[3];
     const uint32_t *occ_bits;           /* sampler 1: bit index ((jx*Ny+jy)*Nz+jz), LSB-first words */
+    float soft_eps;                     /* > 0: soft occupancy function of Eq. 6 with buffer eps; 0: binary mask */
 } orc_scene;
 
 typedef struct {
@@ -140,6 +142,26 @@ int orc_occupied_plane(const orc_scene *s, const float p[3])
     float lo = s->h_lo[(size_t)ix * My + iy];
     float hi = s->h_up[(size_t)ix * My + iy];
     return lo <= p[2] && p[2] <= hi;
+}
+
+/* Soft occupancy function M of Eq. 6, exponent q = 2, evaluated at the nearest grid
+ * point of P_o (Eq. 7).  Written as the paper's four cases; where the two buffer zones overlap (interval thinner than
+ * 2 eps - the paper is silent, R23) the smaller of the two ramps is taken, which keeps M continuous. */
+double orc_soft_mask(const orc_scene *s, const float p[3])
+{
+    int Mx = s->hf_n[0], My = s->hf_n[1];
+    float sx = (float)(Mx - 1) / s->box[0];
+    float sy = (float)(My - 1) / s->box[1];
+    int ix = clampi((int)floorf(fmaf(p[0], sx, 0.5f)), 0, Mx - 1);
+    int iy = clampi((int)floorf(fmaf(p[1], sy, 0.5f)), 0, My - 1);
+    double zmin = (double)s->h_lo[(size_t)ix * My + iy], zmax = (double)s->h_up[(size_t)ix * My + iy];
+    double z = (double)p[2], eps = (double)s->soft_eps;
+    if (z < zmin || z > zmax) return 0.0;                         /* second case of Eq. 6 */
+    if (!(eps > 0.0)) return 1.0;                                 /* binary mask (R3) */
+    double m = 1.0;                                               /* first case */
+    if (z <= zmin + eps) { double a = (z - zmin) / eps; m = a * a; }          /* third case, q = 2 */
+    if (z >= zmax - eps) { double b = (zmax - z) / eps; if (b * b < m) m = b * b; } /* fourth case */
+    return m;
 }
 
 /* config-4 comparator: binary occupancy grid (the structure PAPER.md:188 replaces). */
@@ -406,8 +428,10 @@ static void render_pixel(const orc_scene *s, const orc_camera *cam, int u, int v
         double T = exp(-(double)Q * (1.0 / 1048576.0));       /* T_i = prod_{j<i}(1 - alpha_j) (R6) */
         double alpha = 1.0 - exp(-(double)od);
         double w = T * alpha;                                 /* omega_i = T_i alpha_i (Eq. 1) */
-        for (int c = 0; c < 3; c++) D[c] += w * sigmoid_d((double)t[1 + c]);
-        for (int c = 0; c < 4; c++) Fs[c] += w * sigmoid_d((double)t[4 + c]);
+        /* Eq. 8: the contribution of sample i is M_i omega_i c_i; M = 1 inside the interval for the binary mask */
+        double Mw = (s->soft_eps > 0.0f && s->sampler == 0) ? orc_soft_mask(s, p) * w : w;
+        for (int c = 0; c < 3; c++) D[c] += Mw * sigmoid_d((double)t[1 + c]);
+        for (int c = 0; c < 4; c++) Fs[c] += Mw * sigmoid_d((double)t[4 + c]);
         sum_w += w;
         Q += qk;
         n += 1;

@@ -14,6 +14,7 @@ from .scenes import (  # noqa: F401
     config_resolution,
     custom_scene,
     look_at_camera,
+    low_altitude_cameras,
     orbit_cameras,
     smoothed_bytes,
     CAMERA_FLOATS,

@@ -24,7 +24,7 @@ import numpy as np
 
 CAMERA_FLOATS = 16
 
-_CONFIG_RES = {0: (128, 128), 1: (1920, 1080), 2: (1920, 1080), 3: (3840, 2160), 4: (1920, 1080)}
+_CONFIG_RES = {0: (128, 128), 1: (1920, 1080), 2: (1920, 1080), 3: (3840, 2160), 4: (1920, 1080), 5: (1920, 1080)}
 
 
 def config_resolution(config: int) -> tuple[int, int]:
@@ -205,7 +205,7 @@ def make_scene(config: int) -> Scene:
     """Scene of BASELINE.json configs[config]; seed = scene index (configs 2 and 4 reuse config 1's)."""
     if config == 0:
         return _scene_tiny(0)
-    if config in (1, 2, 4):
+    if config in (1, 2, 4, 5):   # 5 = SURVEY 8(f) item 4: low-altitude cameras in the config-1 scene
         return _scene_city(1, (1000.0, 1000.0, 100.0), 1025, 30.0, 2000, (512, 512, 64), 4096, 512,
                            "cfg1_1080p", occ_n=(2048, 2048, 256))
     if config == 3:
@@ -266,7 +266,35 @@ def make_cameras(config: int) -> np.ndarray:
         pitch = np.linspace(30.0, 60.0, 8)
         return np.stack([_orbit_camera((2000.0, 2000.0, 100.0), pitch[i], yaw[i], z[i], W, H)
                          for i in range(8)])
+    if config == 5:
+        return low_altitude_cameras(make_scene(1), 4, rng, W, H)
     raise ValueError(f"unknown config {config}")
+
+
+def low_altitude_cameras(scene: Scene, n: int, rng, W: int, H: int) -> np.ndarray:
+    """SURVEY 8(f) item 4 / PAPER.md:226-234 (Table 3, low-altitude column): cameras INSIDE the box.
+    Even views stand in a street (a column without a block, 8 m above the upper height field) and look
+    10 degrees below the horizon; odd views sit inside the slab itself (mid-height of a column with a
+    block), so the first lattice samples of most rays are already occupied."""
+    X, Y, _ = scene.box
+    mx, my = scene.h_lo.shape
+    thick = (scene.h_up - scene.h_lo).astype(np.float64)
+    cams = []
+    for i in range(n):
+        want_block = bool(i & 1)
+        while True:
+            ix, iy = int(rng.integers(mx // 5, 4 * mx // 5)), int(rng.integers(my // 5, 4 * my // 5))
+            if (thick[ix, iy] > 15.0) == want_block:
+                break
+        x, y = ix * X / (mx - 1), iy * Y / (my - 1)
+        z = (0.5 * (float(scene.h_lo[ix, iy]) + float(scene.h_up[ix, iy])) if want_block
+             else float(scene.h_up[ix, iy]) + 8.0)
+        yaw = float(rng.uniform(0.0, 2.0 * math.pi))
+        pitch = math.radians(10.0)
+        tgt = (x + 100.0 * math.sin(yaw) * math.cos(pitch), y + 100.0 * math.cos(yaw) * math.cos(pitch),
+               z - 100.0 * math.sin(pitch))
+        cams.append(look_at_camera((x, y, z), tgt, W, H))
+    return np.stack(cams)
 
 
 def orbit_cameras(config: int, n: int) -> np.ndarray:

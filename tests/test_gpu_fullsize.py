@@ -94,3 +94,12 @@ def test_config3_large_scene(omerf):
     cams = synth.make_cameras(3)
     W, H = synth.config_resolution(3)
     _check_sampled(omerf, scene, cams, W, H, 0, 40000, [1080], seed=103)
+
+
+def test_config5_low_altitude_cameras(omerf, city):
+    """cameras inside the box, in streets and inside the slab (rays start occupied)."""
+    cams = synth.make_cameras(5)
+    W, H = synth.config_resolution(5)
+    rgb, ns = _check_sampled(omerf, city, cams, W, H, 0, 30000, [200, 700], seed=105)
+    per_view = ns.reshape(cams.shape[0], -1).sum(axis=1)
+    assert np.all(per_view > 0)
