@@ -95,10 +95,10 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_bounded(scene, cams, W, H, sampler=0, budget_s=15.0):
+def oracle_bounded(scene, cams, W, H, sampler=0, budget_s=15.0, soft_eps=0.0):
     """Time the oracle (clipped loop, OpenMP on all host cores) on every `stride`-th row of view 0."""
     import oracle
-    O = oracle.OracleScene(scene, sampler=sampler)
+    O = oracle.OracleScene(scene, sampler=sampler, soft_eps=soft_eps)
     t0 = time.perf_counter()
     probe_rows = list(range(0, H, max(H // 8, 1)))[:8]
     n = 0
@@ -136,7 +136,7 @@ def run_reference(args):
     budget = 120.0 / max(args.steps + args.warmup, 1)
     times, res = [], None
     for i in range(args.warmup + args.steps):
-        res = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=min(budget, 20.0))
+        res = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=min(budget, 20.0), soft_eps=args.soft_eps)
         if i >= args.warmup:
             times.append(res)
     mp = float(np.mean([r["mpix_s"] for r in times]))
@@ -189,7 +189,7 @@ def run_ours(args):
     W, H = synth.config_resolution(cfg)
     n_views = cams.shape[0]
     sampler = omerf.SAMPLER_GRID if args.sampler == "grid" else omerf.SAMPLER_PLANE
-    h = omerf.scene_create(scene, sampler=sampler)
+    h = omerf.scene_create(scene, sampler=sampler, soft_eps=args.soft_eps)
     info = omerf.scene_info(h)
     out_rgb = torch.empty((n_views, H, W, 3), dtype=torch.float32, device="cuda")
     out_n = torch.empty((n_views, H, W), dtype=torch.int32, device="cuda")
@@ -269,7 +269,7 @@ def run_ours(args):
         alu_ops = samples * OPS_PER_SAMPLE + pixels * OPS_PER_PIXEL
         cpu = None
         if not args.no_cpu_baseline:
-            cpu = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=15.0)
+            cpu = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=15.0, soft_eps=args.soft_eps)
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tpath):
@@ -279,7 +279,7 @@ def run_ours(args):
             "steps": k, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32 (u8 features, integer interpolation)",
             "data": "synthetic",
-            "config": {"workload": workload_name(cfg), "views": n_views, "W": W, "H": H, "sampler": args.sampler,
+            "config": {"workload": workload_name(cfg), "views": n_views, "W": W, "H": H, "sampler": args.sampler, "soft_eps": args.soft_eps,
                        "scene_device_bytes": info["device_bytes"], "l2": "flushed between timed steps (256 MiB fill, "
                        "outside the event pairs); scene 296 MiB > L2", "parallelism": f"replicated scene x{world}"},
             "frames_per_s": world * n_views * k / secs,
@@ -326,6 +326,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4, 5])
     ap.add_argument("--sampler", default="plane", choices=["plane", "grid"])
+    ap.add_argument("--soft-eps", type=float, default=0.0, help="SURVEY 8(f).2: soft occupancy (Eq. 6-8) buffer height; 0 = binary mask")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -56,6 +56,11 @@ typedef struct {
     float bg[3];    /* background colour */
     int32_t sampler; /* OMERF_SAMPLER_PLANE or OMERF_SAMPLER_GRID */
     int32_t occ_n[3]; /* sampler GRID: bitfield resolution (e.g. 2048,2048,256); derived on the device from the slab */
+    float soft_eps;   /* 0: binary mask (render time).  > 0, sampler PLANE only: the soft occupancy
+                         function M of Eq. 6 (q = 2) with buffer zones of height soft_eps weights every
+                         sample's colour contribution, C = sum_i M_i w_i c_i (Eq. 8) - the training-time
+                         forward pass.  Samples, transmittance and termination are those of the binary mask; where the
+                         two buffers of a thin interval overlap the smaller ramp is taken (R23). */
 } omerf_scene_desc;
 
 /* Pinhole camera, world frame. */

@@ -40,6 +40,7 @@ class SceneDesc(C.Structure):
         ("W0", _f32p), ("b0", _f32p), ("W1", _f32p), ("b1", _f32p), ("W2", _f32p), ("b2", _f32p),
         ("step", C.c_float), ("t_stop", C.c_float), ("bg", C.c_float * 3),
         ("sampler", C.c_int32), ("occ_n", C.c_int32 * 3),
+        ("soft_eps", C.c_float),
     ]
 
 
@@ -95,7 +96,7 @@ def _np(a, dt):
     return np.ascontiguousarray(a, dtype=dt)
 
 
-def make_desc(scene, sampler: int = SAMPLER_PLANE):
+def make_desc(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0):
     """Fill an omerf_scene_desc from an object with synth.Scene's attributes. Returns (desc, keepalive)."""
     d = SceneDesc()
     keep = []
@@ -124,6 +125,7 @@ def make_desc(scene, sampler: int = SAMPLER_PLANE):
     d.step, d.t_stop = scene.step, scene.t_stop
     d.bg[:] = scene.bg
     d.sampler = sampler
+    d.soft_eps = soft_eps
     d.occ_n[:] = scene.occ_n
     return d, keep
 
@@ -147,7 +149,7 @@ class SceneHandle:
             pass
 
 
-def scene_create(scene, sampler: int = SAMPLER_PLANE) -> SceneHandle:
+def scene_create(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0) -> SceneHandle:
     """omerf_scene_create: upload + re-layout + pyramid (+ bitfield) on the current CUDA device."""
     import torch
     if not torch.cuda.is_available():
@@ -155,7 +157,7 @@ def scene_create(scene, sampler: int = SAMPLER_PLANE) -> SceneHandle:
     torch.cuda.init()
     torch.cuda.current_stream()          # make sure torch's primary context is current
     L = load_library()
-    d, keep = make_desc(scene, sampler)
+    d, keep = make_desc(scene, sampler, soft_eps)
     out = C.c_void_p()
     _check(L.omerf_scene_create(C.byref(d), C.byref(out)), "omerf_scene_create")
     del keep

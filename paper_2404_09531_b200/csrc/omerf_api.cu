@@ -90,6 +90,8 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
     if (!(d->step > 0) || !isfinite(d->step)) return invalid("step must be > 0");
     if (!(d->t_stop > 0 && d->t_stop < 1)) return invalid("t_stop must be in (0,1)");
     if (d->sampler != OMERF_SAMPLER_PLANE && d->sampler != OMERF_SAMPLER_GRID) return invalid("unknown sampler");
+    if (!(d->soft_eps >= 0) || !isfinite(d->soft_eps)) return invalid("soft_eps must be >= 0");
+    if (d->soft_eps > 0 && d->sampler != OMERF_SAMPLER_PLANE) return invalid("soft_eps needs the occupancy-plane sampler");
     if (d->sampler == OMERF_SAMPLER_GRID)
         for (int i = 0; i < 3; i++)
             if (d->occ_n[i] < 1) return invalid("occ_n must be >= 1 for the grid sampler");
@@ -134,6 +136,8 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
     v.q_stop = (uint32_t)ceil(-log((double)d->t_stop) * 1048576.0);
     for (int i = 0; i < 3; i++) v.bg[i] = d->bg[i];
     v.sampler = d->sampler;
+    v.soft_eps = d->soft_eps;
+    v.inv_soft_eps = d->soft_eps > 0 ? 1.0f / d->soft_eps : 0.0f;
 
     int rc = OMERF_OK;
     float *d_lo = nullptr, *d_up = nullptr;

@@ -36,6 +36,7 @@ struct DevScene {
     float step, inv_step;
     uint32_t q_stop;
     float bg[3];
+    float soft_eps, inv_soft_eps; // > 0: Eq. 6 soft occupancy weights the colour contributions (Eq. 8)
     // sampler GRID (config-4 comparator): multi-resolution binary occupancy grid
     int sampler;
     int N[3];

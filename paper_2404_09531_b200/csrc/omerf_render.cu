@@ -850,6 +850,15 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                         const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
                         next_ready = k < k1 && h.x <= qz && qz <= h.y && in_box(sc, qx, qy, qz);
                     }
+                    float soft_m = 1.0f;
+                    if (SAMPLER == OMERF_SAMPLER_PLANE && sc.soft_eps > 0.0f) {
+                        // Eq. 6 (q = 2) at the nearest grid point of P_o (Eq. 7): the sample is inside [z_min, z_max],
+                        // so M = min(1, ((z - z_min)/eps)^2, ((z_max - z)/eps)^2); it weights the colours only (Eq. 8)
+                        const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
+                        const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
+                        const float m = __saturatef(fminf(pz - h.x, h.y - pz) * sc.inv_soft_eps);
+                        soft_m = m * m;
+                    }
                     uint32_t I[8];
                     gather_features(sc, px, py, pz, I);
                     float t[8];
@@ -859,7 +868,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                     const float od = __fmul_rn(tau, sc.step);
                     const uint32_t qk = (uint32_t)rintf(fminf(__fmul_rn(od, 1048576.0f), (float)sc.q_stop));
                     const float T = __expf(-(float)Q * (1.0f / 1048576.0f)); // colour path: fast math
-                    const float wgt = T * (1.0f - __expf(-od));
+                    const float wgt = T * (1.0f - __expf(-od)) * soft_m;
 #pragma unroll
                     for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, OMERF_SAMPLE_SIGMOID(t[1 + c]), acc[c]);
                     Q += qk;

@@ -249,3 +249,40 @@ def test_planes_with_unrelated_resolutions(omerf, oracle):
     ref = oracle.OracleScene(sc).render(cams, 48, 40, mode="brute")
     assert ref["nsamples"].sum() > 2000
     _assert_parity(rgb, ns, ref, "unrelated plane resolutions")
+
+
+# ----------------------------------------------------------------------------- soft occupancy (Eq. 6-8)
+@pytest.mark.parametrize("eps", [0.3, 1.0, 4.0])
+def test_soft_mask_variant(omerf, oracle, eps):
+    import torch
+    sc, cams = synth.make_scene(0), synth.make_cameras(0)
+    W, H = synth.config_resolution(0)
+    with omerf.scene_create(sc, soft_eps=eps) as h:
+        rgb, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        rgb, ns = rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32)
+    ref = oracle.OracleScene(sc, soft_eps=eps).render(cams, W, H, mode="clipped")
+    _assert_parity(rgb, ns, ref, f"soft mask eps={eps}")
+    hard = oracle.OracleScene(sc).render(cams, W, H, mode="clipped")
+    assert np.array_equal(ns, hard["nsamples"])                 # M weights colours, it does not change the samples
+    assert np.abs(ref["rgb"] - hard["rgb"]).max() > 1e-2        # and the test would notice a missing M
+
+
+def test_soft_mask_thin_intervals_and_rejections(omerf, oracle):
+    rng = np.random.default_rng(12)
+    m = 25
+    lo = (1.0 + rng.random((m, m))).astype(np.float32)
+    hi = (lo + 0.05 + 1.5 * rng.random((m, m))).astype(np.float32)   # many intervals thinner than 2 eps (R23)
+    sc = synth.custom_scene(box=(12.0, 12.0, 4.0), hf_n=(m, m), h_lo=lo, h_up=hi, seed=6, step=0.1, bias_amp=0.2)
+    cams = np.stack([synth.look_at_camera((6.0, -5.0, 9.0), (6.0, 6.0, 1.5), 56, 40)])
+    import torch
+    with omerf.scene_create(sc, soft_eps=0.5) as h:
+        rgb, ns = omerf.render(h, cams, 56, 40)
+        torch.cuda.synchronize()
+    ref = oracle.OracleScene(sc, soft_eps=0.5).render(cams, 56, 40, mode="brute")
+    _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, "thin intervals")
+    with pytest.raises(omerf.OmerfError):
+        omerf.scene_create(sc, soft_eps=-1.0)
+    sc_g = synth.custom_scene(box=(12.0, 12.0, 4.0), hf_n=(m, m), h_lo=lo, h_up=hi, seed=6, occ_n=(24, 24, 8))
+    with pytest.raises(omerf.OmerfError):
+        omerf.scene_create(sc_g, sampler=1, soft_eps=0.5)
