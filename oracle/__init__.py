@@ -214,3 +214,42 @@ class OracleScene:
         if aux:
             out["T_end"], out["sum_w"], out["Q"] = ax[:, 0], ax[:, 1], ax[:, 2]
         return out
+
+
+# ---- sparse-block grid ----------------------------------------------------
+class SparseBlocks:
+    """Oracle-side bake of the sparse-block grid from the occupancy plane (omerf_oracle.c, R24)."""
+
+    def __init__(self, O: OracleScene, B: int = 8, atlas: bool = True):
+        L = lib()
+        L.orc_sparse_mark_blocks.restype = C.c_int64
+        L.orc_sparse_grid_lookup.restype = C.c_int
+        self.O, self.B = O, B
+        G = tuple(int(x) for x in O.c.grid_n)
+        self.nb = tuple((g + B - 1) // B for g in G)
+        self.mark = np.zeros(self.nb, dtype=np.uint8)
+        self.n_alloc = int(L.orc_sparse_mark_blocks(C.byref(O.c), C.c_int(B), _ptr(self.mark, _u8p)))
+        self.table = np.zeros(self.nb, dtype=np.int32)
+        self.atlas = np.zeros((self.n_alloc, B, B, B, 8), dtype=np.uint8) if atlas else None
+        L.orc_sparse_build(C.byref(O.c), C.c_int(B), _ptr(self.mark, _u8p), _ptr(self.table, C.POINTER(C.c_int32)),
+                           _ptr(self.atlas, _u8p) if atlas else None)
+
+    def need_mask(self) -> np.ndarray:
+        G = tuple(int(x) for x in self.O.c.grid_n)
+        need = np.zeros(G, dtype=np.uint8)
+        lib().orc_sparse_need_mask(C.byref(self.O.c), _ptr(need, _u8p))
+        return need
+
+    def lookup(self, p):
+        p = np.ascontiguousarray(p, dtype=np.float32)
+        out = np.zeros(8, dtype=np.uint32)
+        rc = lib().orc_sparse_grid_lookup(_ptr(self.table, C.POINTER(C.c_int32)), _ptr(self.atlas, _u8p), C.c_int(self.B),
+                                          self.O.c.grid_n, self.O.c.box, _ptr(p, _f32p), _ptr(out, _u32p))
+        return rc, out
+
+
+def grid_corners(O: OracleScene, p) -> np.ndarray:
+    p = np.ascontiguousarray(p, dtype=np.float32)
+    c = np.zeros(6, dtype=np.int32)
+    lib().orc_grid_corners(O.c.grid_n, O.c.box, _ptr(p, _f32p), _ptr(c, C.POINTER(C.c_int32)))
+    return c

@@ -564,3 +564,159 @@ int64_t orc_pixel_samples(const orc_scene *s, const orc_camera *cam, int u, int 
     }
     return n;
 }
+
+/* ------------------------------------------------------------------ sparse-block grid */
+/* the low-resolution voxel grid is stored as sparse blocks; PAPER.md:258 (sec. 5.3): the baked
+ * assets are produced from the occupancy plane, which says where features can ever be fetched.  The oracle states
+ * the bake as a plain rule (R24):
+ *   a voxel (i,j,k) of V is NEEDED iff it can be one of the 8 trilinear corners (R10 addressing) of a point whose
+ *   nearest grid point of P_o is (ix,iy) and whose z lies in [z_min, z_max](ix,iy) - with the cell footprint widened
+ *   by 1/64 of a cell on every side and the z interval by 1/64 of a voxel (both far above the fp32 rounding of the
+ *   renderer's coordinates, so every corner the renderer touches is needed);
+ *   a B^3 block is ALLOCATED iff it holds a needed voxel; blocks are numbered in C order of (bx,by,bz);
+ *   the atlas stores the allocated blocks' voxels ([id][B][B][B][8], zeros beyond the grid edge).
+ * Rendering through (table, atlas) fetches exactly the dense grid's texels, so the image is the dense oracle's. */
+static int64_t floordiv64(int64_t a, int64_t b) /* b > 0 */
+{
+    int64_t q = a / b;
+    return (a % b != 0 && a < 0) ? q - 1 : q;
+}
+
+/* corner index range [lo,hi] along one horizontal axis for occupancy cell i (exact integers):
+ * q = x G/X - 1/2 at x = (i -+ 33/64) X/(M-1)  ->  q = (2 (64 i -+ 33) G - 64 (M-1)) / (128 (M-1)) */
+static void cell_corner_range(int i, int M, int G, int *lo, int *hi)
+{
+    int64_t den = 128 * (int64_t)(M - 1);
+    int64_t a = floordiv64(2 * (64 * (int64_t)i - 33) * G - 64 * (int64_t)(M - 1), den);
+    int64_t b = floordiv64(2 * (64 * (int64_t)i + 33) * G - 64 * (int64_t)(M - 1), den) + 1;
+    *lo = (int)(a < 0 ? 0 : a);
+    *hi = (int)(b > G - 1 ? G - 1 : b);
+}
+
+/* needed z-corner range of one column, in double with one rounding per operation; returns 0 if none */
+static int column_corner_range(float lo, float hi, float Z, int G, int *k_lo, int *k_hi)
+{
+    if (!(lo <= hi)) return 0;                                /* empty column (R17) */
+    double zl = lo < 0.0f ? 0.0 : (double)lo, zh = hi > Z ? (double)Z : (double)hi;
+    if (zl > zh) return 0;                                    /* interval outside the box */
+    double qa = zl * (double)G / (double)Z - 0.515625;        /* - 1/2 - 1/64 */
+    double qb = zh * (double)G / (double)Z - 0.484375;        /* - 1/2 + 1/64 */
+    int64_t a = (int64_t)floor(qa), b = (int64_t)floor(qb) + 1;
+    *k_lo = (int)(a < 0 ? 0 : a);
+    *k_hi = (int)(b > G - 1 ? G - 1 : b);
+    return 1;
+}
+
+/* needed-voxel mask, uint8 [Gx][Gy][Gz] (tiny scenes / pins only) */
+void orc_sparse_need_mask(const orc_scene *s, uint8_t *need)
+{
+    const int Mx = s->hf_n[0], My = s->hf_n[1], Gx = s->grid_n[0], Gy = s->grid_n[1], Gz = s->grid_n[2];
+    memset(need, 0, (size_t)Gx * Gy * Gz);
+    for (int ix = 0; ix < Mx; ix++)
+        for (int iy = 0; iy < My; iy++) {
+            int i0, i1, j0, j1, k0, k1;
+            if (!column_corner_range(s->h_lo[(size_t)ix * My + iy], s->h_up[(size_t)ix * My + iy], s->box[2], Gz, &k0, &k1))
+                continue;
+            cell_corner_range(ix, Mx, Gx, &i0, &i1);
+            cell_corner_range(iy, My, Gy, &j0, &j1);
+            for (int i = i0; i <= i1; i++)
+                for (int j = j0; j <= j1; j++)
+                    for (int k = k0; k <= k1; k++) need[((size_t)i * Gy + j) * Gz + k] = 1;
+        }
+}
+
+/* block marks uint8 [nbx][nby][nbz], nb = ceil(G/B); returns the number of allocated blocks */
+int64_t orc_sparse_mark_blocks(const orc_scene *s, int B, uint8_t *mark)
+{
+    const int Mx = s->hf_n[0], My = s->hf_n[1], Gx = s->grid_n[0], Gy = s->grid_n[1], Gz = s->grid_n[2];
+    const int nbx = (Gx + B - 1) / B, nby = (Gy + B - 1) / B, nbz = (Gz + B - 1) / B;
+    memset(mark, 0, (size_t)nbx * nby * nbz);
+    for (int ix = 0; ix < Mx; ix++)
+        for (int iy = 0; iy < My; iy++) {
+            int i0, i1, j0, j1, k0, k1;
+            if (!column_corner_range(s->h_lo[(size_t)ix * My + iy], s->h_up[(size_t)ix * My + iy], s->box[2], Gz, &k0, &k1))
+                continue;
+            cell_corner_range(ix, Mx, Gx, &i0, &i1);
+            cell_corner_range(iy, My, Gy, &j0, &j1);
+            for (int bx = i0 / B; bx <= i1 / B; bx++)
+                for (int by = j0 / B; by <= j1 / B; by++)
+                    for (int bz = k0 / B; bz <= k1 / B; bz++) mark[((size_t)bx * nby + by) * nbz + bz] = 1;
+        }
+    int64_t n = 0;
+    for (size_t i = 0; i < (size_t)nbx * nby * nbz; i++) n += mark[i];
+    return n;
+}
+
+/* table int32 [nbx*nby*nbz]: block id (rank among the allocated blocks in C order) or -1;
+ * atlas uint8 [n_alloc][B][B][B][8] (may be NULL to build the table only) */
+void orc_sparse_build(const orc_scene *s, int B, const uint8_t *mark, int32_t *table, uint8_t *atlas)
+{
+    const int Gx = s->grid_n[0], Gy = s->grid_n[1], Gz = s->grid_n[2];
+    const int nbx = (Gx + B - 1) / B, nby = (Gy + B - 1) / B, nbz = (Gz + B - 1) / B;
+    int32_t id = 0;
+    for (int bx = 0; bx < nbx; bx++)
+        for (int by = 0; by < nby; by++)
+            for (int bz = 0; bz < nbz; bz++) {
+                size_t b = ((size_t)bx * nby + by) * nbz + bz;
+                if (!mark[b]) {
+                    table[b] = -1;
+                    continue;
+                }
+                table[b] = id;
+                if (atlas) {
+                    uint8_t *dst = atlas + (size_t)id * B * B * B * 8;
+                    for (int x = 0; x < B; x++)
+                        for (int y = 0; y < B; y++)
+                            for (int z = 0; z < B; z++) {
+                                int gx = bx * B + x, gy = by * B + y, gz = bz * B + z;
+                                uint8_t *t = dst + (((size_t)x * B + y) * B + z) * 8;
+                                if (gx < Gx && gy < Gy && gz < Gz)
+                                    memcpy(t, s->grid + (((size_t)gx * Gy + gy) * Gz + gz) * 8, 8);
+                                else
+                                    memset(t, 0, 8);
+                            }
+                }
+                id++;
+            }
+}
+
+/* the 8 trilinear corners of p: c = {x0, x1, y0, y1, z0, z1} (R10) */
+void orc_grid_corners(const int32_t G[3], const float box[3], const float p[3], int32_t c[6])
+{
+    uint32_t w;
+    int a, b;
+    for (int ax = 0; ax < 3; ax++) {
+        axis_tap(p[ax], G[ax], box[ax], &a, &b, &w);
+        c[2 * ax] = a;
+        c[2 * ax + 1] = b;
+    }
+}
+
+/* orc_grid_lookup through (table, atlas); returns -1 if a corner lies in an unallocated block */
+int orc_sparse_grid_lookup(const int32_t *table, const uint8_t *atlas, int B, const int32_t G[3], const float box[3],
+                           const float p[3], uint32_t I[8])
+{
+    int x0, x1, y0, y1, z0, z1;
+    uint32_t wx, wy, wz;
+    axis_tap(p[0], G[0], box[0], &x0, &x1, &wx);
+    axis_tap(p[1], G[1], box[1], &y0, &y1, &wy);
+    axis_tap(p[2], G[2], box[2], &z0, &z1, &wz);
+    const int nby = (G[1] + B - 1) / B, nbz = (G[2] + B - 1) / B;
+    const int xs[2] = {x0, x1}, ys[2] = {y0, y1}, zs[2] = {z0, z1};
+    const uint8_t *t[2][2][2];
+    for (int a = 0; a < 2; a++)
+        for (int b = 0; b < 2; b++)
+            for (int c = 0; c < 2; c++) {
+                int32_t id = table[((size_t)(xs[a] / B) * nby + ys[b] / B) * nbz + zs[c] / B];
+                if (id < 0) return -1;
+                t[a][b][c] = atlas + ((((size_t)id * B + xs[a] % B) * B + ys[b] % B) * B + zs[c] % B) * 8;
+            }
+    for (int c = 0; c < 8; c++) {
+        uint32_t Bz[2];
+        for (int sl = 0; sl < 2; sl++)
+            Bz[sl] = (256u - wx) * (256u - wy) * t[0][0][sl][c] + wx * (256u - wy) * t[1][0][sl][c] +
+                     (256u - wx) * wy * t[0][1][sl][c] + wx * wy * t[1][1][sl][c];
+        I[c] = ((256u - wz) * Bz[0] + wz * Bz[1] + 128u) >> 8;
+    }
+    return 0;
+}
