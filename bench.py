@@ -189,7 +189,7 @@ def run_ours(args):
     W, H = synth.config_resolution(cfg)
     n_views = cams.shape[0]
     sampler = omerf.SAMPLER_GRID if args.sampler == "grid" else omerf.SAMPLER_PLANE
-    h = omerf.scene_create(scene, sampler=sampler, soft_eps=args.soft_eps)
+    h = omerf.scene_create(scene, sampler=sampler, soft_eps=args.soft_eps, grid_block=args.grid_block)
     info = omerf.scene_info(h)
     out_rgb = torch.empty((n_views, H, W, 3), dtype=torch.float32, device="cuda")
     out_n = torch.empty((n_views, H, W), dtype=torch.int32, device="cuda")
@@ -279,7 +279,8 @@ def run_ours(args):
             "steps": k, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32 (u8 features, integer interpolation)",
             "data": "synthetic",
-            "config": {"workload": workload_name(cfg), "views": n_views, "W": W, "H": H, "sampler": args.sampler, "soft_eps": args.soft_eps,
+            "config": {"workload": workload_name(cfg), "views": n_views, "W": W, "H": H, "sampler": args.sampler, "soft_eps": args.soft_eps, "grid_block": args.grid_block,
+                       "grid_bytes": info["grid_bytes"], "grid_blocks": [info["grid_blocks_allocated"], info["grid_blocks_total"]],
                        "scene_device_bytes": info["device_bytes"], "l2": "flushed between timed steps (256 MiB fill, "
                        "outside the event pairs); scene 296 MiB > L2", "parallelism": f"replicated scene x{world}"},
             "frames_per_s": world * n_views * k / secs,
@@ -327,6 +328,7 @@ def main():
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4, 5])
     ap.add_argument("--sampler", default="plane", choices=["plane", "grid"])
     ap.add_argument("--soft-eps", type=float, default=0.0, help="SURVEY 8(f).2: soft occupancy (Eq. 6-8) buffer height; 0 = binary mask")
+    ap.add_argument("--grid-block", type=int, default=0, help="SURVEY 8(f).1: store V as sparse blocks of this edge (0 = dense)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -61,6 +61,10 @@ typedef struct {
                          sample's colour contribution, C = sum_i M_i w_i c_i (Eq. 8) - the training-time
                          forward pass.  Samples, transmittance and termination are those of the binary mask; where the
                          two buffers of a thin interval overlap the smaller ramp is taken (R23). */
+    int32_t grid_block; /* 0: V is stored dense.  2, 4, 8 or 16: V is stored as sparse blocks of grid_block^3 voxels
+                            baked on the device from the occupancy plane: only blocks
+                           holding a voxel that a sample inside the slab can touch are kept (R24); the
+                           rendered images are identical to the dense layout's. */
 } omerf_scene_desc;
 
 /* Pinhole camera, world frame. */
@@ -74,6 +78,9 @@ typedef struct {
     int32_t pyramid_levels; /* levels of the min/max pyramid of (h_lo, h_up), level 0 = P_o itself */
     int32_t sampler;
     uint64_t occ_bits_set;  /* sampler GRID: number of set voxels of the derived bitfield, else 0 */
+    uint64_t grid_bytes;        /* device bytes of V: dense array, or atlas + block table */
+    uint64_t grid_blocks_total; /* sparse layout: blocks of the block grid, else 0 */
+    uint64_t grid_blocks_allocated; /* sparse layout: blocks kept (occupancy ratio = allocated / total, cf. Table 5) */
 } omerf_scene_info;
 
 /* S0 + S1 (+ S10 derivation): validate, upload, re-lay out for gathers, build the min/max pyramid
@@ -121,6 +128,8 @@ int omerf_scene_get_info(const omerf_scene *scene, omerf_scene_info *out_info /*
  * *nx, *ny receive the level's size; pass out_min = out_max = NULL to query the size only. */
 int omerf_scene_get_pyramid_level(const omerf_scene *scene, int level, int32_t *nx, int32_t *ny,
                                   float *out_min /*HOST*/, float *out_max /*HOST*/);
+/* sparse layout: out_table HOST int32[n] with n = grid_blocks_total, C order of (bx,by,bz); block id or -1. */
+int omerf_scene_get_block_table(const omerf_scene *scene, int32_t *out_table /*HOST*/, uint64_t n);
 /* sampler GRID: out_words HOST uint32[(Nx*Ny*Nz+31)/32], bit index ((jx*Ny + jy)*Nz + jz), LSB first. */
 int omerf_scene_get_bitfield(const omerf_scene *scene, uint32_t *out_words /*HOST*/, uint64_t n_words);
 

@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     OmerfError,
     SceneHandle,
     bitfield,
+    block_table,
     gather_probe,
     last_launch_count,
     load_library,

@@ -23,7 +23,7 @@ SAMPLER_GRID = 1
 
 EXPORTS = (
     "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_gather_probe", "omerf_last_launch_count",
-    "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield",
+    "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield", "omerf_scene_get_block_table",
     "omerf_scene_destroy", "omerf_last_error", "omerf_version",
 )
 
@@ -40,13 +40,14 @@ class SceneDesc(C.Structure):
         ("W0", _f32p), ("b0", _f32p), ("W1", _f32p), ("b1", _f32p), ("W2", _f32p), ("b2", _f32p),
         ("step", C.c_float), ("t_stop", C.c_float), ("bg", C.c_float * 3),
         ("sampler", C.c_int32), ("occ_n", C.c_int32 * 3),
-        ("soft_eps", C.c_float),
+        ("soft_eps", C.c_float), ("grid_block", C.c_int32),
     ]
 
 
 class SceneInfo(C.Structure):
     _fields_ = [("device_bytes", C.c_uint64), ("pyramid_levels", C.c_int32), ("sampler", C.c_int32),
-                ("occ_bits_set", C.c_uint64)]
+                ("occ_bits_set", C.c_uint64), ("grid_bytes", C.c_uint64), ("grid_blocks_total", C.c_uint64),
+                ("grid_blocks_allocated", C.c_uint64)]
 
 
 class GatherProbeResult(C.Structure):
@@ -81,6 +82,7 @@ def load_library() -> C.CDLL:
     L.omerf_scene_get_pyramid_level.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                                                 C.c_void_p, C.c_void_p]
     L.omerf_scene_get_bitfield.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
+    L.omerf_scene_get_block_table.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
     L.omerf_scene_destroy.argtypes = [C.c_void_p]
     L.omerf_scene_destroy.restype = None
     _lib = L
@@ -96,7 +98,7 @@ def _np(a, dt):
     return np.ascontiguousarray(a, dtype=dt)
 
 
-def make_desc(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0):
+def make_desc(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, grid_block: int = 0):
     """Fill an omerf_scene_desc from an object with synth.Scene's attributes. Returns (desc, keepalive)."""
     d = SceneDesc()
     keep = []
@@ -126,6 +128,7 @@ def make_desc(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0):
     d.bg[:] = scene.bg
     d.sampler = sampler
     d.soft_eps = soft_eps
+    d.grid_block = grid_block
     d.occ_n[:] = scene.occ_n
     return d, keep
 
@@ -149,7 +152,7 @@ class SceneHandle:
             pass
 
 
-def scene_create(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0) -> SceneHandle:
+def scene_create(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, grid_block: int = 0) -> SceneHandle:
     """omerf_scene_create: upload + re-layout + pyramid (+ bitfield) on the current CUDA device."""
     import torch
     if not torch.cuda.is_available():
@@ -157,7 +160,7 @@ def scene_create(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0) -> 
     torch.cuda.init()
     torch.cuda.current_stream()          # make sure torch's primary context is current
     L = load_library()
-    d, keep = make_desc(scene, sampler, soft_eps)
+    d, keep = make_desc(scene, sampler, soft_eps, grid_block)
     out = C.c_void_p()
     _check(L.omerf_scene_create(C.byref(d), C.byref(out)), "omerf_scene_create")
     del keep
@@ -236,7 +239,8 @@ def scene_info(h: SceneHandle) -> dict:
     info = SceneInfo()
     _check(load_library().omerf_scene_get_info(h.ptr, C.byref(info)), "omerf_scene_get_info")
     return {"device_bytes": int(info.device_bytes), "pyramid_levels": int(info.pyramid_levels),
-            "sampler": int(info.sampler), "occ_bits_set": int(info.occ_bits_set)}
+            "sampler": int(info.sampler), "occ_bits_set": int(info.occ_bits_set), "grid_bytes": int(info.grid_bytes),
+            "grid_blocks_total": int(info.grid_blocks_total), "grid_blocks_allocated": int(info.grid_blocks_allocated)}
 
 
 def pyramid_level(h: SceneHandle, level: int):
@@ -248,6 +252,14 @@ def pyramid_level(h: SceneHandle, level: int):
     _check(L.omerf_scene_get_pyramid_level(h.ptr, level, C.byref(nx), C.byref(ny), mn.ctypes.data, mx.ctypes.data),
            "get_pyramid_level")
     return mn, mx
+
+
+def block_table(h: SceneHandle) -> np.ndarray:
+    """omerf_scene_get_block_table: flat int32 block table of the sparse-block grid (C order of bx,by,bz)."""
+    n = scene_info(h)["grid_blocks_total"]
+    out = np.empty(n, dtype=np.int32)
+    _check(load_library().omerf_scene_get_block_table(h.ptr, out.ctypes.data, n), "get_block_table")
+    return out
 
 
 def bitfield(h: SceneHandle, occ_n) -> np.ndarray:

@@ -54,6 +54,7 @@ static void free_scene(omerf_scene *s)
     cudaFree(s->d_pyz);
     cudaFree(s->d_occ);
     cudaFree(s->d_mlp_tab);
+    cudaFree(s->d_blk_table);
     cudaFree(s->d_cams);
     cudaFree(s->d_tile_counter);
     cudaFree(s->d_scratch_rgb);
@@ -90,6 +91,8 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
     if (!(d->step > 0) || !isfinite(d->step)) return invalid("step must be > 0");
     if (!(d->t_stop > 0 && d->t_stop < 1)) return invalid("t_stop must be in (0,1)");
     if (d->sampler != OMERF_SAMPLER_PLANE && d->sampler != OMERF_SAMPLER_GRID) return invalid("unknown sampler");
+    if (d->grid_block != 0 && d->grid_block != 2 && d->grid_block != 4 && d->grid_block != 8 && d->grid_block != 16)
+        return invalid("grid_block must be 0, 2, 4, 8 or 16");
     if (!(d->soft_eps >= 0) || !isfinite(d->soft_eps)) return invalid("soft_eps must be >= 0");
     if (d->soft_eps > 0 && d->sampler != OMERF_SAMPLER_PLANE) return invalid("soft_eps needs the occupancy-plane sampler");
     if (d->sampler == OMERF_SAMPLER_GRID)
@@ -159,6 +162,12 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         if ((rc = upload((void **)&d_lo, d->h_lo, hf_bytes, &tmp))) break;
         if ((rc = upload((void **)&d_up, d->h_up, hf_bytes, &tmp))) break;
         if ((rc = omerf_launch_pyramid(s, d_lo, d_up, 0))) break;
+        // 8(f).1: sparse-block layout of V baked from the occupancy plane (replaces the dense array)
+        s->grid_bytes = (uint64_t)v.G[0] * v.G[1] * v.G[2] * 8;
+        if (d->grid_block) {
+            if ((rc = omerf_bake_sparse_grid(s, &s->d_grid, d->grid_block, 0))) break;
+            s->device_bytes = s->device_bytes - (uint64_t)v.G[0] * v.G[1] * v.G[2] * 8 + s->grid_bytes;
+        }
         // S10: occupancy bitfield + its mip chain, derived on the device from the slab
         if (d->sampler == OMERF_SAMPLER_GRID) {
             for (int i = 0; i < 3; i++) {
@@ -368,6 +377,9 @@ extern "C" int omerf_scene_get_info(const omerf_scene *s, omerf_scene_info *out)
     out->pyramid_levels = s->dev.n_levels;
     out->sampler = s->dev.sampler;
     out->occ_bits_set = s->occ_bits_set;
+    out->grid_bytes = s->grid_bytes;
+    out->grid_blocks_total = s->blocks_total;
+    out->grid_blocks_allocated = s->blocks_allocated;
     return OMERF_OK;
 }
 
@@ -396,6 +408,15 @@ extern "C" int omerf_scene_get_pyramid_level(const omerf_scene *s, int level, in
         out_max[i] = tmp[i].y;
     }
     delete[] tmp;
+    return OMERF_OK;
+}
+
+extern "C" int omerf_scene_get_block_table(const omerf_scene *s, int32_t *out_table, uint64_t n)
+{
+    if (!s || !out_table) return invalid("null scene/out_table");
+    if (!s->dev.blk_shift) return invalid("scene has no block table (grid_block is 0)");
+    if (n != s->blocks_total) return invalid("n does not match grid_blocks_total");
+    OMERF_CUDA(cudaMemcpy(out_table, s->d_blk_table, n * sizeof(int32_t), cudaMemcpyDeviceToHost));
     return OMERF_OK;
 }
 

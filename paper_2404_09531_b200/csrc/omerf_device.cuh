@@ -27,7 +27,10 @@ struct DevScene {
     // features: 8 uint8 channels per texel = one uint2
     int G[3];
     float gs[3];           // G/box per axis
-    const uint2 *grid;     // [Gx][Gy][Gz]
+    const uint2 *grid;     // dense: [Gx][Gy][Gz]; sparse blocks: atlas [id][B][B][B] (omerf_sparse.cu)
+    int blk_shift;         // 0 = dense grid, else log2 of the block edge B
+    int nby, nbz;          // block-grid dims along y and z
+    const int32_t *blk_table; // [nbx][nby][nbz] block id or -1
     int xy_n[2], xz_n[2], yz_n[2];
     float xy_s[2], xz_s[2], yz_s[2];
     const uint2 *pxy, *pxz, *pyz;
@@ -55,7 +58,8 @@ struct DevScene {
 struct omerf_scene {
     DevScene dev;
     int device;
-    void *d_pyr, *d_grid, *d_pxy, *d_pxz, *d_pyz, *d_occ, *d_mlp_tab;
+    void *d_pyr, *d_grid, *d_pxy, *d_pxz, *d_pyz, *d_occ, *d_mlp_tab, *d_blk_table;
+    uint64_t blocks_total, blocks_allocated, grid_bytes;
     uint64_t device_bytes;
     uint64_t occ_bits_set;
     // per-render state (mutable through the const handle: calls must be stream-ordered)
@@ -86,6 +90,7 @@ int omerf_cuda_fail(cudaError_t e, const char *what);
 // kernels' host launchers
 int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, cudaStream_t st);
 int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st);
+int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream_t st);
 int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_t st);
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H,
                         float *out_rgb, uint32_t *out_n, cudaStream_t st, int *launches, uint2 *sample_log = nullptr,

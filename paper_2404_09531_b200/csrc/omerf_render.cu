@@ -329,6 +329,41 @@ __device__ __forceinline__ void plane_taps(const uint2 *__restrict__ tex, int Nb
     t[3] = __ldg(tex + (r1 + (uint32_t)b1));
 }
 
+// texel indices of the 8 trilinear corners of V, order (x0y0, x0y1, x1y0, x1y1) x (z0, z1).  Dense layout: row-major
+// [Gx][Gy][Gz]; sparse blocks (8(f).1): one block-table lookup per corner, then the texel inside the atlas block.
+template <bool GENERAL>
+__device__ __forceinline__ void grid_corner_offsets(const DevScene &sc, int x0, int x1, int y0, int y1, int z0, int z1,
+                                                    uint32_t off[8])
+{
+    if (!GENERAL || sc.blk_shift == 0) {
+        const uint32_t Gy = (uint32_t)sc.G[1], Gz = (uint32_t)sc.G[2];
+        const uint32_t c0 = (uint32_t)x0 * Gy, c1 = (uint32_t)x1 * Gy;
+        const uint32_t r00 = (c0 + (uint32_t)y0) * Gz, r01 = (c0 + (uint32_t)y1) * Gz;
+        const uint32_t r10 = (c1 + (uint32_t)y0) * Gz, r11 = (c1 + (uint32_t)y1) * Gz;
+        off[0] = r00 + (uint32_t)z0; off[1] = r00 + (uint32_t)z1;
+        off[2] = r01 + (uint32_t)z0; off[3] = r01 + (uint32_t)z1;
+        off[4] = r10 + (uint32_t)z0; off[5] = r10 + (uint32_t)z1;
+        off[6] = r11 + (uint32_t)z0; off[7] = r11 + (uint32_t)z1;
+    } else {
+        const int s = sc.blk_shift, m = (1 << s) - 1;
+        const int xs[2] = {x0, x1}, ys[2] = {y0, y1}, zs[2] = {z0, z1};
+#pragma unroll
+        for (int a = 0; a < 2; a++)
+#pragma unroll
+            for (int b = 0; b < 2; b++) {
+                const int col = ((xs[a] >> s) * sc.nby + (ys[b] >> s)) * sc.nbz;
+                const uint32_t in_xy = (uint32_t)((((xs[a] & m) << s) + (ys[b] & m)) << s);
+#pragma unroll
+                for (int c = 0; c < 2; c++) {
+                    // every corner of a sample inside the slab lies in an allocated block (R24); max() only guards memory
+                    const int id = max(__ldg(sc.blk_table + col + (zs[c] >> s)), 0);
+                    off[(a * 2 + b) * 2 + c] = ((uint32_t)id << (3 * s)) + in_xy + (uint32_t)(zs[c] & m);
+                }
+            }
+    }
+}
+
+template <bool GENERAL>
 __device__ __forceinline__ void gather_features(const DevScene &sc, float px, float py, float pz, uint32_t I[8])
 {
     // taps and weights of all four sources first, then all 20 loads, then the arithmetic
@@ -343,15 +378,13 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
     uint2 ga[4], gb[4];
     {
         // low-res voxel grid V: bilinear in (x,y) on the z-slices z0 and z1
-        const uint32_t Gy = (uint32_t)sc.G[1], Gz = (uint32_t)sc.G[2];
+        uint32_t off[8];
+        grid_corner_offsets<GENERAL>(sc, x0, x1, y0, y1, z0, z1, off);
         const uint2 *g = sc.grid;
-        const uint32_t c0 = (uint32_t)x0 * Gy, c1 = (uint32_t)x1 * Gy;
-        const uint32_t r00 = (c0 + (uint32_t)y0) * Gz, r01 = (c0 + (uint32_t)y1) * Gz;
-        const uint32_t r10 = (c1 + (uint32_t)y0) * Gz, r11 = (c1 + (uint32_t)y1) * Gz;
-        ga[0] = __ldg(g + (r00 + (uint32_t)z0)); gb[0] = __ldg(g + (r00 + (uint32_t)z1));
-        ga[1] = __ldg(g + (r01 + (uint32_t)z0)); gb[1] = __ldg(g + (r01 + (uint32_t)z1));
-        ga[2] = __ldg(g + (r10 + (uint32_t)z0)); gb[2] = __ldg(g + (r10 + (uint32_t)z1));
-        ga[3] = __ldg(g + (r11 + (uint32_t)z0)); gb[3] = __ldg(g + (r11 + (uint32_t)z1));
+        ga[0] = __ldg(g + off[0]); gb[0] = __ldg(g + off[1]);
+        ga[1] = __ldg(g + off[2]); gb[1] = __ldg(g + off[3]);
+        ga[2] = __ldg(g + off[4]); gb[2] = __ldg(g + off[5]);
+        ga[3] = __ldg(g + off[6]); gb[3] = __ldg(g + off[7]);
     }
     // triplanes: xy sampled with (x,y), xz with (x,z), yz with (y,z).  When the planes share their resolution per
     // world axis (every config: xy A x A, xz and yz A x B) a tap computed for one plane is the other plane's tap too
@@ -676,7 +709,9 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
 #define OMERF_MIN_BLOCKS 5
 #endif
 // LOG (gather calibration only): every sample taken is appended to sample_log as (pixel, lattice index).
-template <int SAMPLER, bool LOG>
+// GENERAL: the 8(f) variants (soft occupancy, sparse-block grid) behind warp-uniform branches; the plain path
+// (dense grid, binary mask) is compiled without them.
+template <int SAMPLER, bool LOG, bool GENERAL>
 __global__ void __launch_bounds__(32 * OMERF_WARPS, OMERF_MIN_BLOCKS)
 omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__restrict__ cams, int n_views, int W, int H,
                    float *__restrict__ out_rgb, uint32_t *__restrict__ out_n, unsigned int *__restrict__ tile_counter,
@@ -851,7 +886,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                         next_ready = k < k1 && h.x <= qz && qz <= h.y && in_box(sc, qx, qy, qz);
                     }
                     float soft_m = 1.0f;
-                    if (SAMPLER == OMERF_SAMPLER_PLANE && sc.soft_eps > 0.0f) {
+                    if (GENERAL && SAMPLER == OMERF_SAMPLER_PLANE && sc.soft_eps > 0.0f) {
                         // Eq. 6 (q = 2) at the nearest grid point of P_o (Eq. 7): the sample is inside [z_min, z_max],
                         // so M = min(1, ((z - z_min)/eps)^2, ((z_max - z)/eps)^2); it weights the colours only (Eq. 8)
                         const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
@@ -860,7 +895,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                         soft_m = m * m;
                     }
                     uint32_t I[8];
-                    gather_features(sc, px, py, pz, I);
+                    gather_features<GENERAL>(sc, px, py, pz, I);
                     float t[8];
 #pragma unroll
                     for (int c = 0; c < 8; c++) t[c] = __fmaf_rn(__uint2float_rn(I[c]), sc.deq_mul, sc.deq_add);
@@ -969,15 +1004,11 @@ omerf_gather_probe_kernel(const __grid_constant__ DevScene sc, const omerf_camer
     axis_tap(px, sc.gs[0], sc.G[0], x0, x1, w);
     axis_tap(py, sc.gs[1], sc.G[1], y0, y1, w);
     axis_tap(pz, sc.gs[2], sc.G[2], z0, z1, w);
-    const uint32_t Gy = (uint32_t)sc.G[1], Gz = (uint32_t)sc.G[2];
-    const uint32_t c0 = (uint32_t)x0 * Gy, c1 = (uint32_t)x1 * Gy;
-    const uint32_t r00 = (c0 + (uint32_t)y0) * Gz, r01 = (c0 + (uint32_t)y1) * Gz;
-    const uint32_t r10 = (c1 + (uint32_t)y0) * Gz, r11 = (c1 + (uint32_t)y1) * Gz;
+    uint32_t off[8];
+    grid_corner_offsets<true>(sc, x0, x1, y0, y1, z0, z1, off);
     uint2 t[20];
-    t[0] = __ldg(sc.grid + (r00 + (uint32_t)z0)); t[1] = __ldg(sc.grid + (r00 + (uint32_t)z1));
-    t[2] = __ldg(sc.grid + (r01 + (uint32_t)z0)); t[3] = __ldg(sc.grid + (r01 + (uint32_t)z1));
-    t[4] = __ldg(sc.grid + (r10 + (uint32_t)z0)); t[5] = __ldg(sc.grid + (r10 + (uint32_t)z1));
-    t[6] = __ldg(sc.grid + (r11 + (uint32_t)z0)); t[7] = __ldg(sc.grid + (r11 + (uint32_t)z1));
+#pragma unroll
+    for (int q = 0; q < 8; q++) t[q] = __ldg(sc.grid + off[q]);
     axis_tap(px, sc.xy_s[0], sc.xy_n[0], a0, a1, w);
     axis_tap(py, sc.xy_s[1], sc.xy_n[1], b0, b1, w);
     plane_taps(sc.pxy, sc.xy_n[1], a0, a1, b0, b1, t + 8);
@@ -1050,16 +1081,21 @@ int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_
     OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, (sample_log ? 64 : 1) * sizeof(unsigned int), st));
 #endif
     const int grid = s->persistent_blocks;
-#define OMERF_LAUNCH(SAMPLER, LOG)                                                                                          \
-    omerf_march_kernel<SAMPLER, LOG><<<grid, 32 * OMERF_WARPS, 0, st>>>(s->dev, d_cams, n_views, W, H, out_rgb, out_n,      \
-                                                                         s->d_tile_counter, sample_log, log_capacity)
+    const bool general = s->dev.soft_eps > 0.0f || s->dev.blk_shift != 0;
+#define OMERF_LAUNCH(SAMPLER, LOG, GENERAL)                                                                                 \
+    omerf_march_kernel<SAMPLER, LOG, GENERAL><<<grid, 32 * OMERF_WARPS, 0, st>>>(                                          \
+        s->dev, d_cams, n_views, W, H, out_rgb, out_n, s->d_tile_counter, sample_log, log_capacity)
+#define OMERF_LAUNCH2(SAMPLER, LOG)                \
+    if (general) OMERF_LAUNCH(SAMPLER, LOG, true); \
+    else OMERF_LAUNCH(SAMPLER, LOG, false)
     if (s->dev.sampler == OMERF_SAMPLER_PLANE) {
-        if (sample_log) OMERF_LAUNCH(OMERF_SAMPLER_PLANE, true);
-        else OMERF_LAUNCH(OMERF_SAMPLER_PLANE, false);
+        if (sample_log) { OMERF_LAUNCH2(OMERF_SAMPLER_PLANE, true); }
+        else { OMERF_LAUNCH2(OMERF_SAMPLER_PLANE, false); }
     } else {
-        if (sample_log) OMERF_LAUNCH(OMERF_SAMPLER_GRID, true);
-        else OMERF_LAUNCH(OMERF_SAMPLER_GRID, false);
+        if (sample_log) { OMERF_LAUNCH2(OMERF_SAMPLER_GRID, true); }
+        else { OMERF_LAUNCH2(OMERF_SAMPLER_GRID, false); }
     }
+#undef OMERF_LAUNCH2
 #undef OMERF_LAUNCH
     *launches = 1;
     OMERF_CUDA(cudaGetLastError());
@@ -1073,9 +1109,9 @@ int omerf_query_persistent_blocks(int sampler, int *blocks)
     OMERF_CUDA(cudaGetDevice(&dev));
     OMERF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     if (sampler == OMERF_SAMPLER_PLANE)
-        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_PLANE, false>, 32 * OMERF_WARPS, 0));
+        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_PLANE, false, true>, 32 * OMERF_WARPS, 0));
     else
-        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_GRID, false>, 32 * OMERF_WARPS, 0));
+        OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_GRID, false, true>, 32 * OMERF_WARPS, 0));
     *blocks = sms * (per_sm > 0 ? per_sm : 1);
     return OMERF_OK;
 }

@@ -103,3 +103,25 @@ def test_config5_low_altitude_cameras(omerf, city):
     rgb, ns = _check_sampled(omerf, city, cams, W, H, 0, 30000, [200, 700], seed=105)
     per_view = ns.reshape(cams.shape[0], -1).sum(axis=1)
     assert np.all(per_view > 0)
+
+
+def test_config1_sparse_block_grid(omerf, city):
+    """SURVEY 8(f).1 at full size: oracle block table bit-exact, sampled pixels equal to the dense oracle."""
+    import torch
+
+    import oracle
+    cams = synth.make_cameras(1)
+    W, H = synth.config_resolution(1)
+    S = oracle.SparseBlocks(oracle.OracleScene(city), 8, atlas=False)
+    with omerf.scene_create(city, grid_block=8) as h:
+        info = omerf.scene_info(h)
+        assert np.array_equal(omerf.block_table(h), S.table.ravel())
+        assert info["grid_blocks_allocated"] == S.n_alloc and info["grid_bytes"] < 128 << 20
+        rgb, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        rgb, ns = rgb.cpu().numpy(), ns.cpu().numpy().view(np.uint32)
+    rng = np.random.default_rng(106)
+    vuv = _sample_pixels(rng, 1, W, H, 20000, [500])
+    ref = oracle.OracleScene(city).render_pixels(cams, W, H, vuv, mode="clipped")
+    assert np.array_equal(ns[vuv[:, 0], vuv[:, 2], vuv[:, 1]], ref["nsamples"])
+    assert np.abs(rgb[vuv[:, 0], vuv[:, 2], vuv[:, 1]].astype(np.float64) - ref["rgb"]).max() <= RGB_TOL

@@ -286,3 +286,51 @@ def test_soft_mask_thin_intervals_and_rejections(omerf, oracle):
     sc_g = synth.custom_scene(box=(12.0, 12.0, 4.0), hf_n=(m, m), h_lo=lo, h_up=hi, seed=6, occ_n=(24, 24, 8))
     with pytest.raises(omerf.OmerfError):
         omerf.scene_create(sc_g, sampler=1, soft_eps=0.5)
+
+
+# ----------------------------------------------------------------------------- sparse-block grid
+@pytest.mark.parametrize("B", [2, 4, 8, 16])
+def test_sparse_block_grid_matches_oracle_bake_and_dense_render(omerf, oracle, B):
+    """The device bake allocates exactly the oracle's blocks with the oracle's ids (bit-exact table), and rendering
+    through the table gives the dense oracle's image: the same texels are fetched."""
+    import torch
+    rng = np.random.default_rng(21)
+    m = 29
+    lo = (0.5 + 2.0 * rng.random((m, m))).astype(np.float32)
+    hi = (lo + 0.05 + 3.0 * rng.random((m, m))).astype(np.float32)
+    kill = rng.random((m, m)) < 0.2
+    hi[kill] = lo[kill] - 1.0
+    sc = synth.custom_scene(box=(14.0, 13.0, 8.0), hf_n=(m, m), h_lo=lo, h_up=hi, grid_n=(37, 30, 21), xy_n=(64, 64),
+                            xz_n=(64, 32), yz_n=(64, 32), seed=11, step=0.15, smooth=False, bias_amp=0.2)
+    cams = np.stack([synth.look_at_camera((7.0, -8.0, 15.0), (7.0, 6.5, 2.0), 72, 56),
+                     synth.look_at_camera((1.0, 1.5, 3.0), (13.0, 12.0, 2.0), 72, 56)])
+    O = oracle.OracleScene(sc)
+    S = oracle.SparseBlocks(O, B, atlas=False)
+    with omerf.scene_create(sc, grid_block=B) as h:
+        info = omerf.scene_info(h)
+        assert info["grid_blocks_total"] == S.table.size and info["grid_blocks_allocated"] == S.n_alloc
+        assert info["grid_bytes"] == S.n_alloc * B ** 3 * 8 + S.table.size * 4
+        assert np.array_equal(omerf.block_table(h), S.table.ravel())
+        rgb, ns = omerf.render(h, cams, 72, 56)
+        torch.cuda.synchronize()
+        res = omerf.gather_probe(h, cams[0], 72, 56, repeats=1, flush_l2=False)
+    ref = O.render(cams, 72, 56, mode="brute")
+    assert ref["nsamples"].sum() > 5000 and 0 < S.n_alloc < S.table.size
+    _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, f"sparse blocks B={B}")
+    assert res["samples"] == int(ref["nsamples"][0].sum())
+
+
+def test_sparse_block_grid_config0_and_rejections(omerf, oracle):
+    import torch
+    sc, cams = synth.make_scene(0), synth.make_cameras(0)
+    W, H = synth.config_resolution(0)
+    with omerf.scene_create(sc, grid_block=8) as h:
+        rgb, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+    ref = oracle.OracleScene(sc).render(cams, W, H, mode="clipped")
+    _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, "config 0, sparse blocks")
+    with pytest.raises(omerf.OmerfError):
+        omerf.scene_create(sc, grid_block=3)
+    with omerf.scene_create(sc) as h:
+        with pytest.raises(omerf.OmerfError):
+            omerf.block_table(h)
