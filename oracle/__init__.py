@@ -253,3 +253,17 @@ def grid_corners(O: OracleScene, p) -> np.ndarray:
     c = np.zeros(6, dtype=np.int32)
     lib().orc_grid_corners(O.c.grid_n, O.c.box, _ptr(p, _f32p), _ptr(c, C.POINTER(C.c_int32)))
     return c
+
+
+def mlp_smoothness(O: OracleScene, F, d, delta, want_G: bool = False):
+    """Eq. 9-10 forward: per-direction loss terms, and optionally G for every (direction, perturbation)."""
+    F = np.ascontiguousarray(F, dtype=np.float32)
+    d = np.ascontiguousarray(d, dtype=np.float32)
+    delta = np.ascontiguousarray(delta, dtype=np.float32)
+    n, S = delta.shape[0], delta.shape[1]
+    assert F.shape == (n, 7) and d.shape == (n, 3) and delta.shape == (n, S, 3)
+    loss = np.zeros(n, dtype=np.float64)
+    G = np.zeros((n, S + 1, 3), dtype=np.float64) if want_G else None
+    lib().orc_mlp_smoothness(C.byref(O.c), C.c_int64(n), C.c_int(S), _ptr(F, _f32p), _ptr(d, _f32p), _ptr(delta, _f32p),
+                             _ptr(loss, C.POINTER(C.c_double)), _ptr(G, C.POINTER(C.c_double)) if want_G else None)
+    return (loss, G) if want_G else loss

@@ -720,3 +720,44 @@ int orc_sparse_grid_lookup(const int32_t *table, const uint8_t *atlas, int B, co
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------ view-direction smoothness term */
+/* PAPER.md:145-155, Eq. 9-10: for a viewing direction d, perturbed directions s = d + delta (delta ~ N(0, Sigma) is an
+ * INPUT here: the random draws are the caller's) and
+ *     l(d) = sum_s S(d, s) || G(F, s) - G(F, d) ||_2^2,     S = cosine similarity,
+ * the forward pass of the regulariser as a batched workload of the deferred MLP G (Eq. 4).
+ * Readings (R25): s is fed to the direction encoding as it is (not re-normalised; the cosine carries the
+ * norms), F is the 7-vector [sum w c^d, sum w f] of Eq. 4, G's output is its three sigmoid colours.
+ *   F double-free inputs: F float [n][7], d float [n][3], delta float [n][S][3]; s_c = d_c + delta_c in fp32 (one add).
+ *   out_loss double [n]; out_G double [n][S+1][3] or NULL (row 0 = G(F,d)). */
+void orc_mlp_smoothness(const orc_scene *s, int64_t n, int S, const float *F, const float *d, const float *delta,
+                        double *out_loss, double *out_G)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; i++) {
+        double in[64], G0[3], Gs[3];
+        for (int c = 0; c < 7; c++) in[c] = (double)F[i * 7 + c];
+        const float *di = d + i * 3;
+        orc_encode_dir(di, in + 7);
+        orc_mlp(s, in, G0);
+        if (out_G) for (int c = 0; c < 3; c++) out_G[(i * (S + 1)) * 3 + c] = G0[c];
+        double loss = 0.0;
+        for (int j = 0; j < S; j++) {
+            float sv[3];
+            for (int c = 0; c < 3; c++) sv[c] = di[c] + delta[(i * S + j) * 3 + c];
+            orc_encode_dir(sv, in + 7);
+            orc_mlp(s, in, Gs);
+            double dot = 0.0, nd = 0.0, ns = 0.0, diff2 = 0.0;
+            for (int c = 0; c < 3; c++) {
+                dot += (double)di[c] * (double)sv[c];
+                nd += (double)di[c] * (double)di[c];
+                ns += (double)sv[c] * (double)sv[c];
+                diff2 += (Gs[c] - G0[c]) * (Gs[c] - G0[c]);
+            }
+            double cosv = (nd > 0.0 && ns > 0.0) ? dot / sqrt(nd * ns) : 0.0;   /* S(d, s) */
+            loss += cosv * diff2;
+            if (out_G) for (int c = 0; c < 3; c++) out_G[(i * (S + 1) + j + 1) * 3 + c] = Gs[c];
+        }
+        out_loss[i] = loss;
+    }
+}

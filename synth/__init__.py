@@ -17,5 +17,6 @@ from .scenes import (  # noqa: F401
     low_altitude_cameras,
     orbit_cameras,
     smoothed_bytes,
+    smoothness_batch,
     CAMERA_FLOATS,
 )

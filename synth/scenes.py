@@ -340,3 +340,19 @@ def custom_scene(*, box=(8.0, 8.0, 4.0), hf_n=(9, 9), h_lo=1.0, h_up=3.0, grid_n
     return Scene(tuple(float(b) for b in box), hf(h_lo), hf(h_up), tex(grid_n, 3), tex(xy_n, 2),
                  tex(xz_n, 2), tex(yz_n, 2), *mlp, step=step, t_stop=t_stop, bg=tuple(bg),
                  occ_n=tuple(occ_n), name="custom")
+
+
+# --------------------------------------------------------------------------------------
+# inputs of the view-direction smoothness workload (Eq. 9-10) - random draws only
+# --------------------------------------------------------------------------------------
+def smoothness_batch(seed: int, n: int, S: int, sigma: float = 0.05):
+    """F float32 [n][7] ~ U(0,1) (accumulated colour / feature sums of Eq. 4 lie in [0,1]), unit directions d [n][3]
+    on the lower hemisphere (cameras look down), and the Gaussian perturbations delta [n][S][3] ~ N(0, sigma^2 I)
+    of Eq. 9.  The method's arithmetic (encoding, MLP, cosine, loss) is NOT here."""
+    rng = np.random.default_rng(seed)
+    F = rng.random((n, 7), dtype=np.float32)
+    g = rng.standard_normal((n, 3))
+    g[:, 2] = -np.abs(g[:, 2])
+    d = (g / np.linalg.norm(g, axis=1, keepdims=True)).astype(np.float32)
+    delta = (sigma * rng.standard_normal((n, S, 3))).astype(np.float32)
+    return F, d, delta
