@@ -319,6 +319,63 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_smoothness(args):
+    """--workload smoothness: Eq. 9-10 forward over 2^20 directions x 15 perturbations on the
+    config-1 scene's MLP.  Secondary line: same JSON shape, metric = MLP evaluations per second."""
+    import torch
+
+    import paper_2404_09531_b200 as omerf
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    n, S = 1 << 20, 15
+    scene = synth.make_scene(0)                  # the MLP is all this workload uses; weights are Xavier as everywhere
+    F, d, delta = synth.smoothness_batch(7, n, S)
+    h = omerf.scene_create(scene)
+    tF, td, tdl = (torch.from_numpy(a).cuda() for a in (F, d, delta))
+    out = torch.empty(n, dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+    for _ in range(max(args.warmup, 3)):
+        omerf.mlp_smoothness(h, tF, td, tdl, out_loss=out)
+    torch.cuda.synchronize()
+    ms = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        omerf.mlp_smoothness(h, tF, td, tdl, out_loss=out)
+        b.record(stream)
+        torch.cuda.synchronize()
+        ms.append(a.elapsed_time(b))
+    evals = n * (S + 1)
+    t = float(np.mean(ms)) / 1e3
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    alg_bytes = n * (7 + 3 + 3 * S + 1) * 4
+    tflops = evals * 2 * 883 / t / 1e12
+    tf32_peak = float(peaks.get("bf16_tflops", 2250.0)) * 0.5
+    import oracle
+    m = 4096
+    t0 = time.perf_counter()
+    oracle.mlp_smoothness(oracle.OracleScene(scene), F[:m], d[:m], delta[:m])
+    cpu_s = time.perf_counter() - t0
+    line = {"metric": "MLP evaluations/s", "value": evals / t, "unit": "eval/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32 (3xTF32 tensor-core products)", "data": "synthetic",
+            "config": {"workload": "SURVEY 8(f).3 smoothness term, 2^20 directions x 15 perturbations", "n": n, "S": S,
+                       "l2": "flushed between timed steps"},
+            "gpu_launches": args.steps, "mean_loss": float(out.mean().item()),
+            # a dense contraction (883 MACs per evaluation) on tensor cores: tf32 peak = measured bf16 peak x 1/2 (guide's
+            # nominal ratio); the kernel issues 3 tf32 products per algorithmic product (hi/lo split for fp32 accuracy)
+            "roofline": {"bound": "tensor", "achieved": tflops, "peak": tf32_peak, "unit": "TFLOP/s", "frac": tflops / tf32_peak,
+                         "traffic": None, "algorithmic_flops_per_launch": evals * 2 * 883, "executed_mma_tflops": 3 * tflops,
+                         "peak_source": "MEASURED_PEAKS.json bf16_tflops x 0.5 (tf32)" if peaks else "fallback 2250 x 0.5",
+                         "hbm_gbs_algorithmic": alg_bytes / t / 1e9, "hbm_peak": hbm},
+            "cpu_baseline": {"value": m * (S + 1) / cpu_s, "unit": "eval/s", "cores": os.cpu_count(), "kind": "oracle",
+                             "sample": f"first {m} directions"}}
+    print(json.dumps(line))
+    omerf.scene_destroy(h)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -330,8 +387,11 @@ def main():
     ap.add_argument("--soft-eps", type=float, default=0.0, help="SURVEY 8(f).2: soft occupancy (Eq. 6-8) buffer height; 0 = binary mask")
     ap.add_argument("--grid-block", type=int, default=0, help="SURVEY 8(f).1: store V as sparse blocks of this edge (0 = dense)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="render", choices=["render", "smoothness"])
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.workload == "smoothness" and args.impl == "ours":
+        run_smoothness(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -118,6 +118,17 @@ typedef struct {
 int omerf_gather_probe(const omerf_scene *scene, const omerf_camera *camera /*HOST, one view*/, int W, int H,
                        int repeats, int flush_l2, omerf_gather_probe_result *out /*HOST*/);
 
+/* View-direction smoothness term, forward pass (Eq. 9-10): for each of n viewing
+ * directions d_i with deferred-shading input F_i = [sum w c^d (3), sum w f (4)] (Eq. 4) and S perturbations delta_is
+ * (the caller's draws from N(0, Sigma), Eq. 9),
+ *     out_loss[i] = sum_s cos(d_i, d_i + delta_is) * || G(F_i, d_i + delta_is) - G(F_i, d_i) ||_2^2       (Eq. 10)
+ * with the scene's deferred MLP G.  The perturbed direction enters the encoding as it is (R25).
+ *   F DEVICE float32 [n][7], dir DEVICE [n][3], delta DEVICE [n][S][3], out_loss DEVICE [n],
+ *   out_G DEVICE [n][S+1][3] (row 0 = G(F,d)) or NULL.  Asynchronous on `stream`; n >= 0, S >= 0. */
+int omerf_mlp_smoothness(const omerf_scene *scene, int64_t n, int S, const float *F /*DEVICE*/,
+                         const float *dir /*DEVICE*/, const float *delta /*DEVICE*/, float *out_loss /*DEVICE*/,
+                         float *out_G /*DEVICE or NULL*/, void *stream);
+
 /* Number of kernels of this library the last omerf_render / omerf_render_host on this scene launched. */
 int omerf_last_launch_count(const omerf_scene *scene);
 

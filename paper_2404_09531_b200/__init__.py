@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     gather_probe,
     last_launch_count,
     load_library,
+    mlp_smoothness,
     pyramid_level,
     render,
     render_host,

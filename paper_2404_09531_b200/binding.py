@@ -22,7 +22,8 @@ SAMPLER_PLANE = 0
 SAMPLER_GRID = 1
 
 EXPORTS = (
-    "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_gather_probe", "omerf_last_launch_count",
+    "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_gather_probe", "omerf_mlp_smoothness",
+    "omerf_last_launch_count",
     "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield", "omerf_scene_get_block_table",
     "omerf_scene_destroy", "omerf_last_error", "omerf_version",
 )
@@ -77,6 +78,8 @@ def load_library() -> C.CDLL:
     L.omerf_render_host.argtypes = L.omerf_render.argtypes
     L.omerf_gather_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
                                      C.POINTER(GatherProbeResult)]
+    L.omerf_mlp_smoothness.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                       C.c_void_p, C.c_void_p]
     L.omerf_last_launch_count.argtypes = [C.c_void_p]
     L.omerf_scene_get_info.argtypes = [C.c_void_p, C.POINTER(SceneInfo)]
     L.omerf_scene_get_pyramid_level.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
@@ -229,6 +232,24 @@ def gather_probe(h: SceneHandle, camera, W: int, H: int, repeats: int = 10, flus
            "omerf_gather_probe")
     return {"samples": int(res.samples), "ms_frame_order": float(res.ms_frame_order),
             "ms_scattered": float(res.ms_scattered)}
+
+
+def mlp_smoothness(h: SceneHandle, F, dirs, delta, out_loss=None, out_G=None, want_G: bool = False, stream=None):
+    """omerf_mlp_smoothness (Eq. 9-10 forward): DEVICE float32 tensors F [n][7], dirs [n][3], delta [n][S][3].
+    Returns out_loss [n] (and out_G [n][S+1][3] if want_G); asynchronous on `stream`."""
+    import torch
+    n, S = int(delta.shape[0]), int(delta.shape[1])
+    for a, shp in ((F, (n, 7)), (dirs, (n, 3)), (delta, (n, S, 3))):
+        assert a.is_cuda and a.dtype == torch.float32 and a.is_contiguous() and tuple(a.shape) == shp
+    if out_loss is None:
+        out_loss = torch.empty(n, dtype=torch.float32, device="cuda")
+    if want_G and out_G is None:
+        out_G = torch.empty((n, S + 1, 3), dtype=torch.float32, device="cuda")
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(load_library().omerf_mlp_smoothness(h.ptr, n, S, F.data_ptr(), dirs.data_ptr(), delta.data_ptr(),
+                                               out_loss.data_ptr(), out_G.data_ptr() if out_G is not None else None,
+                                               st.cuda_stream), "omerf_mlp_smoothness")
+    return (out_loss, out_G) if want_G else out_loss
 
 
 def last_launch_count(h: SceneHandle) -> int:

@@ -368,6 +368,18 @@ extern "C" int omerf_gather_probe(const omerf_scene *s, const omerf_camera *came
     return rc;
 }
 
+extern "C" int omerf_mlp_smoothness(const omerf_scene *s, int64_t n, int S, const float *F, const float *dir,
+                                    const float *delta, float *out_loss, float *out_G, void *stream)
+{
+    if (!s) return invalid("null scene");
+    if (n < 0 || S < 0) return invalid("n >= 0 and S >= 0 required");
+    if (n == 0) return OMERF_OK;
+    if (!F || !dir || !out_loss || (S > 0 && !delta)) return invalid("null F/dir/delta/out_loss");
+    if ((unsigned long long)n * (unsigned long long)(S + 1) > 0x7fffffffffffull) return invalid("batch too large");
+    s->last_launches = 1;
+    return omerf_launch_smoothness(s, n, S, F, dir, delta, out_loss, out_G, (cudaStream_t)stream);
+}
+
 extern "C" int omerf_last_launch_count(const omerf_scene *s) { return s ? s->last_launches : 0; }
 
 extern "C" int omerf_scene_get_info(const omerf_scene *s, omerf_scene_info *out)

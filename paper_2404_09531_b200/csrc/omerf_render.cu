@@ -29,6 +29,7 @@
 #include <stdio.h>
 
 #include "omerf_device.cuh"
+#include "omerf_mlp.cuh"
 
 namespace {
 
@@ -110,66 +111,15 @@ __device__ __forceinline__ int index_before(float t_end, float inv_step, int k1)
 }
 
 // ---------------------------------------------------------------------------------- S4: one traversal step
-// sampler PLANE.  Advances (k, lvl); returns ST_READY when lattice sample k passes the predicate (Eq. 7),
-// ST_FIN when no sample is left, ST_TRAV otherwise.
-__device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl)
-{
-    if (k > k1) return ST_FIN;
-    float px, py, pz;
-    lattice_point(r, sc.step, k, px, py, pz);
-    const int top = sc.n_levels - 1;
-    // cell indices are clamped, so points of the 2-index padding outside the box still address valid nodes;
-    // the box test is only needed where a sample is declared
-    const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
-    const int nx = ix >> lvl, ny = iy >> lvl;
-    const float2 h = __ldg(sc.pyr + sc.lvl_off[lvl] + nx * sc.lvl_ny[lvl] + ny);
-    const bool above = pz > h.y, below = pz < h.x;
-    if (!above && !below) {
-        if (lvl == 0) {
-            if (in_box(sc, px, py, pz)) return ST_READY; // z_min <= z <= z_max at the nearest grid point (Eq. 7)
-            k++;
-            return ST_TRAV;
-        }
-        lvl = max(lvl - 2, 0); // level policy tuned with a CPU model of this loop on configs[1]: 17 -> 11 steps per ray
-        return ST_TRAV;
-    }
-    // outside the node's z-range: propose a jump to the node's xy exit or to where z reaches the range.
-    // The boundary crossed decides the next level: an even boundary index also leaves the parent node.
-    const int bxi = nx + (r.dx > 0.0f ? 1 : 0), byi = ny + (r.dy > 0.0f ? 1 : 0);
-    const float xb = fmaf((float)(bxi << lvl), sc.cell_x, -0.5f * sc.cell_x);
-    const float yb = fmaf((float)(byi << lvl), sc.cell_y, -0.5f * sc.cell_y);
-    const float tx = r.dx != 0.0f ? (xb - r.ox) * r.ix : INFINITY;
-    const float ty = r.dy != 0.0f ? (yb - r.oy) * r.iy : INFINITY;
-    float tz = INFINITY;
-    if (above && !below && r.dz < 0.0f) tz = (h.y - r.oz) * r.iz;
-    if (below && !above && r.dz > 0.0f) tz = (h.x - r.oz) * r.iz;
-    const float t_end = fminf(fminf(tx, ty), tz);
-    const int kk = index_before(t_end, sc.inv_step, k1);
-    if (kk > k) {
-        float qx, qy, qz;
-        lattice_point(r, sc.step, kk, qx, qy, qz);
-        const int jx = cell_index(qx, sc.sx, sc.Mx) >> lvl, jy = cell_index(qy, sc.sy, sc.My) >> lvl;
-        const bool same_side = (above ? qz > h.y : true) && (below ? qz < h.x : true);
-        if (jx == nx && jy == ny && same_side) {
-            k = kk + 1;
-            if (tz <= fminf(tx, ty)) {
-                lvl = max(lvl - 2, 0); // entering the node's z-range: refine
-            } else {
-                const int crossed = tx <= ty ? bxi : byi;
-                lvl = min(lvl + ((crossed & 1) ^ 1), top); // an even boundary index also leaves the parent node
-            }
-            return ST_TRAV;
-        }
-    }
-    if (lvl > 0) lvl--;
-    else k++; // level 0 and the predicate is false at k
-    return ST_TRAV;
-}
-
-// The same step without branches (selects only): two rays per lane can then be interleaved by the compiler, which
-// doubles the loads in flight of this latency-bound loop, and the warp no longer serialises the inside / jump /
-// descend paths.  Semantics are identical to trav_step_plane (kept above as the readable statement of the step).
-__device__ __forceinline__ int trav_step_plane_bf(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl, int status)
+// sampler PLANE.  One step for a ray in state ST_TRAV (any other status passes through): advances (k, lvl) and returns
+// ST_READY when lattice sample k passes the predicate (Eq. 7), ST_FIN when no sample is left, ST_TRAV otherwise.
+//   inside the node's [min,max]:  level 0 -> the sample is occupied if it is in the box, else k+1; level > 0 -> descend 2
+//   outside:  propose a jump to the node's xy exit or to where z reaches the range; if the last index before that
+//             (kk) is verified to lie in the same node on the same side, k = kk+1 and the level follows the boundary
+//             crossed (entering the z-range: descend 2; an even xy boundary also leaves the parent: ascend 1);
+//             otherwise descend one level, or k+1 at level 0.
+// Written without branches (selects only): the warp does not serialise the inside / jump / descend paths.
+__device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl, int status)
 {
     const bool run = status == ST_TRAV && k <= k1;
     float px, py, pz;
@@ -432,8 +382,6 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
     bilinear8_dp(t3[0], t3[1], t3[2], t3[3], w3, I);
 }
 
-__device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
-
 // per-sample activations (Eq. 3, colour path only): sigmoid(x) = 1/2 + 1/2 tanh(x/2) with one MUFU.TANH.
 // tanh.approx has an absolute error of about 2^-11 = 5e-4, so the sigmoid is off by <= 2.5e-4; the compositing
 // weights sum to <= 1, which bounds the contribution to the pixel at 2.5e-4 of the 2e-3 budget.
@@ -442,110 +390,6 @@ __device__ __forceinline__ float sigmoid_tanh(float x)
     float t;
     asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(0.5f * x));
     return fmaf(t, 0.5f, 0.5f);
-}
-
-// ---------------------------------------------------------------------------------- S8: deferred MLP (Eq. 4)
-// Warp-cooperative: the 34 -> 16 -> 16 -> 3 network of 16 rays at a time as m16n8k8 tensor-core tiles.
-// tf32 operands are split hi + lo (3 mma per tile product), so the result keeps fp32-level accuracy; hidden
-// activations stay in registers (the C fragment of one layer is the A fragment of the next, see mlp_pack_kernel).
-#define OMERF_XS 44 // row stride of the staged input tile in floats: conflict-free A-fragment loads
-
-// x = hi + lo with hi = x truncated to tf32 (10 explicit mantissa bits) and lo = x - hi exactly; the tensor core
-// reads only the tf32 part of lo, which leaves a relative error of about 2^-21 in the product sum
-__device__ __forceinline__ void split_tf32(float x, uint32_t &hi, uint32_t &lo)
-{
-    hi = __float_as_uint(x) & 0xffffe000u;
-    lo = __float_as_uint(x - __uint_as_float(hi));
-}
-
-__device__ __forceinline__ void mma_tf32(float c[4], const uint32_t a[4], float b0, float b1)
-{
-    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(__float_as_uint(b0)), "r"(__float_as_uint(b1)));
-}
-
-// c += A * B for one k-step/n-tile, A given as fp32 values (split here), B from the packed table
-__device__ __forceinline__ void mma_x3(float c[4], const uint32_t ahi[4], const uint32_t alo[4], const float2 *__restrict__ tab,
-                                       int tile, int lane)
-{
-    const float2 bhi = __ldg(tab + (tile * 2 + 0) * 32 + lane), blo = __ldg(tab + (tile * 2 + 1) * 32 + lane);
-    mma_tf32(c, alo, bhi.x, bhi.y);
-    mma_tf32(c, ahi, blo.x, blo.y);
-    mma_tf32(c, ahi, bhi.x, bhi.y);
-}
-
-// MLP input of one ray: [sum w c^d (3), sum w f (4), d (3), sin/cos(2^j d) j = 0..3 (24)]  (R13)
-__device__ __forceinline__ void mlp_input(const float acc[7], float dx, float dy, float dz, float in[OMERF_MLP_IN])
-{
-#pragma unroll
-    for (int i = 0; i < 7; i++) in[i] = acc[i];
-    const float d[3] = {dx, dy, dz};
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        in[7 + c] = d[c];
-        float s, co;
-        sincosf(d[c], &s, &co); // |d| <= 1: no range-reduction slow path
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-            in[10 + (3 * j + c) * 2] = s;
-            in[10 + (3 * j + c) * 2 + 1] = co;
-            const float s2 = 2.0f * s * co, c2 = 1.0f - 2.0f * s * s; // double angle: sin/cos(2^(j+1) d)
-            s = s2;
-            co = c2;
-        }
-    }
-}
-
-// Evaluates G for the rays staged by lanes [16*half, 16*half+16) and returns this lane's share of the output
-// C fragment: out[0], out[1] = row g cols 2t, 2t+1; out[2], out[3] = row g+8 (pre-sigmoid; cols >= 3 unused).
-__device__ __forceinline__ void mlp_half(const float2 *__restrict__ tab, const float *X, int lane, float out[4])
-{
-    const int g = lane >> 2, t = lane & 3;
-    float c1[2][4], c2[2][4];
-#pragma unroll
-    for (int q = 0; q < 2; q++) {
-        const float2 bq = __ldg(tab + OMERF_MLP_BIAS_OFF + q * 32 + lane), bq2 = __ldg(tab + OMERF_MLP_BIAS_OFF + (2 + q) * 32 + lane);
-        c1[q][0] = c1[q][2] = bq.x;
-        c1[q][1] = c1[q][3] = bq.y;
-        c2[q][0] = c2[q][2] = bq2.x;
-        c2[q][1] = c2[q][3] = bq2.y;
-    }
-    // layer 1: K = 34 (padded to 40), N = 16
-#pragma unroll
-    for (int s = 0; s < 5; s++) {
-        uint32_t ahi[4], alo[4];
-        split_tf32(X[g * OMERF_XS + 8 * s + t], ahi[0], alo[0]);
-        split_tf32(X[(g + 8) * OMERF_XS + 8 * s + t], ahi[1], alo[1]);
-        split_tf32(X[g * OMERF_XS + 8 * s + t + 4], ahi[2], alo[2]);
-        split_tf32(X[(g + 8) * OMERF_XS + 8 * s + t + 4], ahi[3], alo[3]);
-#pragma unroll
-        for (int q = 0; q < 2; q++) mma_x3(c1[q], ahi, alo, tab, s * 2 + q, lane);
-    }
-    // layer 2: K = 16, N = 16; A fragment of k-step s = relu(C fragment of n-tile s)
-#pragma unroll
-    for (int s = 0; s < 2; s++) {
-        uint32_t ahi[4], alo[4];
-        split_tf32(fmaxf(c1[s][0], 0.0f), ahi[0], alo[0]);
-        split_tf32(fmaxf(c1[s][2], 0.0f), ahi[1], alo[1]);
-        split_tf32(fmaxf(c1[s][1], 0.0f), ahi[2], alo[2]);
-        split_tf32(fmaxf(c1[s][3], 0.0f), ahi[3], alo[3]);
-#pragma unroll
-        for (int q = 0; q < 2; q++) mma_x3(c2[q], ahi, alo, tab, 10 + s * 2 + q, lane);
-    }
-    // layer 3: K = 16, N = 3 (padded to 8)
-    const float2 b3 = __ldg(tab + OMERF_MLP_BIAS_OFF + 4 * 32 + lane);
-    out[0] = out[2] = b3.x;
-    out[1] = out[3] = b3.y;
-#pragma unroll
-    for (int s = 0; s < 2; s++) {
-        uint32_t ahi[4], alo[4];
-        split_tf32(fmaxf(c2[s][0], 0.0f), ahi[0], alo[0]);
-        split_tf32(fmaxf(c2[s][2], 0.0f), ahi[1], alo[1]);
-        split_tf32(fmaxf(c2[s][1], 0.0f), ahi[2], alo[2]);
-        split_tf32(fmaxf(c2[s][3], 0.0f), ahi[3], alo[3]);
-        mma_x3(out, ahi, alo, tab, 14 + s, lane);
-    }
 }
 
 // ---------------------------------------------------------------------------------- S2 + S3: new ray for a lane
@@ -677,7 +521,7 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
     #pragma unroll
                     for (int q = 0; q < R; q++) {
                         if (SAMPLER == OMERF_SAMPLER_PLANE) {
-                            status[q] = trav_step_plane_bf(sc, r[q], k[q], k1[q], lvl[q], status[q]);
+                            status[q] = trav_step_plane(sc, r[q], k[q], k1[q], lvl[q], status[q]);
                         } else {
                             if (status[q] == ST_TRAV) status[q] = trav_step_grid(sc, r[q], k[q], k1[q], lvl[q]);
                         }
