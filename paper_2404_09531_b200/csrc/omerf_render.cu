@@ -447,10 +447,13 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 #define OMERF_POOL 96          // rays per warp; a multiple of 32
 #endif
 #ifndef OMERF_TRAV_STEPS
-#define OMERF_TRAV_STEPS 6     // traversal steps per visit while at least OMERF_TRAV_KEEP lanes still traverse
+#define OMERF_TRAV_STEPS 48    // cap on the traversal steps of one visit
 #endif
 #ifndef OMERF_TRAV_KEEP
 #define OMERF_TRAV_KEEP 16
+#endif
+#ifndef OMERF_TRAV_SWAP
+#define OMERF_TRAV_SWAP 8      // lanes that must be free before they take the next listed rays
 #endif
 #ifndef OMERF_SAMPLE_KEEP
 #define OMERF_SAMPLE_KEEP 24   // sample again at once while this many lanes stand on an occupied point
@@ -473,7 +476,7 @@ struct WarpPool {
     int k[OMERF_POOL], k1[OMERF_POOL];
     uint32_t Q[OMERF_POOL], n[OMERF_POOL], pix[OMERF_POOL];
     float acc[7][OMERF_POOL];
-    uint32_t list[32];      // slots picked for this round
+    uint8_t list[OMERF_POOL]; // slots in the picked state, in slot order (phases other than traversal use the first 32)
     float X[16 * OMERF_XS]; // staged MLP inputs of 16 rays
 };
 
@@ -483,70 +486,90 @@ __device__ __forceinline__ uint32_t pack_meta(int status, int lvl, uint32_t view
 }
 
 // ---------------------------------------------------------------------------------- S4: one traversal visit
-// A few steps of the hierarchical DDA for the first min(n_sel, 32 R) listed rays, R rays per lane.
-template <int SAMPLER, int R>
+// Steps the hierarchical DDA for the rays listed in P.list[0 .. n_sel) (all rays of the pool in state ST_TRAV).  The
+// first 32 start at once; when OMERF_TRAV_SWAP lanes have finished their ray (it reached a sample or ran out), those
+// lanes write it back and take the next listed rays, so the warp stays full without a new census of the pool.  The
+// visit ends when the list is exhausted and fewer than OMERF_TRAV_KEEP lanes still traverse, or after
+// OMERF_TRAV_STEPS steps (occupied rays then get their samples).
+struct TravLane {
+    Ray r;
+    int k, k1, lvl, status, slot; // slot < 0: the lane holds no ray
+    uint32_t view;
+};
+
+__device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P, const omerf_camera *__restrict__ cams, int slot,
+                                          TravLane &L)
+{
+    L.slot = slot;
+    const int s_ = slot < 0 ? 0 : slot; // idle lanes read slot 0 and step nothing
+    const uint32_t m = P.meta[s_];
+    L.status = slot < 0 ? ST_IDLE : ST_TRAV;
+    L.lvl = (int)((m >> 2) & 31u);
+    L.view = m >> 8;
+    L.k = P.k[s_];
+    L.k1 = P.k1[s_];
+    L.r.dx = P.dx[s_];
+    L.r.dy = P.dy[s_];
+    L.r.dz = P.dz[s_];
+    L.r.ox = __ldg(&cams[L.view].origin[0]);
+    L.r.oy = __ldg(&cams[L.view].origin[1]);
+    L.r.oz = __ldg(&cams[L.view].origin[2]);
+    L.r.ix = L.r.dx != 0.0f ? __fdividef(1.0f, L.r.dx) : INFINITY;
+    L.r.iy = L.r.dy != 0.0f ? __fdividef(1.0f, L.r.dy) : INFINITY;
+    L.r.iz = L.r.dz != 0.0f ? __fdividef(1.0f, L.r.dz) : INFINITY;
+}
+
+__device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, const TravLane &L, float *__restrict__ out_rgb,
+                                           uint32_t *__restrict__ out_n)
+{
+    const int s_ = L.slot;
+    int st_ = L.status;
+    if (st_ == ST_FIN && P.n[s_] == 0) { // no sample at all: background exactly, MLP skipped (R14)
+        const size_t pix = P.pix[s_];
+        out_rgb[pix * 3 + 0] = sc.bg[0];
+        out_rgb[pix * 3 + 1] = sc.bg[1];
+        out_rgb[pix * 3 + 2] = sc.bg[2];
+        out_n[pix] = 0;
+        st_ = ST_IDLE;
+    }
+    P.k[s_] = L.k;
+    P.meta[s_] = pack_meta(st_, L.lvl, L.view);
+}
+
+template <int SAMPLER>
 __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, const omerf_camera *__restrict__ cams, int lane,
                                            int n_sel, float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
 {
-                int status[R], k[R], k1[R], lvl[R], sl[R];
-                uint32_t view[R];
-                Ray r[R];
-                const int n_trav = min(n_sel, 32 * R);
-                const unsigned FULL = 0xffffffffu;
-    #pragma unroll
-                for (int q = 0; q < R; q++) {
-                    const bool on = lane + 32 * q < n_trav;
-                    sl[q] = on ? (int)P.list[lane + 32 * q] : -1;
-                    const int s_ = on ? sl[q] : 0; // idle lanes read slot 0 and step nothing
-                    const uint32_t m = P.meta[s_];
-                    status[q] = on ? ST_TRAV : ST_IDLE;
-                    lvl[q] = (int)((m >> 2) & 31u);
-                    view[q] = m >> 8;
-                    k[q] = P.k[s_];
-                    k1[q] = P.k1[s_];
-                    r[q].dx = P.dx[s_];
-                    r[q].dy = P.dy[s_];
-                    r[q].dz = P.dz[s_];
-                    r[q].ox = __ldg(&cams[view[q]].origin[0]);
-                    r[q].oy = __ldg(&cams[view[q]].origin[1]);
-                    r[q].oz = __ldg(&cams[view[q]].origin[2]);
-                    r[q].ix = r[q].dx != 0.0f ? __fdividef(1.0f, r[q].dx) : INFINITY;
-                    r[q].iy = r[q].dy != 0.0f ? __fdividef(1.0f, r[q].dy) : INFINITY;
-                    r[q].iz = r[q].dz != 0.0f ? __fdividef(1.0f, r[q].dz) : INFINITY;
+    const unsigned FULL = 0xffffffffu;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    TravLane L;
+    trav_load(sc, P, cams, lane < n_sel ? (int)P.list[lane] : -1, L);
+    int next = min(n_sel, 32); // first list entry not yet taken
+#pragma unroll 1
+    for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
+        if (SAMPLER == OMERF_SAMPLER_PLANE) {
+            L.status = trav_step_plane(sc, L.r, L.k, L.k1, L.lvl, L.status);
+        } else {
+            if (L.status == ST_TRAV) L.status = trav_step_grid(sc, L.r, L.k, L.k1, L.lvl);
+        }
+        const unsigned going = __ballot_sync(FULL, L.status == ST_TRAV);
+        if (next < n_sel) {
+            // lanes whose ray is done (or that hold none) take the next listed rays, a batch at a time
+            const bool free_lane = L.status != ST_TRAV;
+            const unsigned fm = ~going;
+            if (__popc(fm) >= OMERF_TRAV_SWAP) {
+                if (free_lane) {
+                    if (L.slot >= 0) trav_store(sc, P, L, out_rgb, out_n);
+                    const int idx = next + __popc(fm & lt_mask);
+                    trav_load(sc, P, cams, idx < n_sel ? (int)P.list[idx] : -1, L);
                 }
-                const int keep = n_trav > 32 ? 2 * OMERF_TRAV_KEEP : OMERF_TRAV_KEEP;
-    #pragma unroll 1
-                for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
-                    int left = 0;
-    #pragma unroll
-                    for (int q = 0; q < R; q++) {
-                        if (SAMPLER == OMERF_SAMPLER_PLANE) {
-                            status[q] = trav_step_plane(sc, r[q], k[q], k1[q], lvl[q], status[q]);
-                        } else {
-                            if (status[q] == ST_TRAV) status[q] = trav_step_grid(sc, r[q], k[q], k1[q], lvl[q]);
-                        }
-                    }
-    #pragma unroll
-                    for (int q = 0; q < R; q++) left += __popc(__ballot_sync(FULL, status[q] == ST_TRAV));
-                    if (left < keep) break;
-                }
-    #pragma unroll
-                for (int q = 0; q < R; q++) {
-                    if (sl[q] >= 0) {
-                        const int s_ = sl[q];
-                        int st_ = status[q];
-                        if (st_ == ST_FIN && P.n[s_] == 0) { // no sample at all: background exactly, MLP skipped (R14)
-                            const size_t pix = P.pix[s_];
-                            out_rgb[pix * 3 + 0] = sc.bg[0];
-                            out_rgb[pix * 3 + 1] = sc.bg[1];
-                            out_rgb[pix * 3 + 2] = sc.bg[2];
-                            out_n[pix] = 0;
-                            st_ = ST_IDLE;
-                        }
-                        P.k[s_] = k[q];
-                        P.meta[s_] = pack_meta(st_, lvl[q], view[q]);
-                    }
-                }
+                next = min(next + __popc(fm), n_sel);
+            }
+        } else if (__popc(going) < OMERF_TRAV_KEEP) {
+            break;
+        }
+    }
+    if (L.slot >= 0) trav_store(sc, P, L, out_rgb, out_n);
 }
 
 #ifndef OMERF_MIN_BLOCKS
@@ -623,13 +646,13 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             break; // pool empty and no tile left (otherwise the refill branch was taken)
         }
 #undef OMERF_PICK
-        // ---- the first 32 slots in that state
+        // ---- the slots in that state, in slot order
         {
             int base = 0;
 #pragma unroll
             for (int j = 0; j < OMERF_PJ; j++) {
                 const int pos = base + __popc(b[j] & lt_mask);
-                if (((b[j] >> lane) & 1u) && pos < 32) P.list[pos] = lane + 32 * j;
+                if ((b[j] >> lane) & 1u) P.list[pos] = (uint8_t)(lane + 32 * j);
                 base += __popc(b[j]);
             }
         }
@@ -682,9 +705,9 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                 }
             }
         } else if (phase == ST_TRAV) {
-            // ---- traversal visit (S4).  R = 2 rays per lane (interleaved dependency chains) was measured slower on
-            // B200 at every threshold (0.80-0.86 ms against 0.76 ms per configs[1] frame), so one ray per lane it is.
-            trav_visit<SAMPLER, 1>(sc, P, cams, lane, n_sel, out_rgb, out_n);
+            // ---- traversal visit (S4).  (Two rays per lane, interleaved dependency chains, was measured slower on
+            // B200 at every threshold: 0.80-0.86 ms against 0.76 ms per configs[1] frame.)
+            trav_visit<SAMPLER>(sc, P, cams, lane, n_sel, out_rgb, out_n);
         } else if (phase == ST_READY) {
             // ---- samples: gather, activations, compositing (S5, S6, S7)
             int status = ST_IDLE, k = 0, k1 = -1, lvl = 0;
