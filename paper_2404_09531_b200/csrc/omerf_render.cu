@@ -452,6 +452,9 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 #ifndef OMERF_TRAV_KEEP
 #define OMERF_TRAV_KEEP 16
 #endif
+#ifndef OMERF_SAMPLE_SWAP
+#define OMERF_SAMPLE_SWAP 8    // lanes that must have left the READY state before they take the next listed rays
+#endif
 #ifndef OMERF_TRAV_SWAP
 #define OMERF_TRAV_SWAP 8      // lanes that must be free before they take the next listed rays
 #endif
@@ -462,6 +465,8 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 #define OMERF_SAMPLE_SIGMOID sigmoid_tanh
 #endif
 #define OMERF_WARPS 4
+static_assert(OMERF_SAMPLE_SWAP >= 1 && OMERF_SAMPLE_SWAP <= 32 && OMERF_TRAV_SWAP >= 1 && OMERF_TRAV_SWAP <= 32,
+              "a swap threshold above the warp size would never release a finished lane");
 #ifndef OMERF_ENDGAME_WARPS
 #define OMERF_ENDGAME_WARPS 2   // endgame starts when fewer than this many tiles per warp are left
 #endif
@@ -709,27 +714,40 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             // B200 at every threshold: 0.80-0.86 ms against 0.76 ms per configs[1] frame.)
             trav_visit<SAMPLER>(sc, P, cams, lane, n_sel, out_rgb, out_n);
         } else if (phase == ST_READY) {
-            // ---- samples: gather, activations, compositing (S5, S6, S7)
-            int status = ST_IDLE, k = 0, k1 = -1, lvl = 0;
+            // ---- samples: gather, activations, compositing (S5, S6, S7) for the rays listed in P.list[0 .. n_sel);
+            // lanes whose ray left the READY state take the next listed rays, OMERF_SAMPLE_SWAP lanes at a time
+            int status = ST_IDLE, k = 0, k1 = -1, lvl = 0, sslot = -1;
             uint32_t view = 0, Q = 0, n = 0;
             float acc[7];
             Ray r;
-            if (active) {
-                view = P.meta[slot] >> 8;
-                status = ST_READY;
-                k = P.k[slot];
-                k1 = P.k1[slot];
-                Q = P.Q[slot];
-                n = P.n[slot];
-                r.dx = P.dx[slot];
-                r.dy = P.dy[slot];
-                r.dz = P.dz[slot];
+            auto load_ray = [&](int s_new) {
+                sslot = s_new;
+                const int s_ = s_new < 0 ? 0 : s_new;
+                view = P.meta[s_] >> 8;
+                status = s_new < 0 ? ST_IDLE : ST_READY;
+                k = P.k[s_];
+                k1 = P.k1[s_];
+                Q = P.Q[s_];
+                n = P.n[s_];
+                r.dx = P.dx[s_];
+                r.dy = P.dy[s_];
+                r.dz = P.dz[s_];
                 r.ox = __ldg(&cams[view].origin[0]);
                 r.oy = __ldg(&cams[view].origin[1]);
                 r.oz = __ldg(&cams[view].origin[2]);
 #pragma unroll
-                for (int c = 0; c < 7; c++) acc[c] = P.acc[c][slot];
-            }
+                for (int c = 0; c < 7; c++) acc[c] = P.acc[c][s_];
+            };
+            auto store_ray = [&]() {
+                P.k[sslot] = k;
+                P.Q[sslot] = Q;
+                P.n[sslot] = n;
+#pragma unroll
+                for (int c = 0; c < 7; c++) P.acc[c][sslot] = acc[c];
+                P.meta[sslot] = pack_meta(status, lvl, view);
+            };
+            load_ray(active ? slot : -1);
+            int next = n_act; // first list entry not yet taken
 #pragma unroll 1
             while (true) {
 #ifdef OMERF_X_STATS
@@ -740,7 +758,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                     lattice_point(r, sc.step, k, px, py, pz);
                     if (LOG) {
                         const unsigned at = atomicAdd(tile_counter + 32, 1u);
-                        if (at < log_capacity) sample_log[at] = make_uint2(P.pix[slot], (uint32_t)k);
+                        if (at < log_capacity) sample_log[at] = make_uint2(P.pix[sslot], (uint32_t)k);
                     }
                     // Inside the slab the next lattice point is usually occupied too: test it here (level 0).  The test
                     // does not depend on the features, so its pyramid load is in flight together with the gather.
@@ -783,16 +801,22 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                         lvl = 0;
                     }
                 }
-                if (__popc(__ballot_sync(FULL, status == ST_READY)) < OMERF_SAMPLE_KEEP) break;
+                const unsigned going = __ballot_sync(FULL, status == ST_READY);
+                if (next < n_sel) {
+                    const unsigned fm = ~going;
+                    if (__popc(fm) >= OMERF_SAMPLE_SWAP) {
+                        if (status != ST_READY) {
+                            if (sslot >= 0) store_ray();
+                            const int idx = next + __popc(fm & lt_mask);
+                            load_ray(idx < n_sel ? (int)P.list[idx] : -1);
+                        }
+                        next = min(next + __popc(fm), n_sel);
+                    }
+                } else if (__popc(going) < OMERF_SAMPLE_KEEP) {
+                    break;
+                }
             }
-            if (active) {
-                P.k[slot] = k;
-                P.Q[slot] = Q;
-                P.n[slot] = n;
-#pragma unroll
-                for (int c = 0; c < 7; c++) P.acc[c][slot] = acc[c];
-                P.meta[slot] = pack_meta(status, lvl, view);
-            }
+            if (sslot >= 0) store_ray();
         } else {
             // ---- retire: deferred MLP on tensor cores + outputs (S8, S9)
 #pragma unroll 1
