@@ -231,6 +231,30 @@ def run_ours(args):
     clk = clocks.stop() if rank == 0 else None
     total_ms = float(np.sum(ms))
     samples = int(out_n.sum(dtype=torch.int64).item())
+    per_view = [int(x) for x in out_n.view(n_views, -1).sum(dim=1, dtype=torch.int64).tolist()]
+
+    # configs[4]: the same frame through the other sampler (binary occupancy grid + DDA), timed the same way
+    ablation = None
+    if cfg == 4 and rank == 0:
+        other = omerf.SAMPLER_PLANE if sampler == omerf.SAMPLER_GRID else omerf.SAMPLER_GRID
+        h2 = omerf.scene_create(scene, sampler=other)
+        n2 = torch.empty_like(out_n)
+        rgb2 = torch.empty_like(out_rgb)
+
+        def other_step():
+            omerf.render(h2, cams, W, H, rgb2, n2, stream=stream)
+
+        for _ in range(3):
+            other_step()
+        ms2 = float(np.mean(timed(args.steps, True, other_step)))
+        s2 = int(n2.sum(dtype=torch.int64).item())
+        name = {omerf.SAMPLER_PLANE: "plane", omerf.SAMPLER_GRID: "grid"}
+        ablation = {name[sampler]: {"ms_per_frame": total_ms / args.steps, "frames_per_s": 1e3 / (total_ms / args.steps),
+                                    "samples_per_ray": samples / pixels, "gsamples_s": samples / (total_ms / args.steps) / 1e6},
+                    name[other]: {"ms_per_frame": ms2, "frames_per_s": 1e3 / ms2, "samples_per_ray": s2 / pixels,
+                                  "gsamples_s": s2 / ms2 / 1e6, "occ_bits_set": omerf.scene_info(h2)["occ_bits_set"] or None},
+                    "pixels_where_counts_differ": int((n2 != out_n).sum().item())}
+        omerf.scene_destroy(h2)
 
     # gather calibration: the same frame's 20 texel loads per sample replayed with no arithmetic
     probe = omerf.gather_probe(h, cams[0], W, H, repeats=10, flush_l2=True) if rank == 0 else None
@@ -286,6 +310,7 @@ def run_ours(args):
             "frames_per_s": world * n_views * k / secs,
             "gsamples_s": world * samples * k / secs / 1e9,
             "samples_per_step": samples, "samples_per_ray": samples / pixels,
+            "per_view_samples": per_view,
             "l2_warm": {"ms_per_step": total_warm_ms / k, "mpixels_s": world * pixels * k / (total_warm_ms / 1e3) / 1e6},
             "e2e": {"value": world * pixels * k / (total_e2e_ms / 1e3) / 1e6, "unit": "Mpixels/s",
                     "h2d_bytes_per_step": int(cams.nbytes), "d2h_bytes_per_step": pixels * BYTES_PER_PIXEL,
@@ -310,6 +335,8 @@ def run_ours(args):
                 "ceiling_gsamples_s": ceil_gs, "ceiling_gbs": ceil_gs * 160,
                 "scattered_gsamples_s": probe["samples"] / probe["ms_scattered"] / 1e6,
                 "march_gsamples_s": view0, "frac": view0 / ceil_gs}
+        if ablation is not None:
+            line["ablation"] = ablation
         if cpu is not None:
             line["cpu_baseline"] = {"value": cpu["mpix_s"], "unit": "Mpixels/s", "cores": cpu["cores"], "kind": "oracle",
                                     "sample": cpu["sample"], "msamples_s": cpu["msamples_s"], "seconds": cpu["seconds"]}

@@ -184,7 +184,7 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         }
         if ((rc = omerf_query_persistent_blocks(d->sampler, &s->persistent_blocks))) break;
         {
-            cudaError_t ee = cudaMalloc((void **)&s->d_tile_counter, 64 * sizeof(unsigned int) + 3 * 8 * 8192);
+            cudaError_t ee = cudaMalloc((void **)&s->d_tile_counter, 64 * sizeof(unsigned int) + 8 * 8 * 8192);
             if (ee != cudaSuccess) {
                 rc = omerf_cuda_fail(ee, "cudaMalloc tile counter");
                 break;

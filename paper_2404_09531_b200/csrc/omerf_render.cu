@@ -604,7 +604,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
     __syncwarp();
 #ifdef OMERF_X_TIMELINE
     unsigned long long *tl = reinterpret_cast<unsigned long long *>(tile_counter + 64);
-    if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 3 + 0] = t; }
+    if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8 + 0] = t; }
 #endif
     bool more = true;
     // Endgame: a warp's pool holds about three tiles of work, which would all drain at falling utilisation once the
@@ -646,11 +646,21 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
         else if (cnt[ST_FIN] > 0) OMERF_PICK(ST_FIN) // finished rays wait for a full MLP batch unless nothing else is left
         else {
 #ifdef OMERF_X_TIMELINE
-            if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 3 + 2] = t; }
+            if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8 + 2] = t; }
 #endif
             break; // pool empty and no tile left (otherwise the refill branch was taken)
         }
 #undef OMERF_PICK
+#ifdef OMERF_X_TIMELINE
+        if (lane == 0) {
+            unsigned long long *e = tl + (blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8;
+            if (!more) {
+                if (e[3] == 0) e[3] = 1ull | ((unsigned long long)cnt[ST_TRAV] << 8) | ((unsigned long long)cnt[ST_READY] << 16) | ((unsigned long long)cnt[ST_FIN] << 24);
+                e[4 + (phase == ST_TRAV ? 0 : phase == ST_READY ? 1 : 2)] += 1;
+                e[7] += (unsigned long long)min(n_sel, 32);
+            }
+        }
+#endif
         // ---- the slots in that state, in slot order
         {
             int base = 0;
@@ -678,7 +688,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             if (tile >= total_tiles) {
                 more = false;
 #ifdef OMERF_X_TIMELINE
-                if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 3 + 1] = t; }
+                if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8 + 1] = t; }
 #endif
             } else {
                 const unsigned view = tile / tiles_per_view, tv = tile - view * tiles_per_view;
@@ -938,21 +948,30 @@ int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_
         static int calls = 0;
         if (calls++ == 8) {
             int nw = s->persistent_blocks * OMERF_WARPS;
-            unsigned long long *h = new unsigned long long[nw * 3];
-            cudaMemcpy(h, s->d_tile_counter + 64, sizeof(unsigned long long) * nw * 3, cudaMemcpyDeviceToHost);
+            unsigned long long *h = new unsigned long long[nw * 8];
+            cudaMemcpy(h, s->d_tile_counter + 64, sizeof(unsigned long long) * nw * 8, cudaMemcpyDeviceToHost);
             unsigned long long t0 = ~0ull;
-            for (int i = 0; i < nw; i++) if (h[i * 3] < t0) t0 = h[i * 3];
-            double sum[3] = {0, 0, 0}, mx[3] = {0, 0, 0}, mn[3] = {1e30, 1e30, 1e30};
-            for (int i = 0; i < nw; i++) for (int c = 0; c < 3; c++) { double v = (double)(h[i * 3 + c] - t0) * 1e-3; sum[c] += v; if (v > mx[c]) mx[c] = v; if (v < mn[c]) mn[c] = v; }
-            for (int c = 0; c < 3; c++) printf("TIMELINE %s us: min %.1f mean %.1f max %.1f\n", c == 0 ? "start" : c == 1 ? "exhausted" : "finish", mn[c], sum[c] / nw, mx[c]);
-            // histogram of finish times
-            int hist[16] = {0};
-            for (int i = 0; i < nw; i++) { int b = (int)((double)(h[i * 3 + 2] - t0) * 1e-3 / 100.0); if (b > 15) b = 15; hist[b]++; }
-            printf("TIMELINE finish histogram (100 us bins):");
-            for (int b = 0; b < 16; b++) printf(" %d", hist[b]);
-            printf("\n");
+            for (int i = 0; i < nw; i++) if (h[i * 8] < t0) t0 = h[i * 8];
+            // sort warps by finish time; print stats for all and for the slowest 2 %
+            int *idx = new int[nw];
+            for (int i = 0; i < nw; i++) idx[i] = i;
+            for (int i = 1; i < nw; i++) { int v = idx[i], j = i - 1; while (j >= 0 && h[idx[j] * 8 + 2] > h[v * 8 + 2]) { idx[j + 1] = idx[j]; j--; } idx[j + 1] = v; }
+            for (int pass = 0; pass < 2; pass++) {
+                int lo = pass == 0 ? 0 : nw - nw / 50, cntw = nw - lo;
+                double ex = 0, fin = 0, tr = 0, rd = 0, fn = 0, rt = 0, rr = 0, rf = 0, lanes = 0;
+                for (int q = lo; q < nw; q++) {
+                    unsigned long long *e = h + idx[q] * 8;
+                    ex += (e[1] - t0) * 1e-3; fin += (e[2] - t0) * 1e-3;
+                    tr += (e[3] >> 8) & 255; rd += (e[3] >> 16) & 255; fn += (e[3] >> 24) & 255;
+                    rt += e[4]; rr += e[5]; rf += e[6]; lanes += e[7];
+                }
+                printf("TIMELINE %s (%d warps): exhausted %.1f us, finish %.1f us; at exhaustion TRAV %.1f READY %.1f FIN %.1f; rounds after: trav %.1f sample %.1f retire %.1f, lanes/round %.1f\n",
+                       pass == 0 ? "all" : "slowest 2%", cntw, ex / cntw, fin / cntw, tr / cntw, rd / cntw, fn / cntw, rt / cntw, rr / cntw, rf / cntw, lanes / (rt + rr + rf));
+            }
+            delete[] idx;
             delete[] h;
         }
+        cudaMemsetAsync(s->d_tile_counter + 64, 0, 8 * 8 * 8192, st);
     }
 #endif
 #ifdef OMERF_X_STATS
