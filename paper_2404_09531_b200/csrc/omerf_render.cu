@@ -35,6 +35,24 @@ namespace {
 
 enum : int { ST_IDLE = 0, ST_TRAV = 1, ST_READY = 2, ST_FIN = 3 };
 
+// level policy of the pyramid traversal (speed only: every jump is verified), tuned on B200 with configs[1]
+#ifndef OMERF_LVL_START
+#define OMERF_LVL_START 6      // first node size: 2^6 cells
+#endif
+#ifndef OMERF_LVL_ENTER
+#define OMERF_LVL_ENTER 2      // levels to descend when a jump ends where z enters the node's range
+#endif
+#ifndef OMERF_LVL_INSIDE
+#define OMERF_LVL_INSIDE 2     // levels to descend when the point is inside the node's z-range
+#endif
+#ifndef OMERF_LVL_FAIL
+#define OMERF_LVL_FAIL 2       // levels to descend when the proposed jump could not be verified
+#endif
+#ifndef OMERF_LVL_UP
+#define OMERF_LVL_UP 1         // levels to ascend after a verified jump across an xy node boundary
+#endif
+
+
 // scheduling thresholds (lanes): tuned on B200 with configs[1]
 #ifndef OMERF_RETIRE_T
 #define OMERF_RETIRE_T 12
@@ -116,8 +134,8 @@ __device__ __forceinline__ int index_before(float t_end, float inv_step, int k1)
 //   inside the node's [min,max]:  level 0 -> the sample is occupied if it is in the box, else k+1; level > 0 -> descend 2
 //   outside:  propose a jump to the node's xy exit or to where z reaches the range; if the last index before that
 //             (kk) is verified to lie in the same node on the same side, k = kk+1 and the level follows the boundary
-//             crossed (entering the z-range: descend 2; an even xy boundary also leaves the parent: ascend 1);
-//             otherwise descend one level, or k+1 at level 0.
+//             crossed (entering the z-range: descend OMERF_LVL_ENTER; an xy boundary: ascend OMERF_LVL_UP);
+//             otherwise descend OMERF_LVL_FAIL levels, or k+1 at level 0.
 // Written without branches (selects only): the warp does not serialise the inside / jump / descend paths.
 __device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl, int status)
 {
@@ -146,9 +164,8 @@ __device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r,
     const bool jump = !inside && kk > k && jx == nx && jy == ny && same_side;
     const bool ready = run && inside && lvl == 0 && in_box(sc, px, py, pz);
     // next (k, lvl)
-    const int crossed = tx <= ty ? bxi : byi;
-    const int lvl_jump = tz <= txy ? max(lvl - 2, 0) : min(lvl + ((crossed & 1) ^ 1), top);
-    const int lvl_next = inside ? max(lvl - 2, 0) : (jump ? lvl_jump : max(lvl - 1, 0));
+    const int lvl_jump = tz <= txy ? max(lvl - OMERF_LVL_ENTER, 0) : min(lvl + OMERF_LVL_UP, top);
+    const int lvl_next = inside ? max(lvl - OMERF_LVL_INSIDE, 0) : (jump ? lvl_jump : max(lvl - OMERF_LVL_FAIL, 0));
     const int k_next = jump ? kk + 1 : ((lvl == 0 && !ready) ? k + 1 : k); // level 0 and the predicate is false at k
     if (run) {
         k = k_next;
@@ -597,7 +614,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
     const int tiles_x = (W + 7) >> 3, tiles_y = (H + 3) >> 2;
     const unsigned tiles_per_view = (unsigned)tiles_x * tiles_y;
     const unsigned total_tiles = tiles_per_view * (unsigned)n_views;
-    const int start_lvl = min((SAMPLER == OMERF_SAMPLER_PLANE ? sc.n_levels : sc.occ_levels) - 1, 6);
+    const int start_lvl = min((SAMPLER == OMERF_SAMPLER_PLANE ? sc.n_levels : sc.occ_levels) - 1, OMERF_LVL_START);
 
 #pragma unroll
     for (int j = 0; j < OMERF_PJ; j++) P.meta[lane + 32 * j] = ST_IDLE;
