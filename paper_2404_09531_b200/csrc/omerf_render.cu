@@ -469,6 +469,9 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 #ifndef OMERF_TRAV_KEEP
 #define OMERF_TRAV_KEEP 16
 #endif
+#ifndef OMERF_DRAIN_TRAV_KEEP
+#define OMERF_DRAIN_TRAV_KEEP 1  // in the endgame and the drain a traversal visit runs until every listed ray is done
+#endif
 #ifndef OMERF_SAMPLE_SWAP
 #define OMERF_SAMPLE_SWAP 8    // lanes that must have left the READY state before they take the next listed rays
 #endif
@@ -560,7 +563,7 @@ __device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, cons
 
 template <int SAMPLER>
 __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, const omerf_camera *__restrict__ cams, int lane,
-                                           int n_sel, float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
+                                           int n_sel, int keep, float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
 {
     const unsigned FULL = 0xffffffffu;
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -587,7 +590,7 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
                 }
                 next = min(next + __popc(fm), n_sel);
             }
-        } else if (__popc(going) < OMERF_TRAV_KEEP) {
+        } else if (__popc(going) < keep) {
             break;
         }
     }
@@ -739,7 +742,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
         } else if (phase == ST_TRAV) {
             // ---- traversal visit (S4).  (Two rays per lane, interleaved dependency chains, was measured slower on
             // B200 at every threshold: 0.80-0.86 ms against 0.76 ms per configs[1] frame.)
-            trav_visit<SAMPLER>(sc, P, cams, lane, n_sel, out_rgb, out_n);
+            trav_visit<SAMPLER>(sc, P, cams, lane, n_sel, (more && !endgame) ? OMERF_TRAV_KEEP : OMERF_DRAIN_TRAV_KEEP, out_rgb, out_n);
         } else if (phase == ST_READY) {
             // ---- samples: gather, activations, compositing (S5, S6, S7) for the rays listed in P.list[0 .. n_sel);
             // lanes whose ray left the READY state take the next listed rays, OMERF_SAMPLE_SWAP lanes at a time
