@@ -485,6 +485,7 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 #define OMERF_SAMPLE_SIGMOID sigmoid_tanh
 #endif
 #define OMERF_WARPS 4
+static_assert(OMERF_POOL <= 255, "the census packs the state counts into bytes");
 static_assert(OMERF_SAMPLE_SWAP >= 1 && OMERF_SAMPLE_SWAP <= 32 && OMERF_TRAV_SWAP >= 1 && OMERF_TRAV_SWAP <= 32,
               "a swap threshold above the warp size would never release a finished lane");
 #ifndef OMERF_ENDGAME_WARPS
@@ -634,20 +635,16 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
     const unsigned endgame_tiles = OMERF_ENDGAME_WARPS * gridDim.x * OMERF_WARPS;
 
     while (true) {
-        // ---- census of the pool (idle = the rest)
-        unsigned bal[4][OMERF_PJ];
-        int cnt[4] = {OMERF_POOL, 0, 0, 0};
+        // ---- census of the pool: every lane adds 1 << (8 * state) for its slots, one warp reduction (REDUX) gives the four
+        // counts as the bytes of one word (a pool holds at most 255 rays); ballots are taken for the picked state only
+        uint32_t st_lane[OMERF_PJ], packed = 0;
 #pragma unroll
         for (int j = 0; j < OMERF_PJ; j++) {
-            const uint32_t st = P.meta[lane + 32 * j] & 3u;
-#pragma unroll
-            for (int s = 1; s < 4; s++) {
-                bal[s][j] = __ballot_sync(FULL, st == (uint32_t)s);
-                cnt[s] += __popc(bal[s][j]);
-            }
-            bal[0][j] = ~(bal[1][j] | bal[2][j] | bal[3][j]);
+            st_lane[j] = P.meta[lane + 32 * j] & 3u;
+            packed += 1u << (8 * st_lane[j]);
         }
-        cnt[0] -= cnt[1] + cnt[2] + cnt[3];
+        packed = __reduce_add_sync(FULL, packed);
+        const int cnt[4] = {(int)(packed & 255u), (int)((packed >> 8) & 255u), (int)((packed >> 16) & 255u), (int)(packed >> 24)};
         // ---- pick a phase: full warps first, then the fullest (all warp-uniform)
         int phase, n_sel;
         unsigned b[OMERF_PJ];
@@ -655,7 +652,6 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
     {                                                           \
         phase = (S);                                            \
         n_sel = cnt[S];                                         \
-        _Pragma("unroll") for (int j = 0; j < OMERF_PJ; j++) b[j] = bal[S][j]; \
     }
         if (cnt[ST_FIN] >= 32) OMERF_PICK(ST_FIN)
         else if (cnt[ST_READY] >= 32) OMERF_PICK(ST_READY)
@@ -671,6 +667,8 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             break; // pool empty and no tile left (otherwise the refill branch was taken)
         }
 #undef OMERF_PICK
+#pragma unroll
+        for (int j = 0; j < OMERF_PJ; j++) b[j] = __ballot_sync(FULL, st_lane[j] == (uint32_t)phase);
 #ifdef OMERF_X_TIMELINE
         if (lane == 0) {
             unsigned long long *e = tl + (blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8;
