@@ -858,7 +858,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                         float acc[7];
 #pragma unroll
                         for (int c = 0; c < 7; c++) acc[c] = P.acc[c][slot];
-                        mlp_input(acc, P.dx[slot], P.dy[slot], P.dz[slot], in);
+                        mlp_input<true>(acc, P.dx[slot], P.dy[slot], P.dz[slot], in);
                     }
                     float4 *row = reinterpret_cast<float4 *>(P.X + (lane & 15) * OMERF_XS);
 #pragma unroll

@@ -50,7 +50,7 @@ omerf_smooth_kernel(const float2 *__restrict__ mlp_tab, long long n, int S, cons
                     const float nn = (dx * dx + dy * dy + dz * dz) * (sx * sx + sy * sy + sz * sz);
                     cosv = nn > 0.0f ? dot * rsqrtf(nn) : 0.0f;
                 }
-                mlp_input(f7, sx, sy, sz, in);
+                mlp_input<false>(f7, sx, sy, sz, in);
             }
             float4 *xr = reinterpret_cast<float4 *>(Xs[w][half] + row * OMERF_XS);
 #pragma unroll
