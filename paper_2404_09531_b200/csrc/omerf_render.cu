@@ -1,13 +1,13 @@
-// omerf_render.cu — S2..S9 of the hot path: one persistent kernel per frame batch.
+// omerf_render.cu — S2..S9 of the hot path: one persistent kernel per frame batch (DESIGN.md 5.1).
 //
-// Persistent warps with ray refill.  Each lane owns one ray at a time and is in one of four states:
+// Each warp owns a pool of OMERF_POOL rays in shared memory; a ray is in one of four states:
 //   IDLE -> (refill: S2 ray generation + S3 box clip) -> TRAV -> READY -> (sample) -> TRAV ... -> FIN -> IDLE
-// A warp round runs, in this order and only when enough lanes want it, (1) retire: deferred MLP + store for
-// FIN lanes, (2) refill: IDLE lanes take the next pixels of the warp's current 8x4 tile (tiles come from a
-// global atomic counter), (3) one traversal step for TRAV lanes, (4) one sample for READY lanes.  Rays have
-// very different lengths (about 4 samples on average, a long tail, many sky rays with none), so binding a ray
-// to a lane for the whole kernel leaves two thirds of the lanes idle (measured: 10.5 of 32 lanes active);
-// refill keeps the expensive phases (sample: ~450 instructions, MLP: ~1100) close to full.
+// A warp round counts the pool by state, lists the slots of ONE state and runs that phase with (nearly) full warps:
+// retire (deferred MLP + stores, full batches of 32), sample, traversal visit, or refill with the next 8x4 pixel tile
+// from a global atomic counter.  Inside a traversal visit or a sample phase, lanes whose ray has left the state write
+// it back and take the next listed rays, so the warp stays full without a new census.  Rays have very different
+// lengths (about 4 samples on average, a long tail, many rays with none), so binding a ray to a lane for the whole
+// kernel leaves two thirds of the lanes idle (measured: 10.5 of 32 lanes active; the pool runs at 27).
 //
 //   S2 ray generation          fp32, one correctly rounded operation per step (bit-exact with the CPU checker)
 //   S3 box clip                fp32 slab test, padded by 2 lattice indices (the exact per-sample predicate decides)
@@ -16,11 +16,13 @@
 //                              z-interval; every jump is VERIFIED with the exact lattice
 //                              arithmetic, so skipping never changes which samples exist
 //   S5 gather                  trilinear grid + 3 bilinear planes, uint8 x 8 channels per 8-byte load,
-//                              8-bit fixed-point weights, exact integer sums (Eq. 2, R9)
-//   S6 activations             exp (exp_q on the decision path), sigmoid (Eq. 3)
+//                              8-bit fixed-point weights, exact integer sums as IDP.2A dot products (Eq. 2, R9)
+//   S6 activations             exp (exp_q on the decision path), sigmoid through MUFU.TANH (Eq. 3)
 //   S7 compositing             front to back, integer optical depth decides termination (Eq. 1/8, R7/R8)
-//   S8 deferred MLP            34 -> 16 -> 16 -> 3 in FFMA, weights read from the constant bank (Eq. 4)
+//   S8 deferred MLP            34 -> 16 -> 16 -> 3 as 3xTF32 tensor-core tiles, 16 rays at a time (Eq. 4; omerf_mlp.cuh)
 //   S9 outputs                 rgb fp32 + per-pixel sample count (Fig. 1)
+// plus the gather calibration of SURVEY 8(d) (sample log + omerf_gather_probe_kernel) and, in the GENERAL
+// instantiation, the 8(f) variants (soft occupancy of Eq. 6-8, sparse-block grid).
 //
 // Why jumps are exact: the lattice point p_k = fma(t_k, d, o) is monotone
 // in k in every component (rounding is monotone), so cell indices and z are monotone in k.  If samples k
@@ -53,16 +55,6 @@ enum : int { ST_IDLE = 0, ST_TRAV = 1, ST_READY = 2, ST_FIN = 3 };
 #endif
 
 
-// scheduling thresholds (lanes): tuned on B200 with configs[1]
-#ifndef OMERF_RETIRE_T
-#define OMERF_RETIRE_T 12
-#endif
-#ifndef OMERF_REFILL_T
-#define OMERF_REFILL_T 8
-#endif
-#ifndef OMERF_SAMPLE_T
-#define OMERF_SAMPLE_T 20
-#endif
 
 struct Ray {
     float ox, oy, oz, dx, dy, dz;
@@ -691,9 +683,6 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
         }
         __syncwarp();
         const int n_act = min(n_sel, 32);
-#ifdef OMERF_X_STATS
-        if (lane == 0) { atomicAdd(tile_counter + 1 + phase, 1u); atomicAdd(tile_counter + 5 + phase, (unsigned)n_act); }
-#endif
         const bool active = lane < n_act;
         const int slot = active ? (int)P.list[lane] : 0;
 
@@ -778,9 +767,6 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             int next = n_act; // first list entry not yet taken
 #pragma unroll 1
             while (true) {
-#ifdef OMERF_X_STATS
-                { unsigned m = __ballot_sync(FULL, status == ST_READY); if (lane == 0) { atomicAdd(tile_counter + 11, 1u); atomicAdd(tile_counter + 12, (unsigned)__popc(m)); } }
-#endif
                 if (status == ST_READY) {
                     float px, py, pz;
                     lattice_point(r, sc.step, k, px, py, pz);
@@ -992,22 +978,7 @@ int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_
         cudaMemsetAsync(s->d_tile_counter + 64, 0, 8 * 8 * 8192, st);
     }
 #endif
-#ifdef OMERF_X_STATS
-    {
-        static int calls = 0;
-        if (calls++ == 8) {
-            unsigned h[16];
-            cudaMemcpy(h, s->d_tile_counter, sizeof h, cudaMemcpyDeviceToHost);
-            const char *nm[4] = {"refill", "trav", "sample", "mlp"};
-            for (int i = 0; i < 4; i++) printf("STATS %s rounds %u avg lanes %.1f\n", nm[i], h[1 + i], h[5 + i] / (double)(h[1 + i] ? h[1 + i] : 1));
-            printf("STATS trav steps(warp) %u avg lanes %.1f thread-steps %u\n", h[9], h[10] / (double)(h[9] ? h[9] : 1), h[10]);
-            printf("STATS sample iters(warp) %u avg lanes %.1f thread-samples %u\n", h[11], h[12] / (double)(h[11] ? h[11] : 1), h[12]);
-        }
-    }
-    OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, 64 * sizeof(unsigned int), st));
-#else
     OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, (sample_log ? 64 : 1) * sizeof(unsigned int), st));
-#endif
     const int grid = s->persistent_blocks;
     const bool general = s->dev.soft_eps > 0.0f || s->dev.blk_shift != 0;
 #define OMERF_LAUNCH(SAMPLER, LOG, GENERAL)                                                                                 \
