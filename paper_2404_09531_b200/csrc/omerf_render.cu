@@ -509,14 +509,32 @@ __device__ __forceinline__ uint32_t pack_meta(int status, int lvl, uint32_t view
 // lanes write it back and take the next listed rays, so the warp stays full without a new census of the pool.  The
 // visit ends when the list is exhausted and fewer than OMERF_TRAV_KEEP lanes still traverse, or after
 // OMERF_TRAV_STEPS steps (occupied rays then get their samples).
+// per-lane cache of the camera origin of the view last used (rays of one lane almost always share the view)
+struct OriginCache {
+    uint32_t view;
+    float ox, oy, oz;
+};
+__device__ __forceinline__ void ray_origin(OriginCache &oc, const omerf_camera *__restrict__ cams, uint32_t view, Ray &r)
+{
+    if (view != oc.view) {
+        oc.view = view;
+        oc.ox = __ldg(&cams[view].origin[0]);
+        oc.oy = __ldg(&cams[view].origin[1]);
+        oc.oz = __ldg(&cams[view].origin[2]);
+    }
+    r.ox = oc.ox;
+    r.oy = oc.oy;
+    r.oz = oc.oz;
+}
+
 struct TravLane {
     Ray r;
     int k, k1, lvl, status, slot; // slot < 0: the lane holds no ray
     uint32_t view;
 };
 
-__device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P, const omerf_camera *__restrict__ cams, int slot,
-                                          TravLane &L)
+__device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P, const omerf_camera *__restrict__ cams,
+                                          OriginCache &oc, int slot, TravLane &L)
 {
     L.slot = slot;
     const int s_ = slot < 0 ? 0 : slot; // idle lanes read slot 0 and step nothing
@@ -529,9 +547,7 @@ __device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P,
     L.r.dx = P.dx[s_];
     L.r.dy = P.dy[s_];
     L.r.dz = P.dz[s_];
-    L.r.ox = __ldg(&cams[L.view].origin[0]);
-    L.r.oy = __ldg(&cams[L.view].origin[1]);
-    L.r.oz = __ldg(&cams[L.view].origin[2]);
+    ray_origin(oc, cams, L.view, L.r);
     L.r.ix = L.r.dx != 0.0f ? __fdividef(1.0f, L.r.dx) : INFINITY;
     L.r.iy = L.r.dy != 0.0f ? __fdividef(1.0f, L.r.dy) : INFINITY;
     L.r.iz = L.r.dz != 0.0f ? __fdividef(1.0f, L.r.dz) : INFINITY;
@@ -555,13 +571,13 @@ __device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, cons
 }
 
 template <int SAMPLER>
-__device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, const omerf_camera *__restrict__ cams, int lane,
-                                           int n_sel, int keep, float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
+__device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, const omerf_camera *__restrict__ cams,
+                                           OriginCache &oc, int lane, int n_sel, int keep, float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
 {
     const unsigned FULL = 0xffffffffu;
     const unsigned lt_mask = (1u << lane) - 1u;
     TravLane L;
-    trav_load(sc, P, cams, lane < n_sel ? (int)P.list[lane] : -1, L);
+    trav_load(sc, P, cams, oc, lane < n_sel ? (int)P.list[lane] : -1, L);
     int next = min(n_sel, 32); // first list entry not yet taken
 #pragma unroll 1
     for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
@@ -579,7 +595,7 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
                 if (free_lane) {
                     if (L.slot >= 0) trav_store(sc, P, L, out_rgb, out_n);
                     const int idx = next + __popc(fm & lt_mask);
-                    trav_load(sc, P, cams, idx < n_sel ? (int)P.list[idx] : -1, L);
+                    trav_load(sc, P, cams, oc, idx < n_sel ? (int)P.list[idx] : -1, L);
                 }
                 next = min(next + __popc(fm), n_sel);
             }
@@ -620,6 +636,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
     if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8 + 0] = t; }
 #endif
     bool more = true;
+    OriginCache oc = {0xffffffffu, 0.0f, 0.0f, 0.0f};
     // Endgame: a warp's pool holds about three tiles of work, which would all drain at falling utilisation once the
     // tile counter runs out.  For the last tiles, warps refill only when (nearly) empty, so the remaining work
     // spreads over all warps and they finish together.
@@ -729,7 +746,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
         } else if (phase == ST_TRAV) {
             // ---- traversal visit (S4).  (Two rays per lane, interleaved dependency chains, was measured slower on
             // B200 at every threshold: 0.80-0.86 ms against 0.76 ms per configs[1] frame.)
-            trav_visit<SAMPLER>(sc, P, cams, lane, n_sel, (more && !endgame) ? OMERF_TRAV_KEEP : OMERF_DRAIN_TRAV_KEEP, out_rgb, out_n);
+            trav_visit<SAMPLER>(sc, P, cams, oc, lane, n_sel, (more && !endgame) ? OMERF_TRAV_KEEP : OMERF_DRAIN_TRAV_KEEP, out_rgb, out_n);
         } else if (phase == ST_READY) {
             // ---- samples: gather, activations, compositing (S5, S6, S7) for the rays listed in P.list[0 .. n_sel);
             // lanes whose ray left the READY state take the next listed rays, OMERF_SAMPLE_SWAP lanes at a time
@@ -749,9 +766,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                 r.dx = P.dx[s_];
                 r.dy = P.dy[s_];
                 r.dz = P.dz[s_];
-                r.ox = __ldg(&cams[view].origin[0]);
-                r.oy = __ldg(&cams[view].origin[1]);
-                r.oz = __ldg(&cams[view].origin[2]);
+                ray_origin(oc, cams, view, r);
 #pragma unroll
                 for (int c = 0; c < 7; c++) acc[c] = P.acc[c][s_];
             };
