@@ -334,3 +334,24 @@ def test_sparse_block_grid_config0_and_rejections(omerf, oracle):
     with omerf.scene_create(sc) as h:
         with pytest.raises(omerf.OmerfError):
             omerf.block_table(h)
+
+
+def test_gather_probe_on_grid_sampler_and_sparse_soft_combination(omerf, oracle):
+    """The calibration probe follows whatever sampler / layout the scene uses; soft mask + sparse blocks combine."""
+    import torch
+    rng = np.random.default_rng(33)
+    m = 33
+    lo = (1.0 + 0.5 * rng.random((m, m))).astype(np.float32)
+    hi = (lo + 0.3 + 1.5 * rng.random((m, m))).astype(np.float32)
+    sc = synth.custom_scene(box=(16.0, 16.0, 4.0), hf_n=(m, m), h_lo=lo, h_up=hi, grid_n=(16, 16, 8), step=0.125,
+                            occ_n=(64, 64, 32), seed=2)
+    cams = np.stack([synth.look_at_camera((8.0, -10.0, 14.0), (8.0, 8.0, 2.0), 64, 48)])
+    with omerf.scene_create(sc, sampler=1) as h:
+        _, ns = omerf.render(h, cams, 64, 48)
+        torch.cuda.synchronize()
+        assert omerf.gather_probe(h, cams[0], 64, 48, repeats=1, flush_l2=False)["samples"] == int(ns.sum().item())
+    with omerf.scene_create(sc, soft_eps=0.4, grid_block=4) as h:
+        rgb, ns = omerf.render(h, cams, 64, 48)
+        torch.cuda.synchronize()
+    ref = oracle.OracleScene(sc, soft_eps=0.4).render(cams, 64, 48, mode="brute")
+    _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, "soft mask + sparse blocks")
