@@ -80,6 +80,12 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         if (d->grid_n[i] < 1) return invalid("grid_n must be >= 1");
     for (int i = 0; i < 2; i++)
         if (d->xy_n[i] < 1 || d->xz_n[i] < 1 || d->yz_n[i] < 1) return invalid("plane sizes must be >= 1");
+    // the gather takes index and weight of a tap from one conversion, exact for fewer than 2^15 texels per axis
+    {
+        const int32_t dims[] = {d->grid_n[0], d->grid_n[1], d->grid_n[2], d->xy_n[0], d->xy_n[1], d->xz_n[0], d->xz_n[1], d->yz_n[0], d->yz_n[1]};
+        for (int32_t n : dims)
+            if (n > (1 << 15)) return invalid("a feature array has more than 32768 texels along an axis");
+    }
     // the gather addresses texels with 32-bit indices
     if ((unsigned long long)d->grid_n[0] * d->grid_n[1] * d->grid_n[2] > 0xffffffffull ||
         (unsigned long long)d->xy_n[0] * d->xy_n[1] > 0xffffffffull || (unsigned long long)d->xz_n[0] * d->xz_n[1] > 0xffffffffull ||

@@ -61,12 +61,6 @@ struct Ray {
     float ix, iy, iz; // reciprocals of d (INF where d == 0), proposals only
 };
 
-__device__ __forceinline__ int floor_int(float x, float &fl)
-{
-    const int i = __float2int_rd(x);
-    fl = __int2float_rn(i);
-    return i;
-}
 __device__ __forceinline__ int floor_int(float x) { return __float2int_rd(x); }
 __device__ __forceinline__ int ceil_int(float x) { return __float2int_ru(x); } // saturates: +inf -> INT_MAX
 
@@ -214,35 +208,29 @@ __device__ __forceinline__ int trav_step_grid(const DevScene &sc, const Ray &r, 
 }
 
 // ---------------------------------------------------------------------------------- S5: gather (Eq. 2)
+// One axis of a bilinear footprint (R9/R10): texel coordinate q = p N/X - 1/2, lower texel floor(q), 8-bit weight
+// floor(frac * 256 + 1/2) in [0,256].  Both come out of ONE conversion: F = floor(fma(q, 256, 1/2)) = 256 floor(q) + w
+// exactly (256 q is exact and, for q < 2^15, so is the sum up to a rounding that cannot cross an integer), so
+// i = F >> 8 and w = F & 255.  A weight of 256 appears as (i + 1, 0): the same texels with the same total weights.
+// The point is inside the box (checked before every sample), hence -1 <= i <= N-1 and one clamp per tap suffices.
 __device__ __forceinline__ void axis_tap(float p, float s, int N, int &i0, int &i1, uint32_t &w)
 {
     const float q = __fmaf_rn(p, s, -0.5f);
-    float fl;
-    const int i = floor_int(q, fl);
-    // (q - floor q) * 256 is exact, so one fma rounds exactly like the mul followed by the add
-    w = (uint32_t)floor_int(__fmaf_rn(__fsub_rn(q, fl), 256.0f, 0.5f));
-    // the point is inside the box (checked before every sample), so -1 <= i <= N-1: one clamp per tap suffices
+    const int F = floor_int(__fmaf_rn(q, 256.0f, 0.5f));
+    const int i = F >> 8;
+    w = (uint32_t)(F & 255);
     i0 = max(i, 0);
     i1 = min(i + 1, N - 1);
 }
 
 // Bilinear footprints as 16-bit x 8-bit dot products (IDP.2A, fma pipe, full rate): the four weights
 // w_ab = (256 - w_a | w_a)(256 - w_b | w_b) are packed as two u16 pairs, the texel bytes of one channel of two
-// texels are brought side by side with one PRMT per two channels.  Only w_00 can reach 2^16 (w_a = w_b = 0, after
-// weight 256 has been folded into the neighbour index); then tap b1 is redirected to b0 and one unit of w_00 moves
+// texels are brought side by side with one PRMT per two channels.  Only w_00 can reach 2^16 (w_a = w_b = 0; the taps never
+// carry a weight of 256, see axis_tap); then tap b1 is redirected to b0 and one unit of w_00 moves
 // to w_01, which multiplies the same texel: the sum stays the exact integer of R9.
 struct BiW {
     uint32_t w0, w1; // (w00 | w01 << 16), (w10 | w11 << 16): pairs along axis b for rows a0 and a1
 };
-
-// fold weight 256 into the index (w in [0,255] afterwards)
-__device__ __forceinline__ void fold_tap(int &i0, int i1, uint32_t &w)
-{
-    if (w == 256u) {
-        i0 = i1;
-        w = 0u;
-    }
-}
 
 __device__ __forceinline__ BiW bilinear_weights(uint32_t wa, uint32_t wb, int b0, int &b1)
 {
@@ -331,8 +319,6 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
     axis_tap(px, sc.gs[0], sc.G[0], x0, x1, wx);
     axis_tap(py, sc.gs[1], sc.G[1], y0, y1, wy);
     axis_tap(pz, sc.gs[2], sc.G[2], z0, z1, wz);
-    fold_tap(x0, x1, wx);
-    fold_tap(y0, y1, wy);
     const BiW wg = bilinear_weights(wx, wy, y0, y1);
     uint2 ga[4], gb[4];
     {
@@ -354,18 +340,12 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
     axis_tap(px, sc.xy_s[0], sc.xy_n[0], xa0, xa1, xw);
     axis_tap(py, sc.xy_s[1], sc.xy_n[1], ya0, ya1, yw);
     axis_tap(pz, sc.xz_s[1], sc.xz_n[1], za0, za1, zw);
-    fold_tap(xa0, xa1, xw);
-    fold_tap(ya0, ya1, yw);
-    fold_tap(za0, za1, zw);
     int xb0 = xa0, xb1 = xa1, yb0 = ya0, yb1 = ya1, zb0 = za0, zb1 = za1; // taps of xz axis 0, yz axis 0, yz axis 1
     uint32_t xbw = xw, ybw = yw, zbw = zw;
     if (!sc.shared_taps) {
         axis_tap(px, sc.xz_s[0], sc.xz_n[0], xb0, xb1, xbw);
         axis_tap(py, sc.yz_s[0], sc.yz_n[0], yb0, yb1, ybw);
         axis_tap(pz, sc.yz_s[1], sc.yz_n[1], zb0, zb1, zbw);
-        fold_tap(xb0, xb1, xbw);
-        fold_tap(yb0, yb1, ybw);
-        fold_tap(zb0, zb1, zbw);
     }
     int b1;
     b1 = ya1;
