@@ -50,6 +50,12 @@ enum : int { ST_IDLE = 0, ST_TRAV = 1, ST_READY = 2, ST_FIN = 3 };
 #ifndef OMERF_LVL_FAIL
 #define OMERF_LVL_FAIL 2       // levels to descend when the proposed jump could not be verified
 #endif
+#ifndef OMERF_GRID_LVL_INSIDE
+#define OMERF_GRID_LVL_INSIDE 1 // config-4 comparator (occupancy mip chain): levels to descend in an occupied node
+#endif
+#ifndef OMERF_GRID_LVL_FAIL
+#define OMERF_GRID_LVL_FAIL 2   // ... and after a proposal that could not be verified
+#endif
 #ifndef OMERF_LVL_UP
 #define OMERF_LVL_UP 1         // levels to ascend after a verified jump across an xy node boundary
 #endif
@@ -167,44 +173,37 @@ __device__ __forceinline__ bool occ_test(const DevScene &sc, int lvl, int jx, in
 }
 
 // sampler GRID (config-4 comparator): multi-resolution binary occupancy grid, DDA-style skipping.
-__device__ __forceinline__ int trav_step_grid(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl)
+__device__ __forceinline__ int trav_step_grid(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl, int status)
 {
-    if (k > k1) return ST_FIN;
+    // same shape as trav_step_plane: branch-free, status other than ST_TRAV passes through
+    const bool run = status == ST_TRAV && k <= k1;
     float px, py, pz;
     lattice_point(r, sc.step, k, px, py, pz);
-    if (!in_box(sc, px, py, pz)) {
-        k++;
-        return ST_TRAV;
-    }
+    const bool inb = in_box(sc, px, py, pz); // the 2-index padding outside the box is walked one index at a time
     const int top = sc.occ_levels - 1;
     const int nx = voxel_index(px, sc.ns[0], sc.N[0]) >> lvl, ny = voxel_index(py, sc.ns[1], sc.N[1]) >> lvl,
               nz = voxel_index(pz, sc.ns[2], sc.N[2]) >> lvl;
-    if (occ_test(sc, lvl, nx, ny, nz)) {
-        if (lvl == 0) return ST_READY;
-        lvl--;
-        return ST_TRAV;
-    }
+    const bool occ = occ_test(sc, lvl, nx, ny, nz);
     const int bxi = nx + (r.dx > 0.0f ? 1 : 0), byi = ny + (r.dy > 0.0f ? 1 : 0), bzi = nz + (r.dz > 0.0f ? 1 : 0);
     const float tx = r.dx != 0.0f ? ((float)(bxi << lvl) * sc.vox[0] - r.ox) * r.ix : INFINITY;
     const float ty = r.dy != 0.0f ? ((float)(byi << lvl) * sc.vox[1] - r.oy) * r.iy : INFINITY;
     const float tz = r.dz != 0.0f ? ((float)(bzi << lvl) * sc.vox[2] - r.oz) * r.iz : INFINITY;
-    const float t_end = fminf(fminf(tx, ty), tz);
-    const int kk = index_before(t_end, sc.inv_step, k1);
-    if (kk > k) {
-        float qx, qy, qz;
-        lattice_point(r, sc.step, kk, qx, qy, qz);
-        if ((voxel_index(qx, sc.ns[0], sc.N[0]) >> lvl) == nx && (voxel_index(qy, sc.ns[1], sc.N[1]) >> lvl) == ny &&
-            (voxel_index(qz, sc.ns[2], sc.N[2]) >> lvl) == nz) {
-            k = kk + 1;
-            const int crossed = (tx <= ty && tx <= tz) ? bxi : (ty <= tz ? byi : bzi);
-            const int up = crossed == 0 ? 31 : __ffs(crossed) - 1;
-            lvl = min(lvl + min(up, 2), top);
-            return ST_TRAV;
-        }
+    const int kk = index_before(fminf(fminf(tx, ty), tz), sc.inv_step, k1);
+    float qx, qy, qz;
+    lattice_point(r, sc.step, kk, qx, qy, qz);
+    const bool same = (voxel_index(qx, sc.ns[0], sc.N[0]) >> lvl) == nx && (voxel_index(qy, sc.ns[1], sc.N[1]) >> lvl) == ny &&
+                      (voxel_index(qz, sc.ns[2], sc.N[2]) >> lvl) == nz;
+    const bool jump = inb && !occ && kk > k && same;
+    const bool ready = run && inb && occ && lvl == 0;
+    const int crossed = (tx <= ty && tx <= tz) ? bxi : (ty <= tz ? byi : bzi);
+    const int up = crossed == 0 ? 2 : min(__ffs(crossed) - 1, 2); // leaving 2^up-aligned parents: ascend that far
+    const int lvl_next = !inb ? lvl : (occ ? max(lvl - OMERF_GRID_LVL_INSIDE, 0) : (jump ? min(lvl + up, top) : max(lvl - OMERF_GRID_LVL_FAIL, 0)));
+    const int k_next = !inb ? k + 1 : (jump ? kk + 1 : ((lvl == 0 && !ready) ? k + 1 : k));
+    if (run) {
+        k = k_next;
+        lvl = lvl_next;
     }
-    if (lvl > 0) lvl--;
-    else k++;
-    return ST_TRAV;
+    return status != ST_TRAV ? status : (k > k1 && !ready ? ST_FIN : (ready ? ST_READY : ST_TRAV));
 }
 
 // ---------------------------------------------------------------------------------- S5: gather (Eq. 2)
@@ -564,7 +563,7 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
         if (SAMPLER == OMERF_SAMPLER_PLANE) {
             L.status = trav_step_plane(sc, L.r, L.k, L.k1, L.lvl, L.status);
         } else {
-            if (L.status == ST_TRAV) L.status = trav_step_grid(sc, L.r, L.k, L.k1, L.lvl);
+            L.status = trav_step_grid(sc, L.r, L.k, L.k1, L.lvl, L.status);
         }
         const unsigned going = __ballot_sync(FULL, L.status == ST_TRAV);
         if (next < n_sel) {
