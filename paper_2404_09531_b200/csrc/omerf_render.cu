@@ -6,7 +6,7 @@
 // retire (deferred MLP + stores, full batches of 32), sample, traversal visit, or refill with the next 8x4 pixel tile
 // from a global atomic counter.  Inside a traversal visit or a sample phase, lanes whose ray has left the state write
 // it back and take the next listed rays, so the warp stays full without a new census.  Rays have very different
-// lengths (about 4 samples on average, a long tail, many rays with none), so binding a ray to a lane for the whole
+// lengths (about 4 samples on average, a long tail, some rays with none), so binding a ray to a lane for the whole
 // kernel leaves two thirds of the lanes idle (measured: 10.5 of 32 lanes active; the pool runs at 27).
 //
 //   S2 ray generation          fp32, one correctly rounded operation per step (bit-exact with the CPU checker)
