@@ -9,9 +9,14 @@
 
 namespace {
 
+#ifndef SMOOTH_WARPS
 #define SMOOTH_WARPS 4
+#endif
 
-__global__ void __launch_bounds__(32 * SMOOTH_WARPS)
+#ifndef SMOOTH_MIN_BLOCKS
+#define SMOOTH_MIN_BLOCKS 5
+#endif
+__global__ void __launch_bounds__(32 * SMOOTH_WARPS, SMOOTH_MIN_BLOCKS)
 omerf_smooth_kernel(const float2 *__restrict__ mlp_tab, long long n, int S, const float *__restrict__ F,
                     const float *__restrict__ dir, const float *__restrict__ delta, float *__restrict__ out_loss,
                     float *__restrict__ out_G)
@@ -25,11 +30,34 @@ omerf_smooth_kernel(const float2 *__restrict__ mlp_tab, long long n, int S, cons
     const int rows_total = S + 1, passes = (rows_total + 31) / 32;
     const int g = lane >> 2, t = lane & 3;
 
+    // inputs of the first pass are fetched one direction ahead, so their DRAM latency overlaps the previous tiles
+    struct In {
+        float f7[7], dx, dy, dz, lx, ly, lz;
+    };
+    auto fetch = [&](long long i, In &q) {
+        if (i >= n) return;
+#pragma unroll
+        for (int c = 0; c < 7; c++) q.f7[c] = __ldg(F + i * 7 + c);
+        q.dx = __ldg(dir + i * 3 + 0);
+        q.dy = __ldg(dir + i * 3 + 1);
+        q.dz = __ldg(dir + i * 3 + 2);
+        q.lx = q.ly = q.lz = 0.0f;
+        if (lane > 0 && lane < rows_total) {
+            const float *dl = delta + (i * S + (lane - 1)) * 3;
+            q.lx = __ldg(dl + 0);
+            q.ly = __ldg(dl + 1);
+            q.lz = __ldg(dl + 2);
+        }
+    };
+    In cur, nxt;
+    fetch((long long)blockIdx.x * SMOOTH_WARPS + w, nxt);
     for (long long i = (long long)blockIdx.x * SMOOTH_WARPS + w; i < n; i += warps) {
+        cur = nxt;
+        fetch(i + warps, nxt);
         float f7[7];
 #pragma unroll
-        for (int c = 0; c < 7; c++) f7[c] = __ldg(F + i * 7 + c);
-        const float dx = __ldg(dir + i * 3 + 0), dy = __ldg(dir + i * 3 + 1), dz = __ldg(dir + i * 3 + 2);
+        for (int c = 0; c < 7; c++) f7[c] = cur.f7[c];
+        const float dx = cur.dx, dy = cur.dy, dz = cur.dz;
         float G0[3] = {0.f, 0.f, 0.f};
         float loss = 0.0f;
         for (int p = 0; p < passes; p++) {
@@ -42,10 +70,16 @@ omerf_smooth_kernel(const float2 *__restrict__ mlp_tab, long long n, int S, cons
             if (j < rows_total) {
                 float sx = dx, sy = dy, sz = dz;
                 if (j > 0) {
-                    const float *dl = delta + (i * S + (j - 1)) * 3;
-                    sx = __fadd_rn(dx, __ldg(dl + 0));
-                    sy = __fadd_rn(dy, __ldg(dl + 1));
-                    sz = __fadd_rn(dz, __ldg(dl + 2));
+                    float lx = cur.lx, ly = cur.ly, lz = cur.lz;
+                    if (p > 0) {
+                        const float *dl = delta + (i * S + (j - 1)) * 3;
+                        lx = __ldg(dl + 0);
+                        ly = __ldg(dl + 1);
+                        lz = __ldg(dl + 2);
+                    }
+                    sx = __fadd_rn(dx, lx);
+                    sy = __fadd_rn(dy, ly);
+                    sz = __fadd_rn(dz, lz);
                     const float dot = dx * sx + dy * sy + dz * sz;
                     const float nn = (dx * dx + dy * dy + dz * dz) * (sx * sx + sy * sy + sz * sz);
                     cosv = nn > 0.0f ? dot * rsqrtf(nn) : 0.0f;
@@ -117,7 +151,9 @@ int omerf_launch_smoothness(const omerf_scene *s, long long n, int S, const floa
     OMERF_CUDA(cudaGetDevice(&dev));
     OMERF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     long long blocks = (n + SMOOTH_WARPS - 1) / SMOOTH_WARPS;
-    const long long cap = (long long)sms * 8; // persistent-style grid: a multiple of the SM count
+    int per_sm = 0;
+    OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_smooth_kernel, 32 * SMOOTH_WARPS, 0));
+    const long long cap = (long long)sms * (per_sm > 0 ? per_sm : 1); // persistent grid: one wave of resident CTAs
     if (blocks > cap) blocks = cap;
     omerf_smooth_kernel<<<(unsigned int)blocks, 32 * SMOOTH_WARPS, 0, st>>>(s->dev.mlp_tab, n, S, F, dir, delta, out_loss, out_G);
     OMERF_CUDA(cudaGetLastError());
