@@ -355,3 +355,24 @@ def test_gather_probe_on_grid_sampler_and_sparse_soft_combination(omerf, oracle)
         torch.cuda.synchronize()
     ref = oracle.OracleScene(sc, soft_eps=0.4).render(cams, 64, 48, mode="brute")
     _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, "soft mask + sparse blocks")
+
+
+def test_more_views_than_the_initial_camera_ring_and_repeated_calls(omerf, oracle):
+    """40 views (the camera staging ring starts at 16 per slot and must grow), then 20 calls back to back (more calls
+    than ring slots), then fewer views again."""
+    import torch
+    sc = synth.make_scene(0)
+    W, H = 24, 16
+    cams = np.stack([synth.look_at_camera((32.0 + 28 * np.cos(a), 32.0 + 28 * np.sin(a), 20.0 + 0.5 * i), (32.0, 32.0, 8.0), W, H)
+                     for i, a in enumerate(np.linspace(0, 6, 40))])
+    ref = oracle.OracleScene(sc).render(cams, W, H, mode="clipped")
+    with omerf.scene_create(sc) as h:
+        rgb, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, "40 views")
+        outs = [omerf.render(h, cams[i:i + 2], W, H) for i in range(20)]
+        torch.cuda.synchronize()
+        for i, (r2, n2) in enumerate(outs):
+            assert np.array_equal(n2.cpu().numpy().view(np.uint32), ref["nsamples"][i:i + 2])
+        h_rgb, h_ns = omerf.render_host(h, cams[:3], W, H)
+        assert np.array_equal(h_ns, ref["nsamples"][:3])
