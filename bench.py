@@ -228,6 +228,20 @@ def run_ours(args):
     launches_per_step = omerf.last_launch_count(h)
     ms_warm = timed(args.steps, False, dev_step)                               # extra: L2-warm static camera
     barrier()
+    # extra (SURVEY 8(d) second regime): a yaw orbit, a new view every frame, no flush
+    ms_orbit = None
+    if n_views == 1 and cfg in (0, 1, 3, 4):
+        orbit = synth.orbit_cameras(cfg, 64)
+        it = iter(range(10 ** 9))
+
+        def orbit_step():
+            omerf.render(h, orbit[next(it) % 64:][:1], W, H, out_rgb, out_n, stream=stream)
+
+        for _ in range(3):
+            orbit_step()
+        ms_orbit = timed(max(args.steps, 64), False, orbit_step)
+        omerf.render(h, cams, W, H, out_rgb, out_n, stream=stream)              # restore the workload's own frame
+        barrier()
     clk = clocks.stop() if rank == 0 else None
     total_ms = float(np.sum(ms))
     samples = int(out_n.sum(dtype=torch.int64).item())
@@ -312,6 +326,9 @@ def run_ours(args):
             "samples_per_step": samples, "samples_per_ray": samples / pixels,
             "per_view_samples": per_view,
             "l2_warm": {"ms_per_step": total_warm_ms / k, "mpixels_s": world * pixels * k / (total_warm_ms / 1e3) / 1e6},
+            "orbit": ({"ms_per_step_median": float(np.median(ms_orbit)), "ms_per_step_mean": float(np.mean(ms_orbit)),
+                       "mpixels_s": pixels / (float(np.median(ms_orbit)) / 1e3) / 1e6, "views": 64} if ms_orbit else None),
+            "ms_per_step_median": float(np.median(ms)),
             "e2e": {"value": world * pixels * k / (total_e2e_ms / 1e3) / 1e6, "unit": "Mpixels/s",
                     "h2d_bytes_per_step": int(cams.nbytes), "d2h_bytes_per_step": pixels * BYTES_PER_PIXEL,
                     "ms_per_step": total_e2e_ms / k, "wall_ms_per_step": wall_e2e * 1e3 / k},
