@@ -95,7 +95,7 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_bounded(scene, cams, W, H, sampler=0, budget_s=15.0, soft_eps=0.0):
+def oracle_bounded(scene, cams, W, H, sampler=0, budget_s=15.0, soft_eps=0.0, count_sectors=False):
     """Time the oracle (clipped loop, OpenMP on all host cores) on every `stride`-th row of view 0."""
     import oracle
     O = oracle.OracleScene(scene, sampler=sampler, soft_eps=soft_eps)
@@ -120,8 +120,15 @@ def oracle_bounded(scene, cams, W, H, sampler=0, budget_s=15.0, soft_eps=0.0):
         threads = r["threads"]
     dt = time.perf_counter() - t0
     px = len(rows) * W
-    return {"mpix_s": px / dt / 1e6, "msamples_s": samples / dt / 1e6, "seconds": dt, "pixels": px, "samples": samples,
-            "cores": threads, "sample": f"{len(rows)} of {H} rows (every {stride}th) of view 0, clipped loop"}
+    out = {"mpix_s": px / dt / 1e6, "msamples_s": samples / dt / 1e6, "seconds": dt, "pixels": px, "samples": samples,
+           "cores": threads, "sample": f"{len(rows)} of {H} rows (every {stride}th) of view 0, clipped loop"}
+    if count_sectors and stride == 1:
+        # distinct 32-byte sectors the frame's samples touch (untimed second pass over the same rows)
+        with oracle.SectorMaps(O) as M:
+            O.render(cams[:1], W, H, mode="clipped")
+        out["compulsory_bytes"] = M.compulsory_bytes()
+        out["sectors"] = M.sectors()
+    return out
 
 
 def run_reference(args):
@@ -307,7 +314,7 @@ def run_ours(args):
         alu_ops = samples * OPS_PER_SAMPLE + pixels * OPS_PER_PIXEL
         cpu = None
         if not args.no_cpu_baseline:
-            cpu = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=15.0, soft_eps=args.soft_eps)
+            cpu = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=15.0, soft_eps=args.soft_eps, count_sectors=True)
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tpath):
@@ -357,6 +364,10 @@ def run_ours(args):
         if cpu is not None:
             line["cpu_baseline"] = {"value": cpu["mpix_s"], "unit": "Mpixels/s", "cores": cpu["cores"], "kind": "oracle",
                                     "sample": cpu["sample"], "msamples_s": cpu["msamples_s"], "seconds": cpu["seconds"]}
+            if "compulsory_bytes" in cpu:     # the HBM ceiling of SURVEY 8(d): bytes an unbounded cache would still fetch
+                line["gather_vs_hbm"]["compulsory_bytes_oracle"] = cpu["compulsory_bytes"]
+                line["gather_vs_hbm"]["compulsory_sectors_oracle"] = cpu["sectors"]
+                line["gather_vs_hbm"]["compulsory_ms_at_peak"] = cpu["compulsory_bytes"] / (hbm * 1e9) * 1e3
         print(json.dumps(line))
     omerf.scene_destroy(h)
     if world > 1:

@@ -267,3 +267,26 @@ def mlp_smoothness(O: OracleScene, F, d, delta, want_G: bool = False):
     lib().orc_mlp_smoothness(C.byref(O.c), C.c_int64(n), C.c_int(S), _ptr(F, _f32p), _ptr(d, _f32p), _ptr(delta, _f32p),
                              _ptr(loss, C.POINTER(C.c_double)), _ptr(G, C.POINTER(C.c_double)) if want_G else None)
     return (loss, G) if want_G else loss
+
+
+class SectorMaps:
+    """Distinct 32-byte sectors touched per feature source by the renders run inside the `with` block (SURVEY 8(d):
+    the compulsory-byte figure of the HBM roofline)."""
+
+    def __init__(self, O: OracleScene):
+        sc = O.scene
+        self.texels = [int(np.prod(a.shape[:-1])) for a in (sc.grid, sc.plane_xy, sc.plane_xz, sc.plane_yz)]
+        self.maps = [np.zeros(((t + 3) // 4 + 7) // 8, dtype=np.uint8) for t in self.texels]
+
+    def __enter__(self):
+        lib().orc_set_sector_maps(*[_ptr(m, _u8p) for m in self.maps])
+        return self
+
+    def __exit__(self, *exc):
+        lib().orc_set_sector_maps(None, None, None, None)
+
+    def sectors(self):
+        return dict(zip(("grid", "xy", "xz", "yz"), (int(np.unpackbits(m).sum()) for m in self.maps)))
+
+    def compulsory_bytes(self) -> int:
+        return 32 * sum(self.sectors().values())

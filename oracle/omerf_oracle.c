@@ -402,6 +402,53 @@ static void clipped_range(const orc_scene *s, const float o[3], const float d[3]
     *k1 = b;
 }
 
+/* ------------------------------------------------------------------ compulsory bytes */
+/* Distinct 32-byte sectors of the four feature arrays ([..][8] uint8, row-major as in the scene) touched by the samples
+ * of a render: the bytes a cache of unbounded size would still have to fetch once.  Bit maps (one bit per sector) are
+ * installed by orc_set_sector_maps and filled by the render loops; maps[0] = grid, 1 = xy, 2 = xz, 3 = yz. */
+static uint8_t *g_sector_map[4] = {0, 0, 0, 0};
+
+void orc_set_sector_maps(uint8_t *grid, uint8_t *xy, uint8_t *xz, uint8_t *yz)
+{
+    g_sector_map[0] = grid;
+    g_sector_map[1] = xy;
+    g_sector_map[2] = xz;
+    g_sector_map[3] = yz;
+}
+
+static inline void mark_texel(uint8_t *map, size_t texel)
+{
+    size_t sector = texel >> 2;                              /* 8-byte texels, 32-byte sectors */
+    uint8_t bit = (uint8_t)(1u << (sector & 7));
+    if (!(map[sector >> 3] & bit)) {
+#pragma omp atomic
+        map[sector >> 3] |= bit;
+    }
+}
+
+static void mark_sample_sectors(const orc_scene *s, const float p[3])
+{
+    int a0, a1, b0, b1, c0, c1;
+    uint32_t w;
+    axis_tap(p[0], s->grid_n[0], s->box[0], &a0, &a1, &w);
+    axis_tap(p[1], s->grid_n[1], s->box[1], &b0, &b1, &w);
+    axis_tap(p[2], s->grid_n[2], s->box[2], &c0, &c1, &w);
+    const int xs[2] = {a0, a1}, ys[2] = {b0, b1}, zs[2] = {c0, c1};
+    for (int i = 0; i < 2; i++)
+        for (int j = 0; j < 2; j++)
+            for (int k = 0; k < 2; k++)
+                mark_texel(g_sector_map[0], ((size_t)xs[i] * s->grid_n[1] + ys[j]) * s->grid_n[2] + zs[k]);
+    const int32_t *pn[3] = {s->xy_n, s->xz_n, s->yz_n};
+    const int ax[3][2] = {{0, 1}, {0, 2}, {1, 2}};
+    for (int q = 0; q < 3; q++) {
+        axis_tap(p[ax[q][0]], pn[q][0], s->box[ax[q][0]], &a0, &a1, &w);
+        axis_tap(p[ax[q][1]], pn[q][1], s->box[ax[q][1]], &b0, &b1, &w);
+        const int as[2] = {a0, a1}, bs[2] = {b0, b1};
+        for (int i = 0; i < 2; i++)
+            for (int j = 0; j < 2; j++) mark_texel(g_sector_map[1 + q], (size_t)as[i] * pn[q][1] + bs[j]);
+    }
+}
+
 static void render_pixel(const orc_scene *s, const orc_camera *cam, int u, int v, int64_t K, int mode,
                          uint32_t q_stop, orc_pixel *out)
 {
@@ -422,6 +469,7 @@ static void render_pixel(const orc_scene *s, const orc_camera *cam, int u, int v
         int32_t I[8];
         float t[8];
         orc_features(s, p, I, t);                             /* Eq. 2 */
+        if (g_sector_map[0]) mark_sample_sectors(s, p);
         float tau = orc_exp_q(t[0]);                          /* Eq. 3, decision path */
         float od = tau * s->step;                             /* tau_i * delta_i, delta = step (R5) */
         uint32_t qk = (uint32_t)rintf(fminf(od * 1048576.0f, (float)q_stop));

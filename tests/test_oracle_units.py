@@ -239,3 +239,40 @@ def test_bitfield_vs_exact_rational_brute_force(hf_n, occ_n):
     n = int(np.prod(occ_n))
     bits = np.unpackbits(O.bits.view(np.uint8), bitorder="little")[:n].reshape(occ_n).astype(bool)
     assert np.array_equal(bits, _brute_bitfield(sc))
+
+
+def test_distinct_sector_count_matches_numpy_recount():
+    """SURVEY 8(d) compulsory-byte figure: distinct 32-byte sectors per source touched by a render, recounted in numpy
+    from the kept sample positions (thin density: no ray terminates, so every kept lattice point is a sample)."""
+    fill = [100, 128, 128, 128, 128, 128, 128, 128]
+    sc = synth.custom_scene(box=(8.0, 8.0, 4.0), hf_n=(9, 9), h_lo=1.0, h_up=3.0, grid_n=(12, 10, 8), xy_n=(40, 36),
+                            xz_n=(40, 16), yz_n=(36, 16), fill=fill, seed=2, step=0.2)
+    O = oracle.OracleScene(sc)
+    cam = synth.look_at_camera((4.0, -3.0, 7.0), (4.0, 4.0, 2.0), 20, 14)
+    with oracle.SectorMaps(O) as M:
+        r = O.render(cam, 20, 14, mode="brute")
+    want = {"grid": set(), "xy": set(), "xz": set(), "yz": set()}
+    total = 0
+    for v in range(14):
+        for u in range(20):
+            n, ks, pos = O.pixel_samples(cam, u, v)
+            assert n == r["nsamples"][0, v, u]
+            total += n
+            for p in pos.astype(np.float64):
+                def taps(x, N, X):
+                    i = int(np.floor(x * N / X - 0.5))
+                    return {min(max(i, 0), N - 1), min(max(i + 1, 0), N - 1)}
+                gx, gy, gz = taps(p[0], 12, 8.0), taps(p[1], 10, 8.0), taps(p[2], 8, 4.0)
+                want["grid"] |= {((x * 10 + y) * 8 + z) // 4 for x in gx for y in gy for z in gz}
+                want["xy"] |= {(a * 36 + b) // 4 for a in taps(p[0], 40, 8.0) for b in taps(p[1], 36, 8.0)}
+                want["xz"] |= {(a * 16 + b) // 4 for a in taps(p[0], 40, 8.0) for b in taps(p[2], 16, 4.0)}
+                want["yz"] |= {(a * 16 + b) // 4 for a in taps(p[1], 36, 8.0) for b in taps(p[2], 16, 4.0)}
+    got = M.sectors()
+    assert total > 1000
+    for k in want:      # float64 vs the oracle's fp32 taps may disagree on a point within an ulp of a texel boundary
+        assert abs(got[k] - len(want[k])) <= 2, (k, got[k], len(want[k]))
+    assert M.compulsory_bytes() == 32 * sum(got.values())
+    # nothing is recorded outside the with-block
+    before = M.sectors()
+    O.render(cam, 20, 14, mode="brute")
+    assert M.sectors() == before
