@@ -100,7 +100,8 @@ int omerf_render(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/,
                  float *out_rgb /*DEVICE*/, uint32_t *out_nsamples /*DEVICE*/, void *stream);
 
 /* Same path with HOST outputs (pinned or pageable): renders into scene-owned device scratch on
- * `stream`, copies both images back and synchronises the stream before returning. */
+ * `stream` in bands of whole tile rows, copies each band back on a scene-owned second stream while the next
+ * band renders, and synchronises both streams before returning. */
 int omerf_render_host(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W,
                       int H, float *out_rgb /*HOST*/, uint32_t *out_nsamples /*HOST*/, void *stream);
 

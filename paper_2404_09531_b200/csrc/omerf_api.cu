@@ -60,6 +60,11 @@ static void free_scene(omerf_scene *s)
     cudaFree(s->d_scratch_rgb);
     cudaFree(s->d_scratch_n);
     if (s->h_cams) cudaFreeHost(s->h_cams);
+    if (s->copy_stream) {
+        cudaStreamDestroy(s->copy_stream);
+        for (int i = 0; i < 16; i++)
+            if (s->band_event[i]) cudaEventDestroy(s->band_event[i]);
+    }
     if (s->slot_event) {
         for (int i = 0; i < OMERF_CAM_SLOTS; i++)
             if (s->slot_event[i]) cudaEventDestroy(s->slot_event[i]);
@@ -243,29 +248,42 @@ static int ensure_cams(const omerf_scene *s, int n_views)
     return OMERF_OK;
 }
 
-extern "C" int omerf_render(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
-                            float *out_rgb, uint32_t *out_nsamples, void *stream)
+// Stages the cameras and launches the march kernel for the tiles [tile_first, tile_end) of the batch (0, 0 = all).
+// *d_cams_io: device cameras of an earlier band of the same call (nullptr: stage them now).
+static int render_impl(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H, float *out_rgb,
+                       uint32_t *out_nsamples, void *stream, unsigned int tile_first, unsigned int tile_end,
+                       omerf_camera **d_cams_io)
 {
     if (!s || !cameras || !out_rgb || !out_nsamples) return invalid("null scene/cameras/output");
     if (n_views < 0 || W <= 0 || H <= 0) return invalid("n_views >= 0, W > 0, H > 0 required");
     if (((uintptr_t)out_rgb & 3) || ((uintptr_t)out_nsamples & 3)) return invalid("misaligned output");
-    s->last_launches = 0;
     if (n_views == 0) return OMERF_OK;
     cudaStream_t st = (cudaStream_t)stream;
     int rc = ensure_cams(s, n_views);
     if (rc) return rc;
-    // stage the cameras: user memory -> pinned ring slot -> device ring slot (stream-ordered)
-    int slot = (int)(s->call_index++ % OMERF_CAM_SLOTS);
-    OMERF_CUDA(cudaEventSynchronize(s->slot_event[slot]));
-    omerf_camera *h = s->h_cams + (size_t)slot * s->cam_capacity;
-    omerf_camera *dv = s->d_cams + (size_t)slot * s->cam_capacity;
-    memcpy(h, cameras, (size_t)n_views * sizeof(omerf_camera));
-    OMERF_CUDA(cudaMemcpyAsync(dv, h, (size_t)n_views * sizeof(omerf_camera), cudaMemcpyHostToDevice, st));
-    OMERF_CUDA(cudaEventRecord(s->slot_event[slot], st));
+    omerf_camera *dv = d_cams_io ? *d_cams_io : nullptr;
+    if (!dv) {
+        // stage the cameras: user memory -> pinned ring slot -> device ring slot (stream-ordered)
+        int slot = (int)(s->call_index++ % OMERF_CAM_SLOTS);
+        OMERF_CUDA(cudaEventSynchronize(s->slot_event[slot]));
+        omerf_camera *h = s->h_cams + (size_t)slot * s->cam_capacity;
+        dv = s->d_cams + (size_t)slot * s->cam_capacity;
+        memcpy(h, cameras, (size_t)n_views * sizeof(omerf_camera));
+        OMERF_CUDA(cudaMemcpyAsync(dv, h, (size_t)n_views * sizeof(omerf_camera), cudaMemcpyHostToDevice, st));
+        OMERF_CUDA(cudaEventRecord(s->slot_event[slot], st));
+        if (d_cams_io) *d_cams_io = dv;
+    }
     int launches = 0;
-    rc = omerf_launch_render(s, dv, n_views, W, H, out_rgb, out_nsamples, st, &launches);
-    s->last_launches = launches;
+    rc = omerf_launch_render(s, dv, n_views, W, H, out_rgb, out_nsamples, st, &launches, nullptr, 0, tile_first, tile_end);
+    s->last_launches += launches;
     return rc;
+}
+
+extern "C" int omerf_render(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
+                            float *out_rgb, uint32_t *out_nsamples, void *stream)
+{
+    if (s) s->last_launches = 0;
+    return render_impl(s, cameras, n_views, W, H, out_rgb, out_nsamples, stream, 0, 0, nullptr);
 }
 
 extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
@@ -287,10 +305,40 @@ extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *camer
         s->scratch_pixels = px;
     }
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = omerf_render(s, cameras, n_views, W, H, s->d_scratch_rgb, s->d_scratch_n, stream);
-    if (rc) return rc;
-    OMERF_CUDA(cudaMemcpyAsync(out_rgb, s->d_scratch_rgb, px * 3 * sizeof(float), cudaMemcpyDeviceToHost, st));
-    OMERF_CUDA(cudaMemcpyAsync(out_nsamples, s->d_scratch_n, px * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    // The batch is rendered in bands of whole tile rows (one launch each, stream-ordered); a band is copied back on a
+    // second stream while the next one renders.  Bands hold at least 10 MiB of output so that the fixed cost of a
+    // launch (about 0.08 ms on B200) stays small against the copy it hides (1080p: 3 bands, 1.02 ms against 1.23 ms).
+    if (!s->copy_stream) {
+        OMERF_CUDA(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 16; i++) OMERF_CUDA(cudaEventCreateWithFlags(&s->band_event[i], cudaEventDisableTiming));
+    }
+    const unsigned int tiles_x = (unsigned int)((W + 7) / 8), tiles_y = (unsigned int)((H + 3) / 4);
+    const uint64_t tile_rows = (uint64_t)n_views * tiles_y, out_bytes = px * 16;
+    int bands = (int)(out_bytes / ((uint64_t)10 << 20));
+    if (getenv("OMERF_HOST_BANDS")) bands = atoi(getenv("OMERF_HOST_BANDS")); // experiment knob
+    bands = bands < 1 ? 1 : (bands > 16 ? 16 : bands);
+    if ((uint64_t)bands > tile_rows) bands = (int)tile_rows;
+    auto pixel_row = [&](uint64_t R) { // first flattened pixel row (view * H + v) of flattened tile row R
+        const uint64_t view = R / tiles_y, ty = R % tiles_y;
+        const uint64_t v = ty * 4 < (uint64_t)H ? ty * 4 : (uint64_t)H;
+        return view * (uint64_t)H + v;
+    };
+    s->last_launches = 0;
+    omerf_camera *d_cams = nullptr;
+    for (int b = 0; b < bands; b++) {
+        const uint64_t R0 = tile_rows * b / bands, R1 = tile_rows * (b + 1) / bands;
+        int rc = render_impl(s, cameras, n_views, W, H, s->d_scratch_rgb, s->d_scratch_n, stream, (unsigned int)(R0 * tiles_x),
+                             (unsigned int)(R1 * tiles_x), &d_cams);
+        if (rc) return rc;
+        OMERF_CUDA(cudaEventRecord(s->band_event[b], st));
+        OMERF_CUDA(cudaStreamWaitEvent(s->copy_stream, s->band_event[b], 0));
+        const uint64_t r0 = pixel_row(R0), r1 = R1 == tile_rows ? (uint64_t)n_views * H : pixel_row(R1);
+        OMERF_CUDA(cudaMemcpyAsync(out_rgb + r0 * W * 3, s->d_scratch_rgb + r0 * W * 3, (r1 - r0) * W * 3 * sizeof(float),
+                                   cudaMemcpyDeviceToHost, s->copy_stream));
+        OMERF_CUDA(cudaMemcpyAsync(out_nsamples + r0 * W, s->d_scratch_n + r0 * W, (r1 - r0) * W * sizeof(uint32_t),
+                                   cudaMemcpyDeviceToHost, s->copy_stream));
+    }
+    OMERF_CUDA(cudaStreamSynchronize(s->copy_stream));
     OMERF_CUDA(cudaStreamSynchronize(st));
     return OMERF_OK;
 }

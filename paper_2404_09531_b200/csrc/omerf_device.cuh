@@ -72,6 +72,8 @@ struct omerf_scene {
     mutable uint32_t *d_scratch_n;
     mutable uint64_t scratch_pixels;
     mutable int last_launches;
+    mutable cudaStream_t copy_stream;  // omerf_render_host: copies a band back while the next one renders
+    mutable cudaEvent_t band_event[16];
     unsigned int *d_tile_counter;     // work queue head of the persistent march kernel
     int persistent_blocks;            // resident CTAs of the march kernel (SMs x occupancy)
 };
@@ -94,7 +96,7 @@ int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream
 int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_t st);
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H,
                         float *out_rgb, uint32_t *out_n, cudaStream_t st, int *launches, uint2 *sample_log = nullptr,
-                        unsigned int log_capacity = 0);
+                        unsigned int log_capacity = 0, unsigned int tile_first = 0, unsigned int tile_end = 0);
 int omerf_launch_gather_probe(const omerf_scene *s, const omerf_camera *d_cam, int W, const uint2 *sample_log,
                               unsigned int n, unsigned int mult, uint32_t *sink, cudaStream_t st);
 int omerf_query_persistent_blocks(int sampler, int *blocks);

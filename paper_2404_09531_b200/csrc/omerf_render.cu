@@ -595,7 +595,7 @@ template <int SAMPLER, bool LOG, bool GENERAL>
 __global__ void __launch_bounds__(32 * OMERF_WARPS, OMERF_MIN_BLOCKS)
 omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__restrict__ cams, int n_views, int W, int H,
                    float *__restrict__ out_rgb, uint32_t *__restrict__ out_n, unsigned int *__restrict__ tile_counter,
-                   uint2 *__restrict__ sample_log, unsigned int log_capacity)
+                   uint2 *__restrict__ sample_log, unsigned int log_capacity, unsigned int tile_first, unsigned int tile_end)
 {
     __shared__ WarpPool pools[OMERF_WARPS];
     WarpPool &P = pools[threadIdx.x >> 5];
@@ -604,7 +604,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
     const unsigned lt_mask = (1u << lane) - 1u;
     const int tiles_x = (W + 7) >> 3, tiles_y = (H + 3) >> 2;
     const unsigned tiles_per_view = (unsigned)tiles_x * tiles_y;
-    const unsigned total_tiles = tiles_per_view * (unsigned)n_views;
+    const unsigned total_tiles = tile_end; // this launch renders the tiles [tile_first, tile_end) of the batch
     const int start_lvl = min((SAMPLER == OMERF_SAMPLER_PLANE ? sc.n_levels : sc.occ_levels) - 1, OMERF_LVL_START);
 
 #pragma unroll
@@ -686,7 +686,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             // ---- refill: one 8x4 tile -> 32 new rays (S2, S3)
             unsigned t = 0;
             if (lane == 0) t = atomicAdd(tile_counter, 1u);
-            const unsigned tile = __shfl_sync(FULL, t, 0);
+            const unsigned tile = tile_first + __shfl_sync(FULL, t, 0);
             if (tile + endgame_tiles >= total_tiles) endgame = true;
             if (tile >= total_tiles) {
                 more = false;
@@ -935,7 +935,8 @@ int omerf_launch_gather_probe(const omerf_scene *s, const omerf_camera *d_cam, i
 }
 
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H, float *out_rgb,
-                        uint32_t *out_n, cudaStream_t st, int *launches, uint2 *sample_log, unsigned int log_capacity)
+                        uint32_t *out_n, cudaStream_t st, int *launches, uint2 *sample_log, unsigned int log_capacity,
+                        unsigned int tile_first, unsigned int tile_end)
 {
     if ((long long)((W + 7) / 8) * ((H + 3) / 4) * n_views > 0x7fffffffll || (long long)W * H * n_views > 0xffffffffll) {
         omerf_set_error("invalid argument: image or batch too large");
@@ -973,11 +974,17 @@ int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_
     }
 #endif
     OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, (sample_log ? 64 : 1) * sizeof(unsigned int), st));
+    const unsigned int all_tiles = (unsigned int)(((W + 7) / 8) * ((H + 3) / 4)) * (unsigned int)n_views;
+    if (tile_end == 0 || tile_end > all_tiles) tile_end = all_tiles; // 0: the whole batch
+    if (tile_first >= tile_end) {
+        *launches = 0;
+        return OMERF_OK;
+    }
     const int grid = s->persistent_blocks;
     const bool general = s->dev.soft_eps > 0.0f || s->dev.blk_shift != 0;
 #define OMERF_LAUNCH(SAMPLER, LOG, GENERAL)                                                                                 \
     omerf_march_kernel<SAMPLER, LOG, GENERAL><<<grid, 32 * OMERF_WARPS, 0, st>>>(                                          \
-        s->dev, d_cams, n_views, W, H, out_rgb, out_n, s->d_tile_counter, sample_log, log_capacity)
+        s->dev, d_cams, n_views, W, H, out_rgb, out_n, s->d_tile_counter, sample_log, log_capacity, tile_first, tile_end)
 #define OMERF_LAUNCH2(SAMPLER, LOG)                \
     if (general) OMERF_LAUNCH(SAMPLER, LOG, true); \
     else OMERF_LAUNCH(SAMPLER, LOG, false)

@@ -125,3 +125,20 @@ def test_config1_sparse_block_grid(omerf, city):
     ref = oracle.OracleScene(city).render_pixels(cams, W, H, vuv, mode="clipped")
     assert np.array_equal(ns[vuv[:, 0], vuv[:, 2], vuv[:, 1]], ref["nsamples"])
     assert np.abs(rgb[vuv[:, 0], vuv[:, 2], vuv[:, 1]].astype(np.float64) - ref["rgb"]).max() <= RGB_TOL
+
+
+def test_render_host_banded_copy_is_bit_identical(omerf, city):
+    """omerf_render_host renders in bands and copies a band back while the next one renders: the host images must
+    equal the device-output path bit for bit, for one view (2 bands), several views and a ragged image height."""
+    import torch
+    cams = synth.make_cameras(2)[:3]
+    W, H = synth.config_resolution(2)
+    with omerf.scene_create(city) as h:
+        for n_views, w_, h_ in ((3, W, H), (1, W, H), (2, 1000, 1079), (1, 64, 50)):
+            rgb, ns = omerf.render(h, cams[:n_views], w_, h_)
+            torch.cuda.synchronize()
+            for _ in range(2):
+                h_rgb, h_ns = omerf.render_host(h, cams[:n_views], w_, h_)
+                assert np.array_equal(h_ns, ns.cpu().numpy().view(np.uint32))
+                assert np.array_equal(h_rgb, rgb.cpu().numpy())
+            assert omerf.last_launch_count(h) >= 1
