@@ -315,7 +315,6 @@ extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *camer
     const unsigned int tiles_x = (unsigned int)((W + 7) / 8), tiles_y = (unsigned int)((H + 3) / 4);
     const uint64_t tile_rows = (uint64_t)n_views * tiles_y, out_bytes = px * 16;
     int bands = (int)(out_bytes / ((uint64_t)10 << 20));
-    if (getenv("OMERF_HOST_BANDS")) bands = atoi(getenv("OMERF_HOST_BANDS")); // experiment knob
     bands = bands < 1 ? 1 : (bands > 16 ? 16 : bands);
     if ((uint64_t)bands > tile_rows) bands = (int)tile_rows;
     auto pixel_row = [&](uint64_t R) { // first flattened pixel row (view * H + v) of flattened tile row R
