@@ -145,6 +145,8 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
     v.shared_taps = d->xy_n[0] == d->xz_n[0] && d->xy_n[1] == d->yz_n[0] && d->xz_n[1] == d->yz_n[1];
     v.deq_mul = d->deq_scale / 65536.0f;
     v.deq_add = 4.0f * d->deq_bias;
+    v.deq_mul_half = 0.5f * v.deq_mul;
+    v.deq_add_half = 0.5f * v.deq_add;
     v.step = d->step;
     v.inv_step = 1.0f / d->step;
     v.q_stop = (uint32_t)ceil(-log((double)d->t_stop) * 1048576.0);

@@ -36,6 +36,7 @@ struct DevScene {
     const uint2 *pxy, *pxz, *pyz;
     int shared_taps;       // xy_n[0] == xz_n[0], xy_n[1] == yz_n[0], xz_n[1] == yz_n[1]: three taps serve the six plane axes
     float deq_mul, deq_add; // scale/65536, 4*bias
+    float deq_mul_half, deq_add_half; // halves of the two: the per-sample sigmoids take tanh of half the pre-activation
     float step, inv_step;
     uint32_t q_stop;
     float bg[3];

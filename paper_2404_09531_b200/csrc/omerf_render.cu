@@ -234,11 +234,12 @@ struct BiW {
 __device__ __forceinline__ BiW bilinear_weights(uint32_t wa, uint32_t wb, int b0, int &b1)
 {
     if (wb == 0u) b1 = b0; // weight of column b1 is zero: point it at b0 so that it can carry the overflow unit
-    const uint32_t ua = 256u - wa, ub = 256u - wb;
-    const uint32_t w00 = ua * ub, c = w00 >> 16;
+    // (256 - wb | wb << 16) times a row weight <= 256 gives both products of the row in one multiply; the only carry
+    // between the halves is w00 = 2^16 (wa = wb = 0), which becomes 65535 in w00 plus 1 in w01 (the same texel then)
+    const uint32_t pb = wb * 0xffffu + 256u;
     BiW r;
-    r.w0 = (w00 - c) + ((ua * wb + c) << 16);
-    r.w1 = wa * ub + ((wa * wb) << 16);
+    r.w0 = (256u - wa) * pb + ((wa | wb) == 0u ? 0xffffu : 0u);
+    r.w1 = wa * pb;
     return r;
 }
 
@@ -370,13 +371,14 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
     bilinear8_dp(t3[0], t3[1], t3[2], t3[3], w3, I);
 }
 
-// per-sample activations (Eq. 3, colour path only): sigmoid(x) = 1/2 + 1/2 tanh(x/2) with one MUFU.TANH.
+// per-sample activations (Eq. 3, colour path only): sigmoid(2x) = 1/2 + 1/2 tanh(x) with one MUFU.TANH; the caller
+// passes HALF the pre-activation (the factor is folded into the dequantisation constants).
 // tanh.approx has an absolute error of about 2^-11 = 5e-4, so the sigmoid is off by <= 2.5e-4; the compositing
 // weights sum to <= 1, which bounds the contribution to the pixel at 2.5e-4 of the 2e-3 budget.
-__device__ __forceinline__ float sigmoid_tanh(float x)
+__device__ __forceinline__ float sigmoid_of_half(float x)
 {
     float t;
-    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(0.5f * x));
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(x));
     return fmaf(t, 0.5f, 0.5f);
 }
 
@@ -451,9 +453,6 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 #endif
 #ifndef OMERF_SAMPLE_KEEP
 #define OMERF_SAMPLE_KEEP 24   // sample again at once while this many lanes stand on an occupied point
-#endif
-#ifndef OMERF_SAMPLE_SIGMOID
-#define OMERF_SAMPLE_SIGMOID sigmoid_tanh
 #endif
 #define OMERF_WARPS 4
 static_assert(OMERF_POOL <= 255, "the census packs the state counts into bytes");
@@ -791,14 +790,15 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                     gather_features<GENERAL>(sc, px, py, pz, I);
                     float t[8];
 #pragma unroll
-                    for (int c = 0; c < 8; c++) t[c] = __fmaf_rn(__uint2float_rn(I[c]), sc.deq_mul, sc.deq_add);
+                    for (int c = 1; c < 8; c++) t[c] = fmaf(__uint2float_rn(I[c]), sc.deq_mul_half, sc.deq_add_half); // colour path
+                    t[0] = __fmaf_rn(__uint2float_rn(I[0]), sc.deq_mul, sc.deq_add);                                     // decision path
                     const float tau = exp_q(t[0]); // decision path
                     const float od = __fmul_rn(tau, sc.step);
                     const uint32_t qk = (uint32_t)rintf(fminf(__fmul_rn(od, 1048576.0f), (float)sc.q_stop));
                     const float T = __expf(-(float)Q * (1.0f / 1048576.0f)); // colour path: fast math
                     const float wgt = T * (1.0f - __expf(-od)) * soft_m;
 #pragma unroll
-                    for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, OMERF_SAMPLE_SIGMOID(t[1 + c]), acc[c]);
+                    for (int c = 0; c < 7; c++) acc[c] = fmaf(wgt, sigmoid_of_half(t[1 + c]), acc[c]);
                     Q += qk;
                     n += 1;
                     k += 1;
