@@ -253,6 +253,7 @@ def run_ours(args):
     total_ms = float(np.sum(ms))
     samples = int(out_n.sum(dtype=torch.int64).item())
     per_view = [int(x) for x in out_n.view(n_views, -1).sum(dim=1, dtype=torch.int64).tolist()]
+    hist = torch.bincount(out_n.view(-1).clamp(max=63).to(torch.int64), minlength=64).tolist()   # samples/ray, last bin = 63+
 
     # configs[4]: the same frame through the other sampler (binary occupancy grid + DDA), timed the same way
     ablation = None
@@ -331,7 +332,7 @@ def run_ours(args):
             "frames_per_s": world * n_views * k / secs,
             "gsamples_s": world * samples * k / secs / 1e9,
             "samples_per_step": samples, "samples_per_ray": samples / pixels,
-            "per_view_samples": per_view,
+            "per_view_samples": per_view, "samples_per_ray_hist": hist,
             "l2_warm": {"ms_per_step": total_warm_ms / k, "mpixels_s": world * pixels * k / (total_warm_ms / 1e3) / 1e6},
             "orbit": ({"ms_per_step_median": float(np.median(ms_orbit)), "ms_per_step_mean": float(np.mean(ms_orbit)),
                        "mpixels_s": pixels / (float(np.median(ms_orbit)) / 1e3) / 1e6, "views": 64} if ms_orbit else None),
