@@ -142,3 +142,22 @@ def test_render_host_banded_copy_is_bit_identical(omerf, city):
                 assert np.array_equal(h_ns, ns.cpu().numpy().view(np.uint32))
                 assert np.array_equal(h_rgb, rgb.cpu().numpy())
             assert omerf.last_launch_count(h) >= 1
+
+
+def test_config1_soft_mask_sampled_pixels(omerf, city):
+    """SURVEY 8(f).2 at full size: sampled pixels of the soft-occupancy render equal the oracle's (eps = 2 m)."""
+    import torch
+
+    import oracle
+    cams = synth.make_cameras(1)
+    W, H = synth.config_resolution(1)
+    with omerf.scene_create(city, soft_eps=2.0) as h:
+        rgb, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        rgb, ns = rgb.cpu().numpy(), ns.cpu().numpy().view(np.uint32)
+    vuv = _sample_pixels(np.random.default_rng(107), 1, W, H, 20000, [333])
+    ref = oracle.OracleScene(city, soft_eps=2.0).render_pixels(cams, W, H, vuv, mode="clipped")
+    hard = oracle.OracleScene(city).render_pixels(cams, W, H, vuv, mode="clipped")
+    assert np.array_equal(ns[vuv[:, 0], vuv[:, 2], vuv[:, 1]], ref["nsamples"])
+    assert np.abs(rgb[vuv[:, 0], vuv[:, 2], vuv[:, 1]].astype(np.float64) - ref["rgb"]).max() <= RGB_TOL
+    assert np.abs(ref["rgb"] - hard["rgb"]).max() > 1e-2
