@@ -39,6 +39,7 @@ BYTES_PER_PIXEL = 16     # 12 B rgb + 4 B sample count written
 OPS_PER_SAMPLE = 450      # lane-operations per sample (extract, interpolate, activate, composite)
 OPS_PER_PIXEL = 1500      # ray setup, traversal, 883-MAC MLP
 ALU_PEAK_TOPS = 148 * 128 * 1.965e9 / 1e12   # B200: SMs x fp32/int lanes x max SM clock
+NCU_DRAM_TRAFFIC = {(1, "plane"): 96_949_760 + 13_321_472}   # bytes per launch, profiles/r01_march_kernel.md
 
 
 def workload_name(cfg: int) -> str:
@@ -316,10 +317,9 @@ def run_ours(args):
         cpu = None
         if not args.no_cpu_baseline:
             cpu = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=15.0, soft_eps=args.soft_eps, count_sectors=True)
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tpath):
-            traffic = json.load(open(tpath)).get(f"config{cfg}_{args.sampler}")
+        # dram__bytes_read.sum + dram__bytes_write.sum of one march-kernel launch from the committed `ncu --set full`
+        # capture (profiles/r01_march_kernel.md); only the workload that was captured has a figure
+        traffic = NCU_DRAM_TRAFFIC.get((cfg, args.sampler)) if not (args.soft_eps or args.grid_block) else None
         line = {
             "metric": "Mpixels/s", "value": aggregate_throughput(pixels, k, world, total_ms) / 1e6, "unit": "Mpixels/s", "n_gpus": world,
             "steps": k, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
