@@ -130,6 +130,14 @@ int omerf_mlp_smoothness(const omerf_scene *scene, int64_t n, int S, const float
                          const float *dir /*DEVICE*/, const float *delta /*DEVICE*/, float *out_loss /*DEVICE*/,
                          float *out_G /*DEVICE or NULL*/, void *stream);
 
+/* Sample-count visualisation (Fig. 1, "number of samples"; S9 of SURVEY.md 8(a)): maps per-pixel sample
+ * counts to an 8-bit colour ramp from blue (0 samples) over green to red (>= n_max samples), in exact integers:
+ *     v = min(n, n_max) * 255 / n_max,   rgb = (v, 255 - |2 v - 255|, 255 - v).
+ * The paper prints no colour map; this ramp is the repo's choice (R26).
+ *   nsamples DEVICE uint32 [n_pixels], out_rgb8 DEVICE uint8 [n_pixels][3]; n_max >= 1; asynchronous on `stream`. */
+int omerf_heatmap(const uint32_t *nsamples /*DEVICE*/, uint64_t n_pixels, uint32_t n_max, uint8_t *out_rgb8 /*DEVICE*/,
+                  void *stream);
+
 /* Number of kernels of this library the last omerf_render / omerf_render_host on this scene launched. */
 int omerf_last_launch_count(const omerf_scene *scene);
 

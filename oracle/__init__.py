@@ -290,3 +290,11 @@ class SectorMaps:
 
     def compulsory_bytes(self) -> int:
         return 32 * sum(self.sectors().values())
+
+
+def heatmap(nsamples, n_max: int) -> np.ndarray:
+    """Sample-count visualisation (Fig. 1; R26), exact integers:
+    v = min(n, n_max) * 255 // n_max, rgb = (v, 255 - |2 v - 255|, 255 - v)."""
+    n = np.minimum(np.asarray(nsamples, dtype=np.int64), n_max)
+    v = n * 255 // n_max
+    return np.stack([v, 255 - np.abs(2 * v - 255), 255 - v], axis=-1).astype(np.uint8)

@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     bitfield,
     block_table,
     gather_probe,
+    heatmap,
     last_launch_count,
     load_library,
     mlp_smoothness,

@@ -22,7 +22,7 @@ SAMPLER_PLANE = 0
 SAMPLER_GRID = 1
 
 EXPORTS = (
-    "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_gather_probe", "omerf_mlp_smoothness",
+    "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_gather_probe", "omerf_mlp_smoothness", "omerf_heatmap",
     "omerf_last_launch_count",
     "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield", "omerf_scene_get_block_table",
     "omerf_scene_destroy", "omerf_last_error", "omerf_version",
@@ -80,6 +80,7 @@ def load_library() -> C.CDLL:
                                      C.POINTER(GatherProbeResult)]
     L.omerf_mlp_smoothness.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                        C.c_void_p, C.c_void_p]
+    L.omerf_heatmap.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]
     L.omerf_last_launch_count.argtypes = [C.c_void_p]
     L.omerf_scene_get_info.argtypes = [C.c_void_p, C.POINTER(SceneInfo)]
     L.omerf_scene_get_pyramid_level.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
@@ -250,6 +251,19 @@ def mlp_smoothness(h: SceneHandle, F, dirs, delta, out_loss=None, out_G=None, wa
                                                out_loss.data_ptr(), out_G.data_ptr() if out_G is not None else None,
                                                st.cuda_stream), "omerf_mlp_smoothness")
     return (out_loss, out_G) if want_G else out_loss
+
+
+def heatmap(nsamples, n_max: int, out=None, stream=None):
+    """omerf_heatmap: DEVICE sample counts (int32-viewed uint32 tensor) -> uint8 [..., 3] colour ramp; asynchronous."""
+    import torch
+    assert nsamples.is_cuda and nsamples.is_contiguous() and nsamples.element_size() == 4
+    if out is None:
+        out = torch.empty((*nsamples.shape, 3), dtype=torch.uint8, device="cuda")
+    assert out.is_cuda and out.is_contiguous() and out.dtype == torch.uint8 and out.numel() == nsamples.numel() * 3
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(load_library().omerf_heatmap(nsamples.data_ptr(), nsamples.numel(), n_max, out.data_ptr(), st.cuda_stream),
+           "omerf_heatmap")
+    return out
 
 
 def last_launch_count(h: SceneHandle) -> int:

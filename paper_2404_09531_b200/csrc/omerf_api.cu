@@ -435,6 +435,14 @@ extern "C" int omerf_mlp_smoothness(const omerf_scene *s, int64_t n, int S, cons
     return omerf_launch_smoothness(s, n, S, F, dir, delta, out_loss, out_G, (cudaStream_t)stream);
 }
 
+extern "C" int omerf_heatmap(const uint32_t *nsamples, uint64_t n_pixels, uint32_t n_max, uint8_t *out_rgb8, void *stream)
+{
+    if (n_pixels == 0) return OMERF_OK;
+    if (!nsamples || !out_rgb8) return invalid("null nsamples/out_rgb8");
+    if (n_max < 1) return invalid("n_max must be >= 1");
+    return omerf_launch_heatmap(nsamples, n_pixels, n_max, out_rgb8, (cudaStream_t)stream);
+}
+
 extern "C" int omerf_last_launch_count(const omerf_scene *s) { return s ? s->last_launches : 0; }
 
 extern "C" int omerf_scene_get_info(const omerf_scene *s, omerf_scene_info *out)

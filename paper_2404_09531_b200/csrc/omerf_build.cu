@@ -291,3 +291,28 @@ int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_
     s->device_bytes += OMERF_MLP_TAB_LEN * sizeof(float2);
     return OMERF_OK;
 }
+
+// ------------------------------------------------------------------------------------------ S9: sample-count heat map
+__global__ void heatmap_kernel(const uint32_t *__restrict__ n, unsigned long long n_pixels, uint32_t n_max, uint8_t *__restrict__ out)
+{
+    const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_pixels) return;
+    const uint32_t c = min(n[i], n_max);
+    const int v = (int)((unsigned long long)c * 255ull / n_max);
+    out[i * 3 + 0] = (uint8_t)v;
+    out[i * 3 + 1] = (uint8_t)(255 - abs(2 * v - 255));
+    out[i * 3 + 2] = (uint8_t)(255 - v);
+}
+
+int omerf_launch_heatmap(const uint32_t *n, unsigned long long n_pixels, uint32_t n_max, uint8_t *out, cudaStream_t st)
+{
+    if (n_pixels == 0) return OMERF_OK;
+    const unsigned long long blocks = (n_pixels + 255) / 256;
+    if (blocks > 0x7fffffffull) {
+        omerf_set_error("invalid argument: too many pixels");
+        return OMERF_ERR_INVALID;
+    }
+    heatmap_kernel<<<(unsigned int)blocks, 256, 0, st>>>(n, n_pixels, n_max, out);
+    OMERF_CUDA(cudaGetLastError());
+    return OMERF_OK;
+}

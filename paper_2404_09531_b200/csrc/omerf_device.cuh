@@ -101,5 +101,6 @@ int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_
 int omerf_launch_gather_probe(const omerf_scene *s, const omerf_camera *d_cam, int W, const uint2 *sample_log,
                               unsigned int n, unsigned int mult, uint32_t *sink, cudaStream_t st);
 int omerf_query_persistent_blocks(int sampler, int *blocks);
+int omerf_launch_heatmap(const uint32_t *n, unsigned long long n_pixels, uint32_t n_max, uint8_t *out, cudaStream_t st);
 int omerf_launch_smoothness(const omerf_scene *s, long long n, int S, const float *F, const float *dir, const float *delta,
                             float *out_loss, float *out_G, cudaStream_t st);

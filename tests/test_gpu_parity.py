@@ -376,3 +376,17 @@ def test_more_views_than_the_initial_camera_ring_and_repeated_calls(omerf, oracl
             assert np.array_equal(n2.cpu().numpy().view(np.uint32), ref["nsamples"][i:i + 2])
         h_rgb, h_ns = omerf.render_host(h, cams[:3], W, H)
         assert np.array_equal(h_ns, ref["nsamples"][:3])
+
+
+def test_heatmap_is_bit_exact(omerf, oracle):
+    import torch
+    sc, cams = synth.make_scene(0), synth.make_cameras(0)
+    W, H = synth.config_resolution(0)
+    with omerf.scene_create(sc) as h:
+        _, ns = omerf.render(h, cams, W, H)
+        for n_max in (1, 7, 16, 255):
+            hm = omerf.heatmap(ns, n_max)
+            torch.cuda.synchronize()
+            assert np.array_equal(hm.cpu().numpy(), oracle.heatmap(ns.cpu().numpy().view(np.uint32), n_max))
+    with pytest.raises(omerf.OmerfError):
+        omerf.heatmap(ns, 0)

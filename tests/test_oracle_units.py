@@ -276,3 +276,14 @@ def test_distinct_sector_count_matches_numpy_recount():
     before = M.sectors()
     O.render(cam, 20, 14, mode="brute")
     assert M.sectors() == before
+
+
+def test_heatmap_ramp_pins():
+    """R26: blue at 0 samples, green at the middle, red at and above n_max; red channel monotone, blue its mirror."""
+    hm = oracle.heatmap(np.arange(0, 40), 32)
+    assert hm.dtype == np.uint8 and hm.shape == (40, 3)
+    assert tuple(hm[0]) == (0, 0, 255) and tuple(hm[32]) == (255, 0, 0) and tuple(hm[39]) == (255, 0, 0)
+    assert tuple(hm[16]) == (127, 254, 128)                       # v = 16 * 255 // 32 = 127
+    assert np.all(np.diff(hm[:, 0].astype(int)) >= 0) and np.array_equal(hm[:, 2], 255 - hm[:, 0])
+    assert hm[:, 1].max() == 254 and hm[:, 1].argmax() == 16
+    assert tuple(oracle.heatmap(np.array([1]), 1)[0]) == (255, 0, 0)
