@@ -298,3 +298,30 @@ def heatmap(nsamples, n_max: int) -> np.ndarray:
     n = np.minimum(np.asarray(nsamples, dtype=np.int64), n_max)
     v = n * 255 // n_max
     return np.stack([v, 255 - np.abs(2 * v - 255), 255 - v], axis=-1).astype(np.uint8)
+
+
+class LowZBand:
+    """Oracle-side low-z bake of the xz / yz planes from the occupancy plane (omerf_oracle.c, DESIGN.md R27;
+    PAPER.md:186).  which in {"xz", "yz"}."""
+
+    def __init__(self, O: OracleScene, which: str, crop: bool = True):
+        assert which in ("xz", "yz")
+        self.O, self.which = O, which
+        n = getattr(O.c, which + "_n")
+        self.Na, self.Nb = int(n[0]), int(n[1])
+        lo, hi = C.c_int(), C.c_int()
+        self.rows = int(lib().orc_lowz_band(C.byref(O.c), C.c_int(self.Nb), C.byref(lo), C.byref(hi)))
+        self.b_lo, self.b_hi = lo.value, hi.value
+        self.band = None
+        if crop:
+            self.band = np.zeros((self.Na, self.rows, 8), dtype=np.uint8)
+            lib().orc_lowz_crop(getattr(O.c, "plane_" + which), C.c_int(self.Na), C.c_int(self.Nb), lo, hi,
+                                _ptr(self.band, _u8p))
+
+    def lookup(self, pa: float, pz: float):
+        Xa = self.O.c.box[0 if self.which == "xz" else 1]
+        out = np.zeros(8, dtype=np.uint32)
+        rc = lib().orc_plane_lookup_band(_ptr(self.band, _u8p), C.c_int(self.Na), C.c_int(self.Nb), C.c_int(self.b_lo),
+                                         C.c_int(self.b_hi), C.c_float(Xa), C.c_float(self.O.c.box[2]), C.c_float(pa),
+                                         C.c_float(pz), _ptr(out, _u32p))
+        return int(rc), out

@@ -769,6 +769,67 @@ int orc_sparse_grid_lookup(const int32_t *table, const uint8_t *atlas, int B, co
     return 0;
 }
 
+/* ------------------------------------------------------------------ low-z triplane bake (second half) */
+/* PAPER.md:186 (sec. 4.4): "For the 2D triplane, we employ a texture map with high resolution in the xy direction and
+ * low resolution in the z direction, according to the upper and lower bounds of the occupancy plane.  This approach
+ * saves a significant amount of video memory during real-time rendering."  The paper gives no rule; reading R27
+ * (DESIGN.md): the xz and yz planes keep ONE contiguous band of z-texel rows [b_lo, b_hi] - the rows that a bilinear
+ * lookup (R10 addressing: q = z Nz/Z - 1/2, taps floor(q) and floor(q)+1, clamped to the plane) can touch for
+ *     z in [z_lo, z_hi],  z_lo = min z_min,  z_hi = max z_max  over the NON-EMPTY columns of P_o (R17), clipped to [0,Z],
+ * widened by 1/64 texel on both sides (far above the fp32 rounding of the renderer's q; same padding as R24).
+ * Every sample of the occupancy-plane sampler has z in [z_lo, z_hi] (Eq. 7), so no row outside the band is ever fetched
+ * and the image is the uncropped oracle's.  A scene with no non-empty column keeps row 0 only (never fetched).
+ * Double arithmetic, one rounding per operation.  Returns the number of rows kept. */
+int orc_lowz_band(const orc_scene *s, int Nz, int *b_lo, int *b_hi)
+{
+    const int Mx = s->hf_n[0], My = s->hf_n[1];
+    const double Z = (double)s->box[2];
+    double zl = 0.0, zh = 0.0;
+    int any = 0;
+    for (size_t i = 0; i < (size_t)Mx * My; i++) {
+        float lo = s->h_lo[i], hi = s->h_up[i];
+        if (!(lo <= hi)) continue;                            /* empty column (R17) */
+        if (!any || (double)lo < zl) zl = (double)lo;
+        if (!any || (double)hi > zh) zh = (double)hi;
+        any = 1;
+    }
+    if (zl < 0.0) zl = 0.0;
+    if (zh > Z) zh = Z;
+    if (!any || zl > zh) {
+        *b_lo = 0;
+        *b_hi = 0;
+        return 1;
+    }
+    double qa = zl * (double)Nz / Z - 0.515625;               /* - 1/2 - 1/64 */
+    double qb = zh * (double)Nz / Z - 0.484375;               /* - 1/2 + 1/64 */
+    int64_t a = (int64_t)floor(qa), b = (int64_t)floor(qb) + 1;
+    *b_lo = (int)(a < 0 ? 0 : a);
+    *b_hi = (int)(b > Nz - 1 ? Nz - 1 : b);
+    return *b_hi - *b_lo + 1;
+}
+
+/* the baked plane: out[Na][b_hi-b_lo+1][8] = tex[Na][b_lo..b_hi][8] */
+void orc_lowz_crop(const uint8_t *tex, int Na, int Nb, int b_lo, int b_hi, uint8_t *out)
+{
+    const int Bk = b_hi - b_lo + 1;
+    for (int a = 0; a < Na; a++)
+        for (int b = 0; b < Bk; b++) memcpy(out + ((size_t)a * Bk + b) * 8, tex + ((size_t)a * Nb + b_lo + b) * 8, 8);
+}
+
+/* orc_plane_lookup through the baked band (taps addressed as in the full plane of Nb rows, then shifted by b_lo);
+ * returns -1 if a z-tap of (pa, pz) lies outside the band */
+int orc_plane_lookup_band(const uint8_t *band, int Na, int Nb, int b_lo, int b_hi, float Xa, float Z, float pa,
+                          float pz, uint32_t B[8])
+{
+    int a0, a1, b0, b1;
+    uint32_t wa, wb;
+    axis_tap(pa, Na, Xa, &a0, &a1, &wa);
+    axis_tap(pz, Nb, Z, &b0, &b1, &wb);
+    if (b0 < b_lo || b1 > b_hi) return -1;
+    bilinear8(band, b_hi - b_lo + 1, a0, a1, wa, b0 - b_lo, b1 - b_lo, wb, B);
+    return 0;
+}
+
 /* ------------------------------------------------------------------ view-direction smoothness term */
 /* PAPER.md:145-155, Eq. 9-10: for a viewing direction d, perturbed directions s = d + delta (delta ~ N(0, Sigma) is an
  * INPUT here: the random draws are the caller's) and

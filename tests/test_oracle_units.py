@@ -241,6 +241,33 @@ def test_bitfield_vs_exact_rational_brute_force(hf_n, occ_n):
     assert np.array_equal(bits, _brute_bitfield(sc))
 
 
+def test_occupied_grid_lookup_reads_the_voxel_that_contains_the_point():
+    """The config-4 predicate (sampler 1) pinned directly: for random points away from voxel faces
+    the voxel (jx,jy,jz) is recomputed in float64 and the answer is read from the exact-rational brute-force bitfield.
+    Non-cubic occ_n with Ny != Nz != Nx: an index swap, a transposed stride or an enlarged set fails."""
+    rng = np.random.default_rng(12)
+    hf_n, occ_n, box = (5, 4), (6, 7, 5), (8.0, 6.0, 4.0)
+    lo = rng.uniform(0.2, 1.5, hf_n).astype(np.float32)
+    hi = (lo + rng.uniform(-0.3, 2.0, hf_n)).astype(np.float32)
+    sc = synth.custom_scene(box=box, hf_n=hf_n, h_lo=lo, h_up=hi, occ_n=occ_n)
+    O = oracle.OracleScene(sc, sampler=1)
+    want = _brute_bitfield(sc)
+    assert 0 < want.sum() < want.size                              # both answers occur
+    seen = {False: 0, True: 0}
+    for p in rng.uniform(0.0, 1.0, (6000, 3)) * np.array(box):
+        q = p * np.array(occ_n) / np.array(box)                   # voxel coordinates, float64
+        if np.any(np.abs(q - np.rint(q)) < 1e-3):                 # too close to a voxel face for fp32 to agree
+            continue
+        j = np.floor(q).astype(int)
+        got = O.occupied(p.astype(np.float32))
+        assert got == bool(want[j[0], j[1], j[2]]), (p, j)
+        seen[got] += 1
+    assert seen[False] > 500 and seen[True] > 500
+    # clamp at the far faces: a point on the box face belongs to the last voxel
+    for p, j in (((8.0, 3.0, 2.0), (5, 3, 2)), ((4.0, 6.0, 2.0), (3, 6, 2)), ((4.0, 3.0, 4.0), (3, 3, 4))):
+        assert O.occupied(np.array(p, dtype=np.float32)) == bool(want[j])
+
+
 def test_distinct_sector_count_matches_numpy_recount():
     """SURVEY 8(d) compulsory-byte figure: distinct 32-byte sectors per source touched by a render, recounted in numpy
     from the kept sample positions (thin density: no ray terminates, so every kept lattice point is a sample)."""
