@@ -114,15 +114,19 @@ def oracle_bounded(scene, cams, W, H, sampler=0, budget_s=15.0, soft_eps=0.0, co
     t0 = time.perf_counter()
     samples = 0
     threads = 1
+    ref_n = np.zeros((len(rows), W), dtype=np.uint32)
+    ref_rgb = np.zeros((len(rows), W, 3), dtype=np.float64)
     # contiguous row blocks are cheaper to call; rows are sampled with a stride so sky and ground both count
-    for v in rows:
+    for i, v in enumerate(rows):
         r = O.render(cams[:1], W, H, mode="clipped", rows=(v, v + 1))
         samples += int(r["nsamples"][0, v].sum())
         threads = r["threads"]
+        ref_n[i], ref_rgb[i] = r["nsamples"][0, v], r["rgb"][0, v]
     dt = time.perf_counter() - t0
     px = len(rows) * W
     out = {"mpix_s": px / dt / 1e6, "msamples_s": samples / dt / 1e6, "seconds": dt, "pixels": px, "samples": samples,
-           "cores": threads, "sample": f"{len(rows)} of {H} rows (every {stride}th) of view 0, clipped loop"}
+           "cores": threads, "sample": f"{len(rows)} of {H} rows (every {stride}th) of view 0, clipped loop",
+           "rows": rows, "ref_n": ref_n, "ref_rgb": ref_rgb}
     if count_sectors and stride == 1:
         # distinct 32-byte sectors the frame's samples touch (untimed second pass over the same rows)
         with oracle.SectorMaps(O) as M:
@@ -363,6 +367,14 @@ def run_ours(args):
         if ablation is not None:
             line["ablation"] = ablation
         if cpu is not None:
+            # element-wise parity of the rows the oracle just rendered (the whole frame when it fits the time budget)
+            # against the device outputs of the timed workload; outside every timed region
+            got_n = out_n[0].cpu().numpy().view(np.uint32)[cpu["rows"]]
+            got_rgb = out_rgb[0].cpu().numpy()[cpu["rows"]].astype(np.float64)
+            line["parity"] = {"pixels_compared": int(got_n.size), "of_pixels_in_view0": W * H,
+                              "count_mismatches": int((got_n != cpu["ref_n"]).sum()),
+                              "max_abs_drgb": float(np.abs(got_rgb - cpu["ref_rgb"]).max()), "rgb_tol": 2e-3,
+                              "against": "oracle (clipped loop), same run"}
             line["cpu_baseline"] = {"value": cpu["mpix_s"], "unit": "Mpixels/s", "cores": cpu["cores"], "kind": "oracle",
                                     "sample": cpu["sample"], "msamples_s": cpu["msamples_s"], "seconds": cpu["seconds"]}
             if "compulsory_bytes" in cpu:     # the HBM ceiling of SURVEY 8(d): bytes an unbounded cache would still fetch

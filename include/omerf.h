@@ -64,7 +64,8 @@ typedef struct {
     int32_t grid_block; /* 0: V is stored dense.  2, 4, 8 or 16: V is stored as sparse blocks of grid_block^3 voxels
                             baked on the device from the occupancy plane: only blocks
                            holding a voxel that a sample inside the slab can touch are kept (R24); the
-                           rendered images are identical to the dense layout's. */
+                           rendered images are identical to the dense layout's.  Sampler PLANE only: the grid sampler's
+                           voxels are a superset of the slab (OMERF_ERR_INVALID otherwise). */
 } omerf_scene_desc;
 
 /* Pinhole camera, world frame. */
@@ -94,14 +95,22 @@ int omerf_scene_create(const omerf_scene_desc *desc /*HOST*/, omerf_scene **out_
  *   out_rgb       DEVICE [n_views][H][W][3] float32, 4-byte aligned
  *   out_nsamples  DEVICE [n_views][H][W] uint32: samples fetched per pixel (Fig. 1)
  *   stream        cudaStream_t (NULL = default stream)
- * Asynchronous: kernels are enqueued on `stream`; results are valid once the caller has synchronised
- * it.  Calls on one scene must be stream-ordered or externally serialised. */
+ * Asynchronous: kernels are enqueued on `stream`; results are valid once the caller has synchronised it.
+ * Threads and streams: a scene handle keeps per-call state (a 16-slot ring of pinned camera staging, device cameras
+ * and work-queue heads, the launch counter, the scratch of omerf_render_host), so it must NOT be used by two host
+ * threads at once - serialise the calls (one thread at a time).  Serialised calls may use different streams: a ring slot
+ * is reused only after the kernel that last used it has finished (the 17th call in flight waits for the 1st).
+ * The scene's device must be the current device (else OMERF_ERR_INVALID).
+ * Allocation: the first call with more views than any call before it re-allocates the camera ring
+ * (cudaDeviceSynchronize + cudaMalloc inside the call); calls after that warm-up do not allocate. */
 int omerf_render(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W, int H,
                  float *out_rgb /*DEVICE*/, uint32_t *out_nsamples /*DEVICE*/, void *stream);
 
 /* Same path with HOST outputs (pinned or pageable): renders into scene-owned device scratch on
  * `stream` in bands of whole tile rows, copies each band back on a scene-owned second stream while the next
- * band renders, and synchronises both streams before returning. */
+ * band renders, and synchronises both streams before returning.  The first call with more pixels than any call
+ * before it (re)allocates the scratch (cudaDeviceSynchronize + cudaMalloc inside the call).  Same threading rule as
+ * omerf_render. */
 int omerf_render_host(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W,
                       int H, float *out_rgb /*HOST*/, uint32_t *out_nsamples /*HOST*/, void *stream);
 

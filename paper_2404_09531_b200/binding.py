@@ -117,9 +117,12 @@ def make_desc(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, grid_b
     _, d.h_up = arr(scene.h_up, np.float32, _f32p)
     d.hf_n[:] = lo.shape
     g, d.grid = arr(scene.grid, np.uint8, _u8p)
+    assert g.ndim == 4 and g.shape[3] == 8, "grid must be [Gx][Gy][Gz][8] uint8"
     d.grid_n[:] = g.shape[:3]
+    assert lo.ndim == 2 and np.shape(scene.h_up) == lo.shape, "h_lo / h_up must be [Mx][My]"
     for nm in ("xy", "xz", "yz"):
         p, ptr = arr(getattr(scene, "plane_" + nm), np.uint8, _u8p)
+        assert p.ndim == 3 and p.shape[2] == 8, f"plane_{nm} must be [A][B][8] uint8"
         getattr(d, nm + "_n")[:] = p.shape[:2]
         setattr(d, "plane_" + nm, ptr)
     d.deq_scale, d.deq_bias = scene.deq_scale, scene.deq_bias

@@ -31,8 +31,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    extra = os.environ.get("OMERF_NVCC_EXTRA", "").split()   # tuning knobs, e.g. -DOMERF_POOL=128
-    cmd = [NVCC, *NVCC_FLAGS, *extra, "-o", tmp, *sources()]
+    cmd = [NVCC, *NVCC_FLAGS, "-o", tmp, *sources()]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         print(res.stdout)

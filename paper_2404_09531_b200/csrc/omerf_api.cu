@@ -106,6 +106,9 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         return invalid("grid_block must be 0, 2, 4, 8 or 16");
     if (!(d->soft_eps >= 0) || !isfinite(d->soft_eps)) return invalid("soft_eps must be >= 0");
     if (d->soft_eps > 0 && d->sampler != OMERF_SAMPLER_PLANE) return invalid("soft_eps needs the occupancy-plane sampler");
+    // the sparse-block bake (R24) keeps what a sample INSIDE THE SLAB can touch; the grid sampler's voxels are a superset of the
+    // slab (R18), so its samples may have corners in blocks that were not kept
+    if (d->grid_block != 0 && d->sampler != OMERF_SAMPLER_PLANE) return invalid("grid_block needs the occupancy-plane sampler");
     if (d->sampler == OMERF_SAMPLER_GRID)
         for (int i = 0; i < 3; i++)
             if (d->occ_n[i] < 1) return invalid("occ_n must be >= 1 for the grid sampler");
@@ -197,7 +200,8 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         }
         if ((rc = omerf_query_persistent_blocks(d->sampler, &s->persistent_blocks))) break;
         {
-            cudaError_t ee = cudaMalloc((void **)&s->d_tile_counter, 64 * sizeof(unsigned int) + 8 * 8 * 8192);
+            // one work-queue head per camera-ring slot (word 0; word 32 counts logged samples in the calibration render)
+            cudaError_t ee = cudaMalloc((void **)&s->d_tile_counter, OMERF_CAM_SLOTS * OMERF_COUNTER_WORDS * sizeof(unsigned int));
             if (ee != cudaSuccess) {
                 rc = omerf_cuda_fail(ee, "cudaMalloc tile counter");
                 break;
@@ -250,35 +254,51 @@ static int ensure_cams(const omerf_scene *s, int n_views)
     return OMERF_OK;
 }
 
+// the scene's device must be the current one: every pointer in the handle belongs to it
+static int check_device(const omerf_scene *s)
+{
+    int dev = -1;
+    OMERF_CUDA(cudaGetDevice(&dev));
+    if (dev != s->device) {
+        omerf_set_error("invalid argument: scene lives on device %d but device %d is current", s->device, dev);
+        return OMERF_ERR_INVALID;
+    }
+    return OMERF_OK;
+}
+
 // Stages the cameras and launches the march kernel for the tiles [tile_first, tile_end) of the batch (0, 0 = all).
-// *d_cams_io: device cameras of an earlier band of the same call (nullptr: stage them now).
+// *slot_io: ring slot of an earlier band of the same call (-1: take the next slot and stage the cameras now).
+// A slot (pinned staging, device cameras, work-queue head) is reused only after the last kernel that used it has
+// finished: its event is recorded after the launch.
 static int render_impl(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H, float *out_rgb,
-                       uint32_t *out_nsamples, void *stream, unsigned int tile_first, unsigned int tile_end,
-                       omerf_camera **d_cams_io)
+                       uint32_t *out_nsamples, void *stream, unsigned int tile_first, unsigned int tile_end, int *slot_io)
 {
     if (!s || !cameras || !out_rgb || !out_nsamples) return invalid("null scene/cameras/output");
     if (n_views < 0 || W <= 0 || H <= 0) return invalid("n_views >= 0, W > 0, H > 0 required");
     if (((uintptr_t)out_rgb & 3) || ((uintptr_t)out_nsamples & 3)) return invalid("misaligned output");
     if (n_views == 0) return OMERF_OK;
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = ensure_cams(s, n_views);
+    int rc = check_device(s);
     if (rc) return rc;
-    omerf_camera *dv = d_cams_io ? *d_cams_io : nullptr;
-    if (!dv) {
+    if ((rc = ensure_cams(s, n_views))) return rc;
+    int slot = slot_io ? *slot_io : -1;
+    if (slot < 0) {
         // stage the cameras: user memory -> pinned ring slot -> device ring slot (stream-ordered)
-        int slot = (int)(s->call_index++ % OMERF_CAM_SLOTS);
+        slot = (int)(s->call_index++ % OMERF_CAM_SLOTS);
         OMERF_CUDA(cudaEventSynchronize(s->slot_event[slot]));
         omerf_camera *h = s->h_cams + (size_t)slot * s->cam_capacity;
-        dv = s->d_cams + (size_t)slot * s->cam_capacity;
         memcpy(h, cameras, (size_t)n_views * sizeof(omerf_camera));
-        OMERF_CUDA(cudaMemcpyAsync(dv, h, (size_t)n_views * sizeof(omerf_camera), cudaMemcpyHostToDevice, st));
-        OMERF_CUDA(cudaEventRecord(s->slot_event[slot], st));
-        if (d_cams_io) *d_cams_io = dv;
+        OMERF_CUDA(cudaMemcpyAsync(s->d_cams + (size_t)slot * s->cam_capacity, h, (size_t)n_views * sizeof(omerf_camera),
+                                   cudaMemcpyHostToDevice, st));
+        if (slot_io) *slot_io = slot;
     }
     int launches = 0;
-    rc = omerf_launch_render(s, dv, n_views, W, H, out_rgb, out_nsamples, st, &launches, nullptr, 0, tile_first, tile_end);
+    rc = omerf_launch_render(s, s->d_cams + (size_t)slot * s->cam_capacity, n_views, W, H, out_rgb, out_nsamples, st,
+                             s->d_tile_counter + (size_t)slot * OMERF_COUNTER_WORDS, &launches, nullptr, 0, tile_first, tile_end);
     s->last_launches += launches;
-    return rc;
+    if (rc) return rc;
+    OMERF_CUDA(cudaEventRecord(s->slot_event[slot], st));
+    return OMERF_OK;
 }
 
 extern "C" int omerf_render(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
@@ -294,6 +314,10 @@ extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *camer
     if (!s || !cameras || !out_rgb || !out_nsamples) return invalid("null scene/cameras/output");
     if (n_views < 0 || W <= 0 || H <= 0) return invalid("n_views >= 0, W > 0, H > 0 required");
     if (n_views == 0) return OMERF_OK;
+    {
+        int rc = check_device(s);
+        if (rc) return rc;
+    }
     uint64_t px = (uint64_t)n_views * W * H;
     if (px > s->scratch_pixels) {
         cudaDeviceSynchronize();
@@ -325,11 +349,11 @@ extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *camer
         return view * (uint64_t)H + v;
     };
     s->last_launches = 0;
-    omerf_camera *d_cams = nullptr;
+    int slot = -1;
     for (int b = 0; b < bands; b++) {
         const uint64_t R0 = tile_rows * b / bands, R1 = tile_rows * (b + 1) / bands;
         int rc = render_impl(s, cameras, n_views, W, H, s->d_scratch_rgb, s->d_scratch_n, stream, (unsigned int)(R0 * tiles_x),
-                             (unsigned int)(R1 * tiles_x), &d_cams);
+                             (unsigned int)(R1 * tiles_x), &slot);
         if (rc) return rc;
         OMERF_CUDA(cudaEventRecord(s->band_event[b], st));
         OMERF_CUDA(cudaStreamWaitEvent(s->copy_stream, s->band_event[b], 0));
@@ -354,8 +378,9 @@ extern "C" int omerf_gather_probe(const omerf_scene *s, const omerf_camera *came
     if (W <= 0 || H <= 0 || repeats <= 0) return invalid("W > 0, H > 0, repeats > 0 required");
     memset(out, 0, sizeof *out);
     const uint64_t px = (uint64_t)W * H;
-    int rc = ensure_cams(s, 1);
+    int rc = check_device(s);
     if (rc) return rc;
+    if ((rc = ensure_cams(s, 1))) return rc;
     OMERF_CUDA(cudaDeviceSynchronize());
     omerf_camera *dv = s->d_cams; // slot 0 of the ring; nothing is in flight after the synchronise
     OMERF_CUDA(cudaMemcpy(dv, camera, sizeof(omerf_camera), cudaMemcpyHostToDevice));
@@ -378,7 +403,7 @@ extern "C" int omerf_gather_probe(const omerf_scene *s, const omerf_camera *came
         for (int attempt = 0; attempt < 2 && rc == OMERF_OK; attempt++) {
             PROBE_CUDA(cudaMalloc((void **)&log, (size_t)cap * sizeof(uint2)));
             int launches = 0;
-            if ((rc = omerf_launch_render(s, dv, 1, W, H, rgb, cnt, 0, &launches, log, cap))) break;
+            if ((rc = omerf_launch_render(s, dv, 1, W, H, rgb, cnt, 0, s->d_tile_counter, &launches, log, cap))) break;
             PROBE_CUDA(cudaMemcpy(&n, s->d_tile_counter + 32, sizeof n, cudaMemcpyDeviceToHost));
             if (n <= cap) break;
             cudaFree(log); // more samples than the first guess: size the log exactly and log again
@@ -431,6 +456,10 @@ extern "C" int omerf_mlp_smoothness(const omerf_scene *s, int64_t n, int S, cons
     if (n == 0) return OMERF_OK;
     if (!F || !dir || !out_loss || (S > 0 && !delta)) return invalid("null F/dir/delta/out_loss");
     if ((unsigned long long)n * (unsigned long long)(S + 1) > 0x7fffffffffffull) return invalid("batch too large");
+    {
+        int rc = check_device(s);
+        if (rc) return rc;
+    }
     s->last_launches = 1;
     return omerf_launch_smoothness(s, n, S, F, dir, delta, out_loss, out_G, (cudaStream_t)stream);
 }

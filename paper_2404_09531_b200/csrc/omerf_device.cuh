@@ -75,11 +75,12 @@ struct omerf_scene {
     mutable int last_launches;
     mutable cudaStream_t copy_stream;  // omerf_render_host: copies a band back while the next one renders
     mutable cudaEvent_t band_event[16];
-    unsigned int *d_tile_counter;     // work queue head of the persistent march kernel
+    unsigned int *d_tile_counter;     // work-queue heads of the persistent march kernel, one per camera-ring slot
     int persistent_blocks;            // resident CTAs of the march kernel (SMs x occupancy)
 };
 
 #define OMERF_CAM_SLOTS 16
+#define OMERF_COUNTER_WORDS 64   // per ring slot: word 0 = work-queue head, word 32 = logged samples (calibration render)
 
 // error plumbing (omerf_api.cu)
 void omerf_set_error(const char *fmt, ...);
@@ -96,7 +97,8 @@ int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st);
 int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream_t st);
 int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_t st);
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H,
-                        float *out_rgb, uint32_t *out_n, cudaStream_t st, int *launches, uint2 *sample_log = nullptr,
+                        float *out_rgb, uint32_t *out_n, cudaStream_t st, unsigned int *tile_counter, int *launches,
+                        uint2 *sample_log = nullptr,
                         unsigned int log_capacity = 0, unsigned int tile_first = 0, unsigned int tile_end = 0);
 int omerf_launch_gather_probe(const omerf_scene *s, const omerf_camera *d_cam, int W, const uint2 *sample_log,
                               unsigned int n, unsigned int mult, uint32_t *sink, cudaStream_t st);

@@ -28,8 +28,6 @@
 // in k in every component (rounding is monotone), so cell indices and z are monotone in k.  If samples k
 // and kk both lie in one pyramid node and both are on the same side outside its [min,max] z-range, so
 // does every sample between them: all of them fail the predicate and may be skipped.
-#include <stdio.h>
-
 #include "omerf_device.cuh"
 #include "omerf_mlp.cuh"
 
@@ -38,27 +36,13 @@ namespace {
 enum : int { ST_IDLE = 0, ST_TRAV = 1, ST_READY = 2, ST_FIN = 3 };
 
 // level policy of the pyramid traversal (speed only: every jump is verified), tuned on B200 with configs[1]
-#ifndef OMERF_LVL_START
-#define OMERF_LVL_START 6      // first node size: 2^6 cells
-#endif
-#ifndef OMERF_LVL_ENTER
-#define OMERF_LVL_ENTER 2      // levels to descend when a jump ends where z enters the node's range
-#endif
-#ifndef OMERF_LVL_INSIDE
-#define OMERF_LVL_INSIDE 2     // levels to descend when the point is inside the node's z-range
-#endif
-#ifndef OMERF_LVL_FAIL
-#define OMERF_LVL_FAIL 2       // levels to descend when the proposed jump could not be verified
-#endif
-#ifndef OMERF_GRID_LVL_INSIDE
-#define OMERF_GRID_LVL_INSIDE 1 // config-4 comparator (occupancy mip chain): levels to descend in an occupied node
-#endif
-#ifndef OMERF_GRID_LVL_FAIL
-#define OMERF_GRID_LVL_FAIL 2   // ... and after a proposal that could not be verified
-#endif
-#ifndef OMERF_LVL_UP
-#define OMERF_LVL_UP 1         // levels to ascend after a verified jump across an xy node boundary
-#endif
+constexpr int OMERF_LVL_START = 6;      // first node size: 2^6 cells
+constexpr int OMERF_LVL_ENTER = 2;      // levels to descend when a jump ends where z enters the node's range
+constexpr int OMERF_LVL_INSIDE = 2;     // levels to descend when the point is inside the node's z-range
+constexpr int OMERF_LVL_FAIL = 2;       // levels to descend when the proposed jump could not be verified
+constexpr int OMERF_GRID_LVL_INSIDE = 1; // config-4 comparator (occupancy mip chain): levels to descend in an occupied node
+constexpr int OMERF_GRID_LVL_FAIL = 2;   // ... and after a proposal that could not be verified
+constexpr int OMERF_LVL_UP = 1;         // levels to ascend after a verified jump across an xy node boundary
 
 
 
@@ -433,37 +417,19 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
 
 // ---------------------------------------------------------------------------------- the persistent kernel
 // Warp-private ray pool in shared memory (structure of arrays, one word per ray and field).
-#ifndef OMERF_POOL
-#define OMERF_POOL 96          // rays per warp; a multiple of 32
-#endif
-#ifndef OMERF_TRAV_STEPS
-#define OMERF_TRAV_STEPS 48    // cap on the traversal steps of one visit
-#endif
-#ifndef OMERF_TRAV_KEEP
-#define OMERF_TRAV_KEEP 16
-#endif
-#ifndef OMERF_DRAIN_TRAV_KEEP
-#define OMERF_DRAIN_TRAV_KEEP 1  // in the endgame and the drain a traversal visit runs until every listed ray is done
-#endif
-#ifndef OMERF_SAMPLE_SWAP
-#define OMERF_SAMPLE_SWAP 8    // lanes that must have left the READY state before they take the next listed rays
-#endif
-#ifndef OMERF_TRAV_SWAP
-#define OMERF_TRAV_SWAP 8      // lanes that must be free before they take the next listed rays
-#endif
-#ifndef OMERF_SAMPLE_KEEP
-#define OMERF_SAMPLE_KEEP 24   // sample again at once while this many lanes stand on an occupied point
-#endif
+constexpr int OMERF_POOL = 96;          // rays per warp; a multiple of 32
+constexpr int OMERF_TRAV_STEPS = 48;    // cap on the traversal steps of one visit
+constexpr int OMERF_TRAV_KEEP = 16;
+constexpr int OMERF_DRAIN_TRAV_KEEP = 1;  // in the endgame and the drain a traversal visit runs until every listed ray is done
+constexpr int OMERF_SAMPLE_SWAP = 8;    // lanes that must have left the READY state before they take the next listed rays
+constexpr int OMERF_TRAV_SWAP = 8;      // lanes that must be free before they take the next listed rays
+constexpr int OMERF_SAMPLE_KEEP = 24;   // sample again at once while this many lanes stand on an occupied point
 #define OMERF_WARPS 4
 static_assert(OMERF_POOL <= 255, "the census packs the state counts into bytes");
 static_assert(OMERF_SAMPLE_SWAP >= 1 && OMERF_SAMPLE_SWAP <= 32 && OMERF_TRAV_SWAP >= 1 && OMERF_TRAV_SWAP <= 32,
               "a swap threshold above the warp size would never release a finished lane");
-#ifndef OMERF_ENDGAME_WARPS
-#define OMERF_ENDGAME_WARPS 2   // endgame starts when fewer than this many tiles per warp are left
-#endif
-#ifndef OMERF_ENDGAME_BUSY
-#define OMERF_ENDGAME_BUSY 32   // in the endgame a warp takes a new tile only with at most this many rays in flight
-#endif
+constexpr int OMERF_ENDGAME_WARPS = 2;   // endgame starts when fewer than this many tiles per warp are left
+constexpr int OMERF_ENDGAME_BUSY = 32;   // in the endgame a warp takes a new tile only with at most this many rays in flight
 #define OMERF_PJ (OMERF_POOL / 32)
 
 struct WarpPool {
@@ -584,9 +550,7 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
     if (L.slot >= 0) trav_store(sc, P, L, out_rgb, out_n);
 }
 
-#ifndef OMERF_MIN_BLOCKS
-#define OMERF_MIN_BLOCKS 5
-#endif
+constexpr int OMERF_MIN_BLOCKS = 5;
 // LOG (gather calibration only): every sample taken is appended to sample_log as (pixel, lattice index).
 // GENERAL: the 8(f) variants (soft occupancy, sparse-block grid) behind warp-uniform branches; the plain path
 // (dense grid, binary mask) is compiled without them.
@@ -609,10 +573,6 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 #pragma unroll
     for (int j = 0; j < OMERF_PJ; j++) P.meta[lane + 32 * j] = ST_IDLE;
     __syncwarp();
-#ifdef OMERF_X_TIMELINE
-    unsigned long long *tl = reinterpret_cast<unsigned long long *>(tile_counter + 64);
-    if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8 + 0] = t; }
-#endif
     bool more = true;
     OriginCache oc = {0xffffffffu, 0.0f, 0.0f, 0.0f};
     // Endgame: a warp's pool holds about three tiles of work, which would all drain at falling utilisation once the
@@ -648,24 +608,11 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
         else if (cnt[ST_TRAV] > 0) OMERF_PICK(ST_TRAV)
         else if (cnt[ST_FIN] > 0) OMERF_PICK(ST_FIN) // finished rays wait for a full MLP batch unless nothing else is left
         else {
-#ifdef OMERF_X_TIMELINE
-            if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8 + 2] = t; }
-#endif
             break; // pool empty and no tile left (otherwise the refill branch was taken)
         }
 #undef OMERF_PICK
 #pragma unroll
         for (int j = 0; j < OMERF_PJ; j++) b[j] = __ballot_sync(FULL, st_lane[j] == (uint32_t)phase);
-#ifdef OMERF_X_TIMELINE
-        if (lane == 0) {
-            unsigned long long *e = tl + (blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8;
-            if (!more) {
-                if (e[3] == 0) e[3] = 1ull | ((unsigned long long)cnt[ST_TRAV] << 8) | ((unsigned long long)cnt[ST_READY] << 16) | ((unsigned long long)cnt[ST_FIN] << 24);
-                e[4 + (phase == ST_TRAV ? 0 : phase == ST_READY ? 1 : 2)] += 1;
-                e[7] += (unsigned long long)min(n_sel, 32);
-            }
-        }
-#endif
         // ---- the slots in that state, in slot order
         {
             int base = 0;
@@ -689,9 +636,6 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             if (tile + endgame_tiles >= total_tiles) endgame = true;
             if (tile >= total_tiles) {
                 more = false;
-#ifdef OMERF_X_TIMELINE
-                if (lane == 0) { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); tl[(blockIdx.x * OMERF_WARPS + (threadIdx.x >> 5)) * 8 + 1] = t; }
-#endif
             } else {
                 const unsigned view = tile / tiles_per_view, tv = tile - view * tiles_per_view;
                 const int ty = (int)(tv / (unsigned)tiles_x), tx = (int)(tv - (unsigned)ty * tiles_x);
@@ -935,45 +879,14 @@ int omerf_launch_gather_probe(const omerf_scene *s, const omerf_camera *d_cam, i
 }
 
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H, float *out_rgb,
-                        uint32_t *out_n, cudaStream_t st, int *launches, uint2 *sample_log, unsigned int log_capacity,
-                        unsigned int tile_first, unsigned int tile_end)
+                        uint32_t *out_n, cudaStream_t st, unsigned int *tile_counter, int *launches, uint2 *sample_log,
+                        unsigned int log_capacity, unsigned int tile_first, unsigned int tile_end)
 {
     if ((long long)((W + 7) / 8) * ((H + 3) / 4) * n_views > 0x7fffffffll || (long long)W * H * n_views > 0xffffffffll) {
         omerf_set_error("invalid argument: image or batch too large");
         return OMERF_ERR_INVALID;
     }
-#ifdef OMERF_X_TIMELINE
-    {
-        static int calls = 0;
-        if (calls++ == 8) {
-            int nw = s->persistent_blocks * OMERF_WARPS;
-            unsigned long long *h = new unsigned long long[nw * 8];
-            cudaMemcpy(h, s->d_tile_counter + 64, sizeof(unsigned long long) * nw * 8, cudaMemcpyDeviceToHost);
-            unsigned long long t0 = ~0ull;
-            for (int i = 0; i < nw; i++) if (h[i * 8] < t0) t0 = h[i * 8];
-            // sort warps by finish time; print stats for all and for the slowest 2 %
-            int *idx = new int[nw];
-            for (int i = 0; i < nw; i++) idx[i] = i;
-            for (int i = 1; i < nw; i++) { int v = idx[i], j = i - 1; while (j >= 0 && h[idx[j] * 8 + 2] > h[v * 8 + 2]) { idx[j + 1] = idx[j]; j--; } idx[j + 1] = v; }
-            for (int pass = 0; pass < 2; pass++) {
-                int lo = pass == 0 ? 0 : nw - nw / 50, cntw = nw - lo;
-                double ex = 0, fin = 0, tr = 0, rd = 0, fn = 0, rt = 0, rr = 0, rf = 0, lanes = 0;
-                for (int q = lo; q < nw; q++) {
-                    unsigned long long *e = h + idx[q] * 8;
-                    ex += (e[1] - t0) * 1e-3; fin += (e[2] - t0) * 1e-3;
-                    tr += (e[3] >> 8) & 255; rd += (e[3] >> 16) & 255; fn += (e[3] >> 24) & 255;
-                    rt += e[4]; rr += e[5]; rf += e[6]; lanes += e[7];
-                }
-                printf("TIMELINE %s (%d warps): exhausted %.1f us, finish %.1f us; at exhaustion TRAV %.1f READY %.1f FIN %.1f; rounds after: trav %.1f sample %.1f retire %.1f, lanes/round %.1f\n",
-                       pass == 0 ? "all" : "slowest 2%", cntw, ex / cntw, fin / cntw, tr / cntw, rd / cntw, fn / cntw, rt / cntw, rr / cntw, rf / cntw, lanes / (rt + rr + rf));
-            }
-            delete[] idx;
-            delete[] h;
-        }
-        cudaMemsetAsync(s->d_tile_counter + 64, 0, 8 * 8 * 8192, st);
-    }
-#endif
-    OMERF_CUDA(cudaMemsetAsync(s->d_tile_counter, 0, (sample_log ? 64 : 1) * sizeof(unsigned int), st));
+    OMERF_CUDA(cudaMemsetAsync(tile_counter, 0, (sample_log ? OMERF_COUNTER_WORDS : 1) * sizeof(unsigned int), st));
     const unsigned int all_tiles = (unsigned int)(((W + 7) / 8) * ((H + 3) / 4)) * (unsigned int)n_views;
     if (tile_end == 0 || tile_end > all_tiles) tile_end = all_tiles; // 0: the whole batch
     if (tile_first >= tile_end) {
@@ -984,7 +897,7 @@ int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_
     const bool general = s->dev.soft_eps > 0.0f || s->dev.blk_shift != 0;
 #define OMERF_LAUNCH(SAMPLER, LOG, GENERAL)                                                                                 \
     omerf_march_kernel<SAMPLER, LOG, GENERAL><<<grid, 32 * OMERF_WARPS, 0, st>>>(                                          \
-        s->dev, d_cams, n_views, W, H, out_rgb, out_n, s->d_tile_counter, sample_log, log_capacity, tile_first, tile_end)
+        s->dev, d_cams, n_views, W, H, out_rgb, out_n, tile_counter, sample_log, log_capacity, tile_first, tile_end)
 #define OMERF_LAUNCH2(SAMPLER, LOG)                \
     if (general) OMERF_LAUNCH(SAMPLER, LOG, true); \
     else OMERF_LAUNCH(SAMPLER, LOG, false)

@@ -71,6 +71,12 @@ def test_invalid_arguments_are_rejected_before_touching_cuda(omerf):
         assert not out.value
     d, keep = make_desc(sc, sampler=1)          # grid sampler needs occ_n
     assert L.omerf_scene_create(C.byref(d), C.byref(out)) == -1
+    # 8(f) options that are defined by the slab need the occupancy-plane sampler: the grid sampler's voxels are a superset
+    sg = synth.custom_scene(occ_n=(8, 8, 8))
+    for kw, word in (({"grid_block": 4}, "grid_block"), ({"soft_eps": 0.5}, "soft_eps")):
+        d, keep = make_desc(sg, sampler=1, **kw)
+        assert L.omerf_scene_create(C.byref(d), C.byref(out)) == -1
+        assert word in L.omerf_last_error().decode() and not out.value
     assert L.omerf_render(None, None, 1, 4, 4, None, None, None) == -1
     assert L.omerf_render_host(None, None, 1, 4, 4, None, None, None) == -1
     L.omerf_scene_destroy(None)                  # no-op
