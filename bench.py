@@ -12,9 +12,14 @@ value   = Mpixels/s, whole job (all ranks), scene resident in HBM, device-timed 
           launching stream; L2 is flushed between timed steps (the flush is outside the event pairs).
 e2e     = the same through omerf_render_host: cameras from host memory, rgb + counts copied back to pinned
           host memory inside the timed region.
-roofline= march kernel: algorithmic bytes (168 B per sample + 16 B per pixel) / launch duration
-          against the measured HBM copy rate in MEASURED_PEAKS.json.
+roofline= march kernel against the BINDING ceiling of SURVEY 8(d) ("the smallest ceiling is the roofline"): the gather
+          rate calibrated live by omerf_gather_probe on the same frame and layout (requested texel bytes per second);
+gather_vs_hbm = algorithmic bytes (168 B per sample + 16 B per pixel) / launch duration against the measured
+          HBM copy rate in MEASURED_PEAKS.json; issue = executed lane-operations (ncu capture, cited) against the issue peak.
+parity  = element-wise comparison of the timed frame with the oracle's render of the same run (outside the timed region).
 cpu_baseline = the CPU oracle as it stands on this box's host cores, on a bounded sample of the same frame.
+--gpus N starts N ranks itself (torchrun) when it is not already running under one; N > 1 adds "strong": the batch
+          partitioned across the ranks by samples (paper_2404_09531_b200/partition.py), beside the weak-scaling replicas.
 """
 from __future__ import annotations
 
@@ -36,10 +41,11 @@ import synth  # noqa: E402
 
 BYTES_PER_SAMPLE = 168   # 20 texels x 8 B (64 B grid + 96 B planes) + one (z_min, z_max) pair of 8 B
 BYTES_PER_PIXEL = 16     # 12 B rgb + 4 B sample count written
-OPS_PER_SAMPLE = 450      # lane-operations per sample (extract, interpolate, activate, composite)
-OPS_PER_PIXEL = 1500      # ray setup, traversal, 883-MAC MLP
-ALU_PEAK_TOPS = 148 * 128 * 1.965e9 / 1e12   # B200: SMs x fp32/int lanes x max SM clock
-NCU_DRAM_TRAFFIC = {(1, "plane"): 96_949_760 + 13_321_472}   # bytes per launch, profiles/r01_march_kernel.md
+TEXEL_BYTES_PER_SAMPLE = 160   # what the gather requests: 20 texels x 8 B
+# Figures of ONE march-kernel launch on configs[1] from the committed `ncu --set full` capture (profiles/r02_march_kernel.md,
+# which names the command and the commit it was taken at); cited constants, not measured by this run:
+NCU_CAPTURE = {"profile": "profiles/r02_march_kernel.md", "commit": "see profile",
+               "dram_bytes": None, "warp_instructions": None, "lanes_per_instruction": None}
 
 
 def workload_name(cfg: int) -> str:
@@ -180,6 +186,100 @@ def aggregate_throughput(units_per_rank_step: float, steps: int, world: int, max
     return world * units_per_rank_step * steps / (max_total_ms / 1e3)
 
 
+def gather_shares(plans, rank, my_rgb, my_n, n_views, H, W, device):
+    """Optional last step of SURVEY 8(e): every rank's share is sent to rank 0 (peer copy over NVLink under NCCL, plain
+    sockets under gloo), which assembles the batch.  my_rgb / my_n: this rank's share as torch tensors on `device` -
+    mode "views": [len(views)][H][W][3] and [len(views)][H][W]; mode "rows": [rows][W][3] and [rows][W] for the flattened
+    pixel rows of its band.  Returns (rgb, nsamples) on rank 0, None elsewhere."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2404_09531_b200 import partition
+    if rank != 0:
+        if my_n.numel():
+            dist.send(my_rgb.contiguous(), 0)
+            dist.send(my_n.contiguous(), 0)
+        return None
+    rgb = torch.zeros((n_views, H, W, 3), dtype=my_rgb.dtype, device=device)
+    ns = torch.zeros((n_views, H, W), dtype=my_n.dtype, device=device)
+    seen = np.zeros(n_views * H, dtype=np.int32)
+    for plan in plans:
+        if plan.mode == "views":
+            shape_rgb, shape_n = (len(plan.views), H, W, 3), (len(plan.views), H, W)
+        else:
+            r0, r1 = partition.pixel_row_range(plan, H)
+            shape_rgb, shape_n = (r1 - r0, W, 3), (r1 - r0, W)
+        if plan.rank == 0:
+            p_rgb, p_n = my_rgb, my_n
+        else:
+            p_rgb = torch.empty(shape_rgb, dtype=my_rgb.dtype, device=device)
+            p_n = torch.empty(shape_n, dtype=my_n.dtype, device=device)
+            if p_n.numel():
+                dist.recv(p_rgb, plan.rank)
+                dist.recv(p_n, plan.rank)
+        if plan.mode == "views":
+            for i, v in enumerate(plan.views):
+                rgb[v], ns[v] = p_rgb[i], p_n[i]
+                seen[v * H:(v + 1) * H] += 1
+        else:
+            rgb.view(n_views * H, W, 3)[r0:r1] = p_rgb
+            ns.view(n_views * H, W)[r0:r1] = p_n
+            seen[r0:r1] += 1
+    assert np.all(seen == 1), "every pixel row must be rendered by exactly one rank"
+    return rgb, ns
+
+
+def run_partitioned(omerf, h, cams, W, H, prev_n, world, rank, steps, timed, barrier, stream):
+    """Strong scaling: the batch partitioned across the ranks by the previous frame's sample counts, timed
+    like the main region (L2 flushed, CUDA events, max over ranks); then the shares are gathered on rank 0 and compared
+    bit for bit with this rank's own full render."""
+    import torch
+
+    from paper_2404_09531_b200 import partition
+    n_views = cams.shape[0]
+    prev = prev_n.cpu().numpy().view(np.uint32)
+    plans = partition.make_plans(prev, world)
+    plan = plans[rank]
+    full_rgb = torch.empty((n_views, H, W, 3), dtype=torch.float32, device="cuda")
+    full_n = torch.zeros((n_views, H, W), dtype=torch.int32, device="cuda")
+    if plan.mode == "views":
+        my_cams = cams[plan.views]
+        my_rgb = torch.empty((len(plan.views), H, W, 3), dtype=torch.float32, device="cuda")
+        my_n = torch.empty((len(plan.views), H, W), dtype=torch.int32, device="cuda")
+
+        def step():
+            if len(plan.views):
+                omerf.render(h, my_cams, W, H, my_rgb, my_n, stream=stream)
+    else:
+        def step():
+            omerf.render_tiles(h, cams, W, H, full_rgb, full_n, plan.tile_first, plan.tile_end, stream=stream)
+    for _ in range(3):
+        step()
+    barrier()
+    ms = timed(steps, True, step)
+    barrier()
+    if plan.mode == "rows":
+        r0, r1 = partition.pixel_row_range(plan, H)
+        my_rgb, my_n = full_rgb.view(n_views * H, W, 3)[r0:r1], full_n.view(n_views * H, W)[r0:r1]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    got = gather_shares(plans, rank, my_rgb, my_n, n_views, H, W, "cuda")
+    e1.record(stream)
+    barrier()
+    total = max_over_ranks([float(np.sum(ms))], world, "cuda")[0]
+    out = {"scaling": "strong", "mode": plan.mode, "ms_per_step": total / steps, "frames_per_s": n_views * steps / (total / 1e3),
+           "mpixels_s": n_views * W * H * steps / (total / 1e3) / 1e6, "cost_imbalance": plan.imbalance,
+           "sample_imbalance": plan.sample_imbalance, "samples_per_rank": [p.samples for p in plans],
+           "gather_to_rank0_ms": e0.elapsed_time(e1), "parallelism": f"scene replicated x{world}, batch partitioned by {plan.mode}"}
+    if rank == 0:
+        ref_rgb = torch.empty_like(got[0])
+        ref_n = torch.empty_like(got[1])
+        omerf.render(h, cams, W, H, ref_rgb, ref_n, stream=stream)
+        torch.cuda.synchronize()
+        out["stitched_equals_single_rank"] = bool(torch.equal(got[1], ref_n) and torch.equal(got[0], ref_rgb))
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -201,7 +301,7 @@ def run_ours(args):
     W, H = synth.config_resolution(cfg)
     n_views = cams.shape[0]
     sampler = omerf.SAMPLER_GRID if args.sampler == "grid" else omerf.SAMPLER_PLANE
-    h = omerf.scene_create(scene, sampler=sampler, soft_eps=args.soft_eps, grid_block=args.grid_block)
+    h = omerf.scene_create(scene, sampler=sampler, soft_eps=args.soft_eps, grid_block=args.grid_block, lowz_bake=args.lowz)
     info = omerf.scene_info(h)
     out_rgb = torch.empty((n_views, H, W, 3), dtype=torch.float32, device="cuda")
     out_n = torch.empty((n_views, H, W), dtype=torch.int32, device="cuda")
@@ -260,6 +360,12 @@ def run_ours(args):
     per_view = [int(x) for x in out_n.view(n_views, -1).sum(dim=1, dtype=torch.int64).tolist()]
     hist = torch.bincount(out_n.view(-1).clamp(max=63).to(torch.int64), minlength=64).tolist()   # samples/ray, last bin = 63+
 
+    # N > 1: the SAME batch partitioned across the ranks: by views or by bands of tile rows, balanced by the
+    # previous frame's sample counts; scene replicated, no collective on the data path; shares gathered on rank 0 afterwards
+    strong = None
+    if world > 1:
+        strong = run_partitioned(omerf, h, cams, W, H, out_n, world, rank, args.steps, timed, barrier, stream)
+
     # configs[4]: the same frame through the other sampler (binary occupancy grid + DDA), timed the same way
     ablation = None
     if cfg == 4 and rank == 0:
@@ -317,19 +423,20 @@ def run_ours(args):
         march_ms = total_ms / k                                  # one launch per step: the fused march kernel
         alg_bytes = samples * BYTES_PER_SAMPLE + pixels * BYTES_PER_PIXEL
         achieved = alg_bytes / (march_ms / 1e3) / 1e9
-        alu_ops = samples * OPS_PER_SAMPLE + pixels * OPS_PER_PIXEL
         cpu = None
         if not args.no_cpu_baseline:
             cpu = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=15.0, soft_eps=args.soft_eps, count_sectors=True)
-        # dram__bytes_read.sum + dram__bytes_write.sum of one march-kernel launch from the committed `ncu --set full`
-        # capture (profiles/r01_march_kernel.md); only the workload that was captured has a figure
-        traffic = NCU_DRAM_TRAFFIC.get((cfg, args.sampler)) if not (args.soft_eps or args.grid_block) else None
+        # figures of the committed ncu capture apply to the workload that was captured only
+        captured = cfg == 1 and args.sampler == "plane" and not (args.soft_eps or args.grid_block or args.lowz)
+        props = torch.cuda.get_device_properties(local)
+        issue_peak = props.multi_processor_count * 128 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12   # Tlane-op/s
         line = {
             "metric": "Mpixels/s", "value": aggregate_throughput(pixels, k, world, total_ms) / 1e6, "unit": "Mpixels/s", "n_gpus": world,
             "steps": k, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32 (u8 features, integer interpolation)",
             "data": "synthetic",
             "config": {"workload": workload_name(cfg), "views": n_views, "W": W, "H": H, "sampler": args.sampler, "soft_eps": args.soft_eps, "grid_block": args.grid_block,
+                       "lowz_bake": bool(args.lowz), "plane_bytes": info["plane_bytes"], "xz_band": info["xz_band"], "yz_band": info["yz_band"],
                        "grid_bytes": info["grid_bytes"], "grid_blocks": [info["grid_blocks_allocated"], info["grid_blocks_total"]],
                        "scene_device_bytes": info["device_bytes"], "l2": "flushed between timed steps (256 MiB fill, "
                        "outside the event pairs); scene 296 MiB > L2", "parallelism": f"replicated scene x{world}"},
@@ -345,25 +452,38 @@ def run_ours(args):
                     "h2d_bytes_per_step": int(cams.nbytes), "d2h_bytes_per_step": pixels * BYTES_PER_PIXEL,
                     "ms_per_step": total_e2e_ms / k, "wall_ms_per_step": wall_e2e * 1e3 / k},
             "gpu_launches": launches_per_step * k,
-            # the march kernel is bound by instruction issue, not by HBM (profiles/): lane-operations against the
-            # ALU peak DESIGN.md derives (148 SMs x 128 lanes x 1.965 GHz); the gather rate vs HBM is kept beside it
-            "roofline": {"bound": "alu", "kernel": "omerf_march_kernel", "achieved": alu_ops / (march_ms / 1e3) / 1e12,
-                         "peak": ALU_PEAK_TOPS, "unit": "Tlane-op/s", "frac": alu_ops / (march_ms / 1e3) / 1e12 / ALU_PEAK_TOPS,
-                         "traffic": traffic, "peak_source": "DESIGN.md 5.1: 148 SMs x 128 lanes x 1.965 GHz",
-                         "algorithmic_lane_ops_per_launch": alu_ops, "launch_ms": march_ms},
+            # filled in below: the binding ceiling is the gather rate calibrated live on this frame
+            "roofline": None,
             "gather_vs_hbm": {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
                               "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "fallback 6650 (of fallback)",
-                              "algorithmic_bytes_per_launch": alg_bytes},
+                              "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": march_ms,
+                              "traffic": NCU_CAPTURE["dram_bytes"] if captured else None, "traffic_source": NCU_CAPTURE["profile"]},
             "clocks": clk,
         }
         if probe and probe["samples"]:
             ceil_gs = probe["samples"] / probe["ms_frame_order"] / 1e6           # Gsamples/s, gather only, frame order
-            view0 = probe["samples"] / (march_ms / n_views) / 1e6 if n_views == 1 else world * samples * k / secs / 1e9 / world
-            line["gather_calibrated"] = {
-                "what": "omerf_gather_probe: 20 x 8-byte loads per sample of view 0, no arithmetic, L2 flushed",
-                "ceiling_gsamples_s": ceil_gs, "ceiling_gbs": ceil_gs * 160,
-                "scattered_gsamples_s": probe["samples"] / probe["ms_scattered"] / 1e6,
-                "march_gsamples_s": view0, "frac": view0 / ceil_gs}
+            view0 = probe["samples"] / (march_ms / n_views) / 1e6 if n_views == 1 else samples * k / secs / 1e9
+            # "the smallest ceiling is the roofline" - the L2/L1 gather rate, calibrated on this frame, this
+            # layout, this GPU, in this run: requested texel bytes per second of the march kernel against the gather-only replay
+            line["roofline"] = {
+                "bound": "gather (L2/L1 gather rate, SURVEY 8(d); calibrated live, not HBM)", "kernel": "omerf_march_kernel",
+                "achieved": view0 * TEXEL_BYTES_PER_SAMPLE, "peak": ceil_gs * TEXEL_BYTES_PER_SAMPLE, "unit": "GB/s",
+                "frac": view0 / ceil_gs, "traffic": NCU_CAPTURE["dram_bytes"] if captured else None,
+                "traffic_source": NCU_CAPTURE["profile"],
+                "peak_source": "omerf_gather_probe in this run: the frame's texel loads replayed with no arithmetic, one sample "
+                               "per thread, frame order, L2 flushed",
+                "march_gsamples_s": view0, "ceiling_gsamples_s": ceil_gs, "launch_ms": march_ms,
+                "scattered_gsamples_s": probe["samples"] / probe["ms_scattered"] / 1e6}
+            line["gather_calibrated"] = {"frac": view0 / ceil_gs, "ceiling_gsamples_s": ceil_gs, "march_gsamples_s": view0}
+        if captured and NCU_CAPTURE["warp_instructions"]:
+            lane_ops = NCU_CAPTURE["warp_instructions"] * NCU_CAPTURE["lanes_per_instruction"]
+            line["issue"] = {"bound": "alu", "achieved": lane_ops / (march_ms / 1e3) / 1e12, "peak": issue_peak, "unit": "Tlane-op/s",
+                             "frac": lane_ops / (march_ms / 1e3) / 1e12 / issue_peak,
+                             "what": "executed lane-operations of one launch (smsp__inst_executed.sum x lanes per instruction, "
+                                     "ncu capture) / this run's launch time, against SMs x 128 lanes x max SM clock of this device",
+                             "source": NCU_CAPTURE["profile"], "commit": NCU_CAPTURE["commit"]}
+        if strong is not None:
+            line["strong"] = strong
         if ablation is not None:
             line["ablation"] = ablation
         if cpu is not None:
@@ -454,9 +574,19 @@ def main():
     ap.add_argument("--sampler", default="plane", choices=["plane", "grid"])
     ap.add_argument("--soft-eps", type=float, default=0.0, help="SURVEY 8(f).2: soft occupancy (Eq. 6-8) buffer height; 0 = binary mask")
     ap.add_argument("--grid-block", type=int, default=0, help="SURVEY 8(f).1: store V as sparse blocks of this edge (0 = dense)")
+    ap.add_argument("--lowz", action="store_true", help="SURVEY 8(f).1: low-z bake of the xz / yz planes (PAPER.md:186)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workload", default="render", choices=["render", "smoothness"])
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        # not under a launcher yet: start one rank per GPU ourselves (same command line), NCCL over NVLink for the barriers
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        raise SystemExit(subprocess.call(cmd))
     if args.workload == "smoothness" and args.impl == "ours":
         run_smoothness(args)
     elif args.impl == "reference":

@@ -66,6 +66,11 @@ typedef struct {
                            holding a voxel that a sample inside the slab can touch are kept (R24); the
                            rendered images are identical to the dense layout's.  Sampler PLANE only: the grid sampler's
                            voxels are a superset of the slab (OMERF_ERR_INVALID otherwise). */
+    int32_t lowz_bake;  /* 0: plane_xz / plane_yz are stored whole.  1: low-z bake ("a texture map with high
+                           resolution in the xy direction and low resolution in the z direction, according to the upper
+                           and lower bounds of the occupancy plane"): only the band of z rows that a sample inside
+                           [min z_min, max z_max] of the occupancy plane can touch is uploaded and stored (DESIGN.md
+                           R27); the rendered images are identical.  Sampler PLANE only. */
 } omerf_scene_desc;
 
 /* Pinhole camera, world frame. */
@@ -82,6 +87,9 @@ typedef struct {
     uint64_t grid_bytes;        /* device bytes of V: dense array, or atlas + block table */
     uint64_t grid_blocks_total; /* sparse layout: blocks of the block grid, else 0 */
     uint64_t grid_blocks_allocated; /* sparse layout: blocks kept (occupancy ratio = allocated / total, cf. Table 5) */
+    uint64_t plane_bytes;       /* device bytes of the three planes (cf. the VRAM column of Table 3) */
+    int32_t xz_band[2], yz_band[2]; /* first and last z row of plane_xz / plane_yz that is stored (the whole plane without
+                                       lowz_bake) */
 } omerf_scene_info;
 
 /* S0 + S1 (+ S10 derivation): validate, upload, re-lay out for gathers, build the min/max pyramid
@@ -105,6 +113,15 @@ int omerf_scene_create(const omerf_scene_desc *desc /*HOST*/, omerf_scene **out_
  * (cudaDeviceSynchronize + cudaMalloc inside the call); calls after that warm-up do not allocate. */
 int omerf_render(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W, int H,
                  float *out_rgb /*DEVICE*/, uint32_t *out_nsamples /*DEVICE*/, void *stream);
+
+/* A share of the same work (pixels and views are independent, the scene is read-only, so a batch is
+ * partitioned across GPUs with no exchange): renders only the 8x4-pixel tiles [tile_first, tile_end) of the batch, tiles
+ * numbered view-major, then row-major inside a view (tiles_x = ceil(W/8), tiles_y = ceil(H/4)).  out_rgb / out_nsamples
+ * are the FULL batch buffers; pixels of other tiles are not written.  tile_first <= tile_end <= n_views*tiles_x*tiles_y
+ * (else OMERF_ERR_INVALID); an empty range is a no-op.  Everything else as omerf_render. */
+int omerf_render_tiles(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W, int H,
+                       float *out_rgb /*DEVICE*/, uint32_t *out_nsamples /*DEVICE*/, uint32_t tile_first,
+                       uint32_t tile_end, void *stream);
 
 /* Same path with HOST outputs (pinned or pageable): renders into scene-owned device scratch on
  * `stream` in bands of whole tile rows, copies each band back on a scene-owned second stream while the next

@@ -24,6 +24,7 @@ from .binding import (  # noqa: F401
     pyramid_level,
     render,
     render_host,
+    render_tiles,
     scene_create,
     scene_destroy,
     scene_info,

@@ -22,7 +22,7 @@ SAMPLER_PLANE = 0
 SAMPLER_GRID = 1
 
 EXPORTS = (
-    "omerf_scene_create", "omerf_render", "omerf_render_host", "omerf_gather_probe", "omerf_mlp_smoothness", "omerf_heatmap",
+    "omerf_scene_create", "omerf_render", "omerf_render_tiles", "omerf_render_host", "omerf_gather_probe", "omerf_mlp_smoothness", "omerf_heatmap",
     "omerf_last_launch_count",
     "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield", "omerf_scene_get_block_table",
     "omerf_scene_destroy", "omerf_last_error", "omerf_version",
@@ -41,14 +41,15 @@ class SceneDesc(C.Structure):
         ("W0", _f32p), ("b0", _f32p), ("W1", _f32p), ("b1", _f32p), ("W2", _f32p), ("b2", _f32p),
         ("step", C.c_float), ("t_stop", C.c_float), ("bg", C.c_float * 3),
         ("sampler", C.c_int32), ("occ_n", C.c_int32 * 3),
-        ("soft_eps", C.c_float), ("grid_block", C.c_int32),
+        ("soft_eps", C.c_float), ("grid_block", C.c_int32), ("lowz_bake", C.c_int32),
     ]
 
 
 class SceneInfo(C.Structure):
     _fields_ = [("device_bytes", C.c_uint64), ("pyramid_levels", C.c_int32), ("sampler", C.c_int32),
                 ("occ_bits_set", C.c_uint64), ("grid_bytes", C.c_uint64), ("grid_blocks_total", C.c_uint64),
-                ("grid_blocks_allocated", C.c_uint64)]
+                ("grid_blocks_allocated", C.c_uint64), ("plane_bytes", C.c_uint64),
+                ("xz_band", C.c_int32 * 2), ("yz_band", C.c_int32 * 2)]
 
 
 class GatherProbeResult(C.Structure):
@@ -76,6 +77,8 @@ def load_library() -> C.CDLL:
     L.omerf_scene_create.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
     L.omerf_render.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
     L.omerf_render_host.argtypes = L.omerf_render.argtypes
+    L.omerf_render_tiles.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_uint32,
+                                     C.c_uint32, C.c_void_p]
     L.omerf_gather_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
                                      C.POINTER(GatherProbeResult)]
     L.omerf_mlp_smoothness.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
@@ -102,7 +105,7 @@ def _np(a, dt):
     return np.ascontiguousarray(a, dtype=dt)
 
 
-def make_desc(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, grid_block: int = 0):
+def make_desc(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, grid_block: int = 0, lowz_bake: bool = False):
     """Fill an omerf_scene_desc from an object with synth.Scene's attributes. Returns (desc, keepalive)."""
     d = SceneDesc()
     keep = []
@@ -136,6 +139,7 @@ def make_desc(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, grid_b
     d.sampler = sampler
     d.soft_eps = soft_eps
     d.grid_block = grid_block
+    d.lowz_bake = int(lowz_bake)
     d.occ_n[:] = scene.occ_n
     return d, keep
 
@@ -159,7 +163,8 @@ class SceneHandle:
             pass
 
 
-def scene_create(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, grid_block: int = 0) -> SceneHandle:
+def scene_create(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, grid_block: int = 0,
+                 lowz_bake: bool = False) -> SceneHandle:
     """omerf_scene_create: upload + re-layout + pyramid (+ bitfield) on the current CUDA device."""
     import torch
     if not torch.cuda.is_available():
@@ -167,7 +172,7 @@ def scene_create(scene, sampler: int = SAMPLER_PLANE, soft_eps: float = 0.0, gri
     torch.cuda.init()
     torch.cuda.current_stream()          # make sure torch's primary context is current
     L = load_library()
-    d, keep = make_desc(scene, sampler, soft_eps, grid_block)
+    d, keep = make_desc(scene, sampler, soft_eps, grid_block, lowz_bake)
     out = C.c_void_p()
     _check(L.omerf_scene_create(C.byref(d), C.byref(out)), "omerf_scene_create")
     del keep
@@ -202,6 +207,21 @@ def render(h: SceneHandle, cameras, W: int, H: int, out_rgb=None, out_nsamples=N
     st = torch.cuda.current_stream() if stream is None else stream
     _check(load_library().omerf_render(h.ptr, cams.ctypes.data, n, W, H, out_rgb.data_ptr(), out_nsamples.data_ptr(),
                                        st.cuda_stream), "omerf_render")
+    return out_rgb, out_nsamples
+
+
+def render_tiles(h: SceneHandle, cameras, W: int, H: int, out_rgb, out_nsamples, tile_first: int, tile_end: int, stream=None):
+    """omerf_render_tiles: only the 8x4 tiles [tile_first, tile_end) of the batch are rendered into the FULL batch
+    buffers (DEVICE torch tensors); asynchronous."""
+    import torch
+    cams = _cams(cameras)
+    n = cams.shape[0]
+    assert out_rgb.is_cuda and out_rgb.is_contiguous() and out_rgb.dtype == torch.float32 and out_rgb.numel() == n * H * W * 3
+    assert out_nsamples.is_cuda and out_nsamples.is_contiguous() and out_nsamples.element_size() == 4 \
+        and out_nsamples.numel() == n * H * W
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(load_library().omerf_render_tiles(h.ptr, cams.ctypes.data, n, W, H, out_rgb.data_ptr(), out_nsamples.data_ptr(),
+                                             int(tile_first), int(tile_end), st.cuda_stream), "omerf_render_tiles")
     return out_rgb, out_nsamples
 
 
@@ -278,7 +298,8 @@ def scene_info(h: SceneHandle) -> dict:
     _check(load_library().omerf_scene_get_info(h.ptr, C.byref(info)), "omerf_scene_get_info")
     return {"device_bytes": int(info.device_bytes), "pyramid_levels": int(info.pyramid_levels),
             "sampler": int(info.sampler), "occ_bits_set": int(info.occ_bits_set), "grid_bytes": int(info.grid_bytes),
-            "grid_blocks_total": int(info.grid_blocks_total), "grid_blocks_allocated": int(info.grid_blocks_allocated)}
+            "grid_blocks_total": int(info.grid_blocks_total), "grid_blocks_allocated": int(info.grid_blocks_allocated),
+            "plane_bytes": int(info.plane_bytes), "xz_band": tuple(info.xz_band), "yz_band": tuple(info.yz_band)}
 
 
 def pyramid_level(h: SceneHandle, level: int):

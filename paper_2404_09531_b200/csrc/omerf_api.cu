@@ -109,6 +109,8 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
     // the sparse-block bake (R24) keeps what a sample INSIDE THE SLAB can touch; the grid sampler's voxels are a superset of the
     // slab (R18), so its samples may have corners in blocks that were not kept
     if (d->grid_block != 0 && d->sampler != OMERF_SAMPLER_PLANE) return invalid("grid_block needs the occupancy-plane sampler");
+    if (d->lowz_bake != 0 && d->lowz_bake != 1) return invalid("lowz_bake must be 0 or 1");
+    if (d->lowz_bake && d->sampler != OMERF_SAMPLER_PLANE) return invalid("lowz_bake needs the occupancy-plane sampler");
     if (d->sampler == OMERF_SAMPLER_GRID)
         for (int i = 0; i < 3; i++)
             if (d->occ_n[i] < 1) return invalid("occ_n must be >= 1 for the grid sampler");
@@ -160,30 +162,74 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
 
     int rc = OMERF_OK;
     float *d_lo = nullptr, *d_up = nullptr;
+    void *d_raw = nullptr; // raw texels of the array being laid out
     uint64_t tmp = 0;
     size_t hf_bytes = (size_t)v.Mx * v.My * sizeof(float);
     do {
-        // S0: features.  8 channels per texel -> one 8-byte word; row-major order kept.
-        if ((rc = upload(&s->d_grid, d->grid, (size_t)v.G[0] * v.G[1] * v.G[2] * 8, &s->device_bytes))) break;
-        if ((rc = upload(&s->d_pxy, d->plane_xy, (size_t)v.xy_n[0] * v.xy_n[1] * 8, &s->device_bytes))) break;
-        if ((rc = upload(&s->d_pxz, d->plane_xz, (size_t)v.xz_n[0] * v.xz_n[1] * 8, &s->device_bytes))) break;
-        if ((rc = upload(&s->d_pyz, d->plane_yz, (size_t)v.yz_n[0] * v.yz_n[1] * 8, &s->device_bytes))) break;
-        v.grid = (const uint2 *)s->d_grid;
-        v.pxy = (const uint2 *)s->d_pxy;
-        v.pxz = (const uint2 *)s->d_pxz;
-        v.pyz = (const uint2 *)s->d_pyz;
-        // S0: deferred-MLP weights -> tensor-core fragment order, tf32 hi/lo split (device kernel)
-        if ((rc = omerf_launch_mlp_pack(s, d, 0))) break;
         // S1: min/max pyramid of the two height fields, built on the device
         if ((rc = upload((void **)&d_lo, d->h_lo, hf_bytes, &tmp))) break;
         if ((rc = upload((void **)&d_up, d->h_up, hf_bytes, &tmp))) break;
         if ((rc = omerf_launch_pyramid(s, d_lo, d_up, 0))) break;
-        // 8(f).1: sparse-block layout of V baked from the occupancy plane (replaces the dense array)
-        s->grid_bytes = (uint64_t)v.G[0] * v.G[1] * v.G[2] * 8;
-        if (d->grid_block) {
-            if ((rc = omerf_bake_sparse_grid(s, &s->d_grid, d->grid_block, 0))) break;
-            s->device_bytes = s->device_bytes - (uint64_t)v.G[0] * v.G[1] * v.G[2] * 8 + s->grid_bytes;
+        // 8(f).1: z band of the xz / yz planes kept by the low-z bake (the whole plane without it)
+        s->band[0] = s->band[2] = 0;
+        s->band[1] = v.xz_n[1] - 1;
+        s->band[3] = v.yz_n[1] - 1;
+        if (d->lowz_bake && (rc = omerf_lowz_band(s, d_lo, d_up, v.xz_n[1], v.yz_n[1], s->band, 0))) break;
+        v.xz_zoff = s->band[0];
+        v.xz_rows = s->band[1] - s->band[0] + 1;
+        v.yz_zoff = s->band[2];
+        v.yz_rows = s->band[3] - s->band[2] + 1;
+        // S0: features.  8 channels per texel = 8 bytes; stored as 16-byte entries of two texels adjacent along the fastest
+        // axis (omerf_build.cu: pair_layout_kernel).  Only the kept z band of xz / yz is uploaded at all.
+        struct {
+            const uint8_t *host;
+            size_t rows;
+            int n_host, first, n;
+            void **dst;
+        } arr[4] = {{d->grid, (size_t)v.G[0] * v.G[1], v.G[2], 0, v.G[2], &s->d_grid},
+                    {d->plane_xy, (size_t)v.xy_n[0], v.xy_n[1], 0, v.xy_n[1], &s->d_pxy},
+                    {d->plane_xz, (size_t)v.xz_n[0], v.xz_n[1], v.xz_zoff, v.xz_rows, &s->d_pxz},
+                    {d->plane_yz, (size_t)v.yz_n[0], v.yz_n[1], v.yz_zoff, v.yz_rows, &s->d_pyz}};
+        for (int a = 0; a < 4 && rc == OMERF_OK; a++) {
+            const size_t raw_bytes = arr[a].rows * arr[a].n * 8;
+            cudaError_t e = cudaMalloc(&d_raw, raw_bytes);
+            if (e == cudaSuccess)
+                e = cudaMemcpy2D(d_raw, (size_t)arr[a].n * 8, arr[a].host + (size_t)arr[a].first * 8, (size_t)arr[a].n_host * 8,
+                                 (size_t)arr[a].n * 8, arr[a].rows, cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) {
+                rc = omerf_cuda_fail(e, "feature upload");
+                break;
+            }
+            if (a == 0 && d->grid_block) {
+                // 8(f).1: sparse-block layout of V baked from the occupancy plane (takes the raw texels, frees them)
+                s->d_grid = d_raw;
+                d_raw = nullptr;
+                rc = omerf_bake_sparse_grid(s, &s->d_grid, d->grid_block, 0);
+                s->device_bytes += s->grid_bytes;
+                continue;
+            }
+            if ((e = cudaMalloc(arr[a].dst, raw_bytes * 2)) != cudaSuccess) {
+                rc = omerf_cuda_fail(e, "feature layout");
+                break;
+            }
+            if ((rc = omerf_launch_pair_layout(d_raw, *arr[a].dst, arr[a].rows, arr[a].n, 0))) break;
+            if ((e = cudaDeviceSynchronize()) != cudaSuccess) {
+                rc = omerf_cuda_fail(e, "feature layout");
+                break;
+            }
+            cudaFree(d_raw);
+            d_raw = nullptr;
+            s->device_bytes += raw_bytes * 2;
+            if (a == 0) s->grid_bytes = raw_bytes * 2;
+            else s->plane_bytes += raw_bytes * 2;
         }
+        if (rc) break;
+        if (!d->grid_block) v.grid = (const uint4 *)s->d_grid;
+        v.pxy = (const uint4 *)s->d_pxy;
+        v.pxz = (const uint4 *)s->d_pxz;
+        v.pyz = (const uint4 *)s->d_pyz;
+        // S0: deferred-MLP weights -> tensor-core fragment order, tf32 hi/lo split (device kernel)
+        if ((rc = omerf_launch_mlp_pack(s, d, 0))) break;
         // S10: occupancy bitfield + its mip chain, derived on the device from the slab
         if (d->sampler == OMERF_SAMPLER_GRID) {
             for (int i = 0; i < 3; i++) {
@@ -222,6 +268,7 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
     } while (0);
     cudaFree(d_lo);
     cudaFree(d_up);
+    cudaFree(d_raw);
     if (rc != OMERF_OK) {
         free_scene(s);
         return rc;
@@ -306,6 +353,18 @@ extern "C" int omerf_render(const omerf_scene *s, const omerf_camera *cameras, i
 {
     if (s) s->last_launches = 0;
     return render_impl(s, cameras, n_views, W, H, out_rgb, out_nsamples, stream, 0, 0, nullptr);
+}
+
+extern "C" int omerf_render_tiles(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
+                                  float *out_rgb, uint32_t *out_nsamples, uint32_t tile_first, uint32_t tile_end, void *stream)
+{
+    if (W > 0 && H > 0 && n_views >= 0) {
+        const unsigned long long all = (unsigned long long)((W + 7) / 8) * ((H + 3) / 4) * (unsigned long long)n_views;
+        if (tile_first > tile_end || tile_end > all) return invalid("tile range must satisfy first <= end <= tiles of the batch");
+    }
+    if (s) s->last_launches = 0;
+    if (tile_first == tile_end && s && cameras && out_rgb && out_nsamples && W > 0 && H > 0 && n_views >= 0) return OMERF_OK;
+    return render_impl(s, cameras, n_views, W, H, out_rgb, out_nsamples, stream, tile_first, tile_end, nullptr);
 }
 
 extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
@@ -484,6 +543,11 @@ extern "C" int omerf_scene_get_info(const omerf_scene *s, omerf_scene_info *out)
     out->grid_bytes = s->grid_bytes;
     out->grid_blocks_total = s->blocks_total;
     out->grid_blocks_allocated = s->blocks_allocated;
+    out->plane_bytes = s->plane_bytes;
+    for (int i = 0; i < 2; i++) {
+        out->xz_band[i] = s->band[i];
+        out->yz_band[i] = s->band[2 + i];
+    }
     return OMERF_OK;
 }
 

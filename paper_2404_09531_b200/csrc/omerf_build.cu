@@ -8,6 +8,112 @@
 
 #include "omerf_device.cuh"
 
+// ------------------------------------------------------------------------------------------ S0: gather layout
+// Every feature array is stored as ENTRIES of two texels adjacent along its fastest axis:
+//     dst[r][j] = (src[r][j], src[r][min(j + 1, n - 1)]),   8 + 8 = 16 bytes,
+// so that the two taps a bilinear / trilinear footprint takes along that axis (z for V, the second axis for the planes)
+// arrive with ONE 16-byte load instead of two 8-byte loads: 10 gathers per sample instead of 20 for twice the memory
+// (PAPER.md:186 stores the features as textures; SURVEY 8(a) S0 "re-lay out for gathers").  The clamp reproduces
+// clamp-to-edge addressing (R10) at the last texel; the first texel needs none (omerf_render.cu: axis_tap).
+__global__ void pair_layout_kernel(const uint2 *__restrict__ src, uint4 *__restrict__ dst, unsigned long long rows, int n)
+{
+    const unsigned long long total = rows * (unsigned long long)n;
+    for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+         e += (unsigned long long)gridDim.x * blockDim.x) {
+        const int j = (int)(e % (unsigned long long)n);
+        const uint2 a = src[e], b = src[j + 1 < n ? e + 1 : e];
+        dst[e] = make_uint4(a.x, a.y, b.x, b.y);
+    }
+}
+
+int omerf_launch_pair_layout(const void *d_src, void *d_dst, unsigned long long rows, int n, cudaStream_t st)
+{
+    if (rows == 0 || n <= 0) return OMERF_OK;
+    const unsigned long long total = rows * (unsigned long long)n;
+    const unsigned int blocks = (unsigned int)((total + 255) / 256 < (1u << 20) ? (total + 255) / 256 : (1u << 20));
+    pair_layout_kernel<<<blocks, 256, 0, st>>>((const uint2 *)d_src, (uint4 *)d_dst, rows, n);
+    OMERF_CUDA(cudaGetLastError());
+    return OMERF_OK;
+}
+
+// ------------------------------------------------------------------------------------------ low-z triplane bake
+// "For the 2D triplane, we employ a texture map with high resolution in the xy direction and low resolution
+// in the z direction, according to the upper and lower bounds of the occupancy plane."  DESIGN.md R27: the xz and yz
+// planes keep the band of z rows a bilinear lookup can touch for z in [min z_min, max z_max] over the non-empty columns
+// of P_o (clipped to the box, widened by 1/64 texel).  Step 1: the two bounds (ordered-integer keys, atomics);
+// step 2: the band of each plane, in double with one rounding per operation.
+__device__ __forceinline__ unsigned int lowz_key(float f)
+{
+    const unsigned int b = __float_as_uint(f);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u); // monotone in f
+}
+
+__device__ __forceinline__ float lowz_unkey(unsigned int k) { return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k); }
+
+__global__ void lowz_bounds_kernel(const float *__restrict__ lo, const float *__restrict__ up, int n, unsigned int *__restrict__ keys)
+{
+    unsigned int kmin = 0xffffffffu, kmax = 0u;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float a = lo[i], b = up[i];
+        if (a <= b) { // non-empty column (R17)
+            kmin = min(kmin, lowz_key(a));
+            kmax = max(kmax, lowz_key(b));
+        }
+    }
+    kmin = __reduce_min_sync(0xffffffffu, kmin);
+    kmax = __reduce_max_sync(0xffffffffu, kmax);
+    if ((threadIdx.x & 31) == 0) {
+        atomicMin(keys + 0, kmin);
+        atomicMax(keys + 1, kmax);
+    }
+}
+
+__global__ void lowz_band_kernel(const unsigned int *__restrict__ keys, float Zf, int n_xz, int n_yz, int *__restrict__ band)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int N[2] = {n_xz, n_yz};
+    const double Z = (double)Zf;
+    double zl = 0.0, zh = -1.0;
+    if (keys[0] <= keys[1]) { // some column is non-empty
+        zl = (double)lowz_unkey(keys[0]);
+        zh = (double)lowz_unkey(keys[1]);
+        if (zl < 0.0) zl = 0.0;
+        if (zh > Z) zh = Z;
+    }
+    for (int p = 0; p < 2; p++) {
+        int b0 = 0, b1 = 0; // nothing can be fetched: one row is kept so that the array is not empty
+        if (zl <= zh) {
+            const double qa = __dsub_rn(__ddiv_rn(__dmul_rn(zl, (double)N[p]), Z), 0.515625); // - 1/2 - 1/64
+            const double qb = __dsub_rn(__ddiv_rn(__dmul_rn(zh, (double)N[p]), Z), 0.484375); // - 1/2 + 1/64
+            const long long a = (long long)floor(qa), b = (long long)floor(qb) + 1;
+            b0 = (int)(a < 0 ? 0 : a);
+            b1 = (int)(b > N[p] - 1 ? N[p] - 1 : b);
+        }
+        band[2 * p] = b0;
+        band[2 * p + 1] = b1;
+    }
+}
+
+// band[4] (HOST) = first/last kept z row of plane xz, then of plane yz.  Synchronises `st`.
+int omerf_lowz_band(const omerf_scene *s, const float *d_lo, const float *d_up, int n_xz, int n_yz, int *band, cudaStream_t st)
+{
+    unsigned int *d_keys = nullptr;
+    OMERF_CUDA(cudaMalloc((void **)&d_keys, 2 * sizeof(unsigned int) + 4 * sizeof(int)));
+    const unsigned int init[2] = {0xffffffffu, 0u};
+    cudaError_t e = cudaMemcpyAsync(d_keys, init, sizeof init, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        const int n = s->dev.Mx * s->dev.My;
+        lowz_bounds_kernel<<<(n + 1023) / 1024 < 1184 ? (n + 1023) / 1024 : 1184, 256, 0, st>>>(d_lo, d_up, n, d_keys);
+        lowz_band_kernel<<<1, 32, 0, st>>>(d_keys, s->dev.box[2], n_xz, n_yz, (int *)(d_keys + 2));
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(band, d_keys + 2, 4 * sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_keys);
+    if (e != cudaSuccess) return omerf_cuda_fail(e, "low-z band");
+    return OMERF_OK;
+}
+
 // ------------------------------------------------------------------------------------------ pyramid
 __global__ void pyr_level0_kernel(const float *__restrict__ lo, const float *__restrict__ up,
                                   float2 *__restrict__ out, int n)

@@ -24,16 +24,20 @@ struct DevScene {
     int n_levels;
     const float2 *pyr;     // all levels, (min of h_lo, max of h_up) per node, [nx][ny] row-major
     int lvl_off[OMERF_MAX_LEVELS], lvl_nx[OMERF_MAX_LEVELS], lvl_ny[OMERF_MAX_LEVELS];
-    // features: 8 uint8 channels per texel = one uint2
+    // features: 8 uint8 channels per texel = 8 bytes; every array ENTRY is a pair of texels adjacent along the array's
+    // fastest axis, (t[i], t[min(i+1, N-1)]) = one 16-byte word, so the two taps of that axis come with one load (S0 layout)
     int G[3];
     float gs[3];           // G/box per axis
-    const uint2 *grid;     // dense: [Gx][Gy][Gz]; sparse blocks: atlas [id][B][B][B] (omerf_sparse.cu)
+    const uint4 *grid;     // dense: [Gx][Gy][Gz] entries (pairs along z); sparse blocks: atlas [id][B][B][B] (omerf_sparse.cu)
     int blk_shift;         // 0 = dense grid, else log2 of the block edge B
     int nby, nbz;          // block-grid dims along y and z
     const int32_t *blk_table; // [nbx][nby][nbz] block id or -1
     int xy_n[2], xz_n[2], yz_n[2];
     float xy_s[2], xz_s[2], yz_s[2];
-    const uint2 *pxy, *pxz, *pyz;
+    const uint4 *pxy, *pxz, *pyz; // [A][B] entries, pairs along the second axis
+    int xz_rows, yz_rows;  // stored entries per row of xz / yz: the z band kept by the low-z bake (= xz_n[1] without it)
+    int xz_zoff, yz_zoff;  // first stored z row ("low resolution in the z direction, according to the upper and
+                           // lower bounds of the occupancy plane"; R27)
     int shared_taps;       // xy_n[0] == xz_n[0], xy_n[1] == yz_n[0], xz_n[1] == yz_n[1]: three taps serve the six plane axes
     float deq_mul, deq_add; // scale/65536, 4*bias
     float deq_mul_half, deq_add_half; // halves of the two: the per-sample sigmoids take tanh of half the pre-activation
@@ -60,7 +64,8 @@ struct omerf_scene {
     DevScene dev;
     int device;
     void *d_pyr, *d_grid, *d_pxy, *d_pxz, *d_pyz, *d_occ, *d_mlp_tab, *d_blk_table;
-    uint64_t blocks_total, blocks_allocated, grid_bytes;
+    uint64_t blocks_total, blocks_allocated, grid_bytes, plane_bytes;
+    int band[4];           // first/last stored z row of plane xz, then of plane yz
     uint64_t device_bytes;
     uint64_t occ_bits_set;
     // per-render state (mutable through the const handle: calls must be stream-ordered)
@@ -94,6 +99,8 @@ int omerf_cuda_fail(cudaError_t e, const char *what);
 // kernels' host launchers
 int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, cudaStream_t st);
 int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st);
+int omerf_launch_pair_layout(const void *d_src, void *d_dst, unsigned long long rows, int n, cudaStream_t st);
+int omerf_lowz_band(const omerf_scene *s, const float *d_lo, const float *d_up, int n_xz, int n_yz, int *band, cudaStream_t st);
 int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream_t st);
 int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_t st);
 int omerf_launch_render(const omerf_scene *s, const omerf_camera *d_cams, int n_views, int W, int H,

@@ -195,164 +195,162 @@ __device__ __forceinline__ int trav_step_grid(const DevScene &sc, const Ray &r, 
 // floor(frac * 256 + 1/2) in [0,256].  Both come out of ONE conversion: F = floor(fma(q, 256, 1/2)) = 256 floor(q) + w
 // exactly (256 q is exact and, for q < 2^15, so is the sum up to a rounding that cannot cross an integer), so
 // i = F >> 8 and w = F & 255.  A weight of 256 appears as (i + 1, 0): the same texels with the same total weights.
-// The point is inside the box (checked before every sample), hence -1 <= i <= N-1 and one clamp per tap suffices.
-__device__ __forceinline__ void axis_tap(float p, float s, int N, int &i0, int &i1, uint32_t &w)
+// The point is inside the box (checked before every sample), hence -1 <= i <= N-1; i = -1 (both taps are texel 0) is
+// folded into (i, w) = (0, 0), which gives texel 0 the whole weight as well.
+__device__ __forceinline__ void axis_tap(float p, float s, int &i, uint32_t &w)
 {
     const float q = __fmaf_rn(p, s, -0.5f);
-    const int F = floor_int(__fmaf_rn(q, 256.0f, 0.5f));
-    const int i = F >> 8;
+    const int F = max(floor_int(__fmaf_rn(q, 256.0f, 0.5f)), 0);
+    i = F >> 8;
     w = (uint32_t)(F & 255);
-    i0 = max(i, 0);
-    i1 = min(i + 1, N - 1);
 }
 
 // Bilinear footprints as 16-bit x 8-bit dot products (IDP.2A, fma pipe, full rate): the four weights
 // w_ab = (256 - w_a | w_a)(256 - w_b | w_b) are packed as two u16 pairs, the texel bytes of one channel of two
-// texels are brought side by side with one PRMT per two channels.  Only w_00 can reach 2^16 (w_a = w_b = 0; the taps never
-// carry a weight of 256, see axis_tap); then tap b1 is redirected to b0 and one unit of w_00 moves
-// to w_01, which multiplies the same texel: the sum stays the exact integer of R9.
+// texels are brought side by side with one PRMT per two channels.  Only w_00 can reach 2^16 (w_a = w_b = 0; the taps
+// never carry a weight of 256, see axis_tap): it is then stored as 65535 and the missing unit of texel (a0, b0) is added
+// by the caller (`ovf`, a rare branch): the sum stays the exact integer of R9.
 struct BiW {
     uint32_t w0, w1; // (w00 | w01 << 16), (w10 | w11 << 16): pairs along axis b for rows a0 and a1
+    bool ovf;
 };
 
-__device__ __forceinline__ BiW bilinear_weights(uint32_t wa, uint32_t wb, int b0, int &b1)
+__device__ __forceinline__ BiW bilinear_weights(uint32_t wa, uint32_t wb)
 {
-    if (wb == 0u) b1 = b0; // weight of column b1 is zero: point it at b0 so that it can carry the overflow unit
-    // (256 - wb | wb << 16) times a row weight <= 256 gives both products of the row in one multiply; the only carry
-    // between the halves is w00 = 2^16 (wa = wb = 0), which becomes 65535 in w00 plus 1 in w01 (the same texel then)
+    // (256 - wb | wb << 16) times a row weight <= 256 gives both products of the row in one multiply
     const uint32_t pb = wb * 0xffffu + 256u;
     BiW r;
-    r.w0 = (256u - wa) * pb + ((wa | wb) == 0u ? 0xffffu : 0u);
+    r.ovf = (wa | wb) == 0u;
+    r.w0 = r.ovf ? 0xffffu : (256u - wa) * pb;
     r.w1 = wa * pb;
     return r;
 }
 
-// acc[0..7] += sum over the 2x2 footprint of w_ab * texel_ab[c]
-__device__ __forceinline__ void bilinear8_dp(const uint2 t00, const uint2 t01, const uint2 t10, const uint2 t11, const BiW w,
-                                             uint32_t acc[8])
+// acc[0..7] += sum over the 2x2 footprint of w_ab * texel_ab[c]; ra = texels (a0,b0),(a0,b1), rb = (a1,b0),(a1,b1)
+// (8 channels = 2 words per texel: .x/.y the first texel of the pair, .z/.w the second)
+__device__ __forceinline__ void bilinear8_dp(const uint32_t a0x, const uint32_t a0y, const uint32_t a1x, const uint32_t a1y,
+                                             const uint32_t b0x, const uint32_t b0y, const uint32_t b1x, const uint32_t b1y,
+                                             const BiW w, uint32_t acc[8])
 {
+    // a0* = texel (a0,b0), a1* = texel (a0,b1), b0* = texel (a1,b0), b1* = texel (a1,b1)
     uint32_t p, q;
-    p = __byte_perm(t00.x, t01.x, 0x5140);
-    q = __byte_perm(t10.x, t11.x, 0x5140);
+    p = __byte_perm(a0x, a1x, 0x5140);
+    q = __byte_perm(b0x, b1x, 0x5140);
     acc[0] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[0]));
     acc[1] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[1]));
-    p = __byte_perm(t00.x, t01.x, 0x7362);
-    q = __byte_perm(t10.x, t11.x, 0x7362);
+    p = __byte_perm(a0x, a1x, 0x7362);
+    q = __byte_perm(b0x, b1x, 0x7362);
     acc[2] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[2]));
     acc[3] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[3]));
-    p = __byte_perm(t00.y, t01.y, 0x5140);
-    q = __byte_perm(t10.y, t11.y, 0x5140);
+    p = __byte_perm(a0y, a1y, 0x5140);
+    q = __byte_perm(b0y, b1y, 0x5140);
     acc[4] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[4]));
     acc[5] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[5]));
-    p = __byte_perm(t00.y, t01.y, 0x7362);
-    q = __byte_perm(t10.y, t11.y, 0x7362);
+    p = __byte_perm(a0y, a1y, 0x7362);
+    q = __byte_perm(b0y, b1y, 0x7362);
     acc[6] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[6]));
     acc[7] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[7]));
+    if (w.ovf) { // w_00 = 2^16 was stored as 2^16 - 1 (probability 2^-16 per footprint)
+        acc[0] += a0x & 255u; acc[1] += (a0x >> 8) & 255u; acc[2] += (a0x >> 16) & 255u; acc[3] += a0x >> 24;
+        acc[4] += a0y & 255u; acc[5] += (a0y >> 8) & 255u; acc[6] += (a0y >> 16) & 255u; acc[7] += a0y >> 24;
+    }
 }
 
-__device__ __forceinline__ void plane_taps(const uint2 *__restrict__ tex, int Nb, int a0, int a1, int b0, int b1, uint2 t[4])
-{
-    // 32-bit texel indices (every source has fewer than 2^32 texels; checked at scene creation)
-    const uint32_t r0 = (uint32_t)a0 * (uint32_t)Nb, r1 = (uint32_t)a1 * (uint32_t)Nb;
-    t[0] = __ldg(tex + (r0 + (uint32_t)b0));
-    t[1] = __ldg(tex + (r0 + (uint32_t)b1));
-    t[2] = __ldg(tex + (r1 + (uint32_t)b0));
-    t[3] = __ldg(tex + (r1 + (uint32_t)b1));
-}
-
-// texel indices of the 8 trilinear corners of V, order (x0y0, x0y1, x1y0, x1y1) x (z0, z1).  Dense layout: row-major
-// [Gx][Gy][Gz]; sparse blocks (8(f).1): one block-table lookup per corner, then the texel inside the atlas block.
+// Entry indices of the 4 (x,y) corner columns of V at tap z, order x0y0, x0y1, x1y0, x1y1; every entry holds the texels
+// (z, z+1) of its column (S0 layout, omerf_build.cu).  Dense layout: row-major [Gx][Gy][Gz]; sparse blocks (8(f).1):
+// one block-table lookup per corner column, then the entry inside the atlas block (the z+1 texel of an entry was
+// copied from the neighbouring block at bake time, so one lookup serves both z taps).
 template <bool GENERAL>
-__device__ __forceinline__ void grid_corner_offsets(const DevScene &sc, int x0, int x1, int y0, int y1, int z0, int z1,
-                                                    uint32_t off[8])
+__device__ __forceinline__ void grid_corner_offsets(const DevScene &sc, int x0, int x1, int y0, int y1, int z, uint32_t off[4])
 {
     if (!GENERAL || sc.blk_shift == 0) {
         const uint32_t Gy = (uint32_t)sc.G[1], Gz = (uint32_t)sc.G[2];
         const uint32_t c0 = (uint32_t)x0 * Gy, c1 = (uint32_t)x1 * Gy;
-        const uint32_t r00 = (c0 + (uint32_t)y0) * Gz, r01 = (c0 + (uint32_t)y1) * Gz;
-        const uint32_t r10 = (c1 + (uint32_t)y0) * Gz, r11 = (c1 + (uint32_t)y1) * Gz;
-        off[0] = r00 + (uint32_t)z0; off[1] = r00 + (uint32_t)z1;
-        off[2] = r01 + (uint32_t)z0; off[3] = r01 + (uint32_t)z1;
-        off[4] = r10 + (uint32_t)z0; off[5] = r10 + (uint32_t)z1;
-        off[6] = r11 + (uint32_t)z0; off[7] = r11 + (uint32_t)z1;
+        off[0] = (c0 + (uint32_t)y0) * Gz + (uint32_t)z;
+        off[1] = (c0 + (uint32_t)y1) * Gz + (uint32_t)z;
+        off[2] = (c1 + (uint32_t)y0) * Gz + (uint32_t)z;
+        off[3] = (c1 + (uint32_t)y1) * Gz + (uint32_t)z;
     } else {
         const int s = sc.blk_shift, m = (1 << s) - 1;
-        const int xs[2] = {x0, x1}, ys[2] = {y0, y1}, zs[2] = {z0, z1};
+        const int xs[2] = {x0, x1}, ys[2] = {y0, y1};
 #pragma unroll
         for (int a = 0; a < 2; a++)
 #pragma unroll
             for (int b = 0; b < 2; b++) {
-                const int col = ((xs[a] >> s) * sc.nby + (ys[b] >> s)) * sc.nbz;
-                const uint32_t in_xy = (uint32_t)((((xs[a] & m) << s) + (ys[b] & m)) << s);
-#pragma unroll
-                for (int c = 0; c < 2; c++) {
-                    // every corner of a sample inside the slab lies in an allocated block (R24); max() only guards memory
-                    const int id = max(__ldg(sc.blk_table + col + (zs[c] >> s)), 0);
-                    off[(a * 2 + b) * 2 + c] = ((uint32_t)id << (3 * s)) + in_xy + (uint32_t)(zs[c] & m);
-                }
+                // every corner of a sample inside the slab lies in an allocated block (R24); max() only guards memory
+                const int id = max(__ldg(sc.blk_table + ((xs[a] >> s) * sc.nby + (ys[b] >> s)) * sc.nbz + (z >> s)), 0);
+                off[a * 2 + b] = ((uint32_t)id << (3 * s)) + (uint32_t)(((((xs[a] & m) << s) + (ys[b] & m)) << s) + (z & m));
             }
     }
 }
 
+// The 10 gathers of one sample: every load fetches a PAIR of texels that are adjacent along the array's fastest axis
+// (z for V, the second axis for the planes) as one 16-byte word.
+struct Footprints {
+    uint4 g[4];  // V: corner columns x0y0, x0y1, x1y0, x1y1, each (z0 | z1)
+    uint4 p[6];  // xy rows a0, a1; xz rows a0, a1; yz rows a0, a1, each (b0 | b1)
+};
+
 template <bool GENERAL>
 __device__ __forceinline__ void gather_features(const DevScene &sc, float px, float py, float pz, uint32_t I[8])
 {
-    // taps and weights of all four sources first, then all 20 loads, then the arithmetic
-    int x0, x1, y0, y1, z0, z1;
+    // taps and weights of all four sources first, then all 10 loads, then the arithmetic
+    int x0, y0, zi;
     uint32_t wx, wy, wz;
-    axis_tap(px, sc.gs[0], sc.G[0], x0, x1, wx);
-    axis_tap(py, sc.gs[1], sc.G[1], y0, y1, wy);
-    axis_tap(pz, sc.gs[2], sc.G[2], z0, z1, wz);
-    const BiW wg = bilinear_weights(wx, wy, y0, y1);
-    uint2 ga[4], gb[4];
+    axis_tap(px, sc.gs[0], x0, wx);
+    axis_tap(py, sc.gs[1], y0, wy);
+    axis_tap(pz, sc.gs[2], zi, wz);
+    const int x1 = min(x0 + 1, sc.G[0] - 1), y1 = min(y0 + 1, sc.G[1] - 1);
+    Footprints f;
     {
-        // low-res voxel grid V: bilinear in (x,y) on the z-slices z0 and z1
-        uint32_t off[8];
-        grid_corner_offsets<GENERAL>(sc, x0, x1, y0, y1, z0, z1, off);
-        const uint2 *g = sc.grid;
-        ga[0] = __ldg(g + off[0]); gb[0] = __ldg(g + off[1]);
-        ga[1] = __ldg(g + off[2]); gb[1] = __ldg(g + off[3]);
-        ga[2] = __ldg(g + off[4]); gb[2] = __ldg(g + off[5]);
-        ga[3] = __ldg(g + off[6]); gb[3] = __ldg(g + off[7]);
+        uint32_t off[4];
+        grid_corner_offsets<GENERAL>(sc, x0, x1, y0, y1, zi, off);
+#pragma unroll
+        for (int c = 0; c < 4; c++) f.g[c] = __ldg(sc.grid + off[c]);
     }
     // triplanes: xy sampled with (x,y), xz with (x,z), yz with (y,z).  When the planes share their resolution per
     // world axis (every config: xy A x A, xz and yz A x B) a tap computed for one plane is the other plane's tap too
     // (same scale, same arithmetic), so three taps serve all six plane axes.
-    uint2 t1[4], t2[4], t3[4];
-    int xa0, xa1, ya0, ya1, za0, za1;
+    int xa, ya, za;
     uint32_t xw, yw, zw;
-    axis_tap(px, sc.xy_s[0], sc.xy_n[0], xa0, xa1, xw);
-    axis_tap(py, sc.xy_s[1], sc.xy_n[1], ya0, ya1, yw);
-    axis_tap(pz, sc.xz_s[1], sc.xz_n[1], za0, za1, zw);
-    int xb0 = xa0, xb1 = xa1, yb0 = ya0, yb1 = ya1, zb0 = za0, zb1 = za1; // taps of xz axis 0, yz axis 0, yz axis 1
+    axis_tap(px, sc.xy_s[0], xa, xw);
+    axis_tap(py, sc.xy_s[1], ya, yw);
+    axis_tap(pz, sc.xz_s[1], za, zw);
+    int xb = xa, yb = ya, zb = za; // taps of xz axis 0, yz axis 0, yz axis 1
     uint32_t xbw = xw, ybw = yw, zbw = zw;
     if (!sc.shared_taps) {
-        axis_tap(px, sc.xz_s[0], sc.xz_n[0], xb0, xb1, xbw);
-        axis_tap(py, sc.yz_s[0], sc.yz_n[0], yb0, yb1, ybw);
-        axis_tap(pz, sc.yz_s[1], sc.yz_n[1], zb0, zb1, zbw);
+        axis_tap(px, sc.xz_s[0], xb, xbw);
+        axis_tap(py, sc.yz_s[0], yb, ybw);
+        axis_tap(pz, sc.yz_s[1], zb, zbw);
     }
-    int b1;
-    b1 = ya1;
-    const BiW w1 = bilinear_weights(xw, yw, ya0, b1);
-    plane_taps(sc.pxy, sc.xy_n[1], xa0, xa1, ya0, b1, t1);
-    b1 = za1;
-    const BiW w2 = bilinear_weights(xbw, zw, za0, b1);
-    plane_taps(sc.pxz, sc.xz_n[1], xb0, xb1, za0, b1, t2);
-    b1 = zb1;
-    const BiW w3 = bilinear_weights(ybw, zbw, zb0, b1);
-    plane_taps(sc.pyz, sc.yz_n[1], yb0, yb1, zb0, b1, t3);
+    {
+        // 32-bit entry indices (every source has fewer than 2^32 texels; checked at scene creation)
+        const uint32_t Nxy = (uint32_t)sc.xy_n[1], Nxz = (uint32_t)sc.xz_rows, Nyz = (uint32_t)sc.yz_rows;
+        const uint32_t xa1 = (uint32_t)min(xa + 1, sc.xy_n[0] - 1), xb1 = (uint32_t)min(xb + 1, sc.xz_n[0] - 1),
+                       yb1 = (uint32_t)min(yb + 1, sc.yz_n[0] - 1);
+        const uint32_t zr = (uint32_t)(za - sc.xz_zoff), zs = (uint32_t)(zb - sc.yz_zoff); // low-z bake: rows below the band are not stored
+        f.p[0] = __ldg(sc.pxy + ((uint32_t)xa * Nxy + (uint32_t)ya));
+        f.p[1] = __ldg(sc.pxy + (xa1 * Nxy + (uint32_t)ya));
+        f.p[2] = __ldg(sc.pxz + ((uint32_t)xb * Nxz + zr));
+        f.p[3] = __ldg(sc.pxz + (xb1 * Nxz + zr));
+        f.p[4] = __ldg(sc.pyz + ((uint32_t)yb * Nyz + zs));
+        f.p[5] = __ldg(sc.pyz + (yb1 * Nyz + zs));
+    }
+    const BiW wg = bilinear_weights(wx, wy);
+    const BiW w1 = bilinear_weights(xw, yw), w2 = bilinear_weights(xbw, zw), w3 = bilinear_weights(ybw, zbw);
 
     uint32_t A[8], B[8];
 #pragma unroll
     for (int c = 0; c < 8; c++) A[c] = B[c] = 0u;
-    bilinear8_dp(ga[0], ga[1], ga[2], ga[3], wg, A);
-    bilinear8_dp(gb[0], gb[1], gb[2], gb[3], wg, B);
+    // V: bilinear in (x,y) on the z-slices z0 (.x/.y of every corner column) and z1 (.z/.w)
+    bilinear8_dp(f.g[0].x, f.g[0].y, f.g[1].x, f.g[1].y, f.g[2].x, f.g[2].y, f.g[3].x, f.g[3].y, wg, A);
+    bilinear8_dp(f.g[0].z, f.g[0].w, f.g[1].z, f.g[1].w, f.g[2].z, f.g[2].w, f.g[3].z, f.g[3].w, wg, B);
     // the z lerp rounds once (R9): (256 - wz) A + wz B < 2^32
 #pragma unroll
     for (int c = 0; c < 8; c++) I[c] = ((256u - wz) * A[c] + wz * B[c] + 128u) >> 8;
-    bilinear8_dp(t1[0], t1[1], t1[2], t1[3], w1, I);
-    bilinear8_dp(t2[0], t2[1], t2[2], t2[3], w2, I);
-    bilinear8_dp(t3[0], t3[1], t3[2], t3[3], w3, I);
+    bilinear8_dp(f.p[0].x, f.p[0].y, f.p[0].z, f.p[0].w, f.p[1].x, f.p[1].y, f.p[1].z, f.p[1].w, w1, I);
+    bilinear8_dp(f.p[2].x, f.p[2].y, f.p[2].z, f.p[2].w, f.p[3].x, f.p[3].y, f.p[3].z, f.p[3].w, w2, I);
+    bilinear8_dp(f.p[4].x, f.p[4].y, f.p[4].z, f.p[4].w, f.p[5].x, f.p[5].y, f.p[5].z, f.p[5].w, w3, I);
 }
 
 // per-sample activations (Eq. 3, colour path only): sigmoid(2x) = 1/2 + 1/2 tanh(x) with one MUFU.TANH; the caller
@@ -822,7 +820,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 }
 
 // ---------------------------------------------------------------------------------- gather calibration
-// Replays the 20 feature loads (8 grid + 3 x 4 plane texels, 8 bytes each) of logged samples with no filtering,
+// Replays the 10 feature loads (4 grid + 3 x 2 plane entries, 16 bytes = two adjacent texels each) of logged samples with no filtering,
 // activation or compositing: one sample per thread, every lane busy, full occupancy.  The rate it reaches is the
 // gather ceiling of this scene, camera and load width on this GPU; `order` selects frame order (the order the
 // march kernel took the samples) or a scattered order (multiplicative permutation of the log).
@@ -842,28 +840,34 @@ omerf_gather_probe_kernel(const __grid_constant__ DevScene sc, const omerf_camer
     r.oz = cam->origin[2];
     float px, py, pz;
     lattice_point(r, sc.step, (int)e.y, px, py, pz);
-    int x0, x1, y0, y1, z0, z1, a0, a1, b0, b1;
+    // the same 10 sixteen-byte loads as gather_features (addresses only; weights are not needed)
+    int x0, y0, zi, xa, ya, za, xb, yb, zb;
     uint32_t w;
-    axis_tap(px, sc.gs[0], sc.G[0], x0, x1, w);
-    axis_tap(py, sc.gs[1], sc.G[1], y0, y1, w);
-    axis_tap(pz, sc.gs[2], sc.G[2], z0, z1, w);
-    uint32_t off[8];
-    grid_corner_offsets<true>(sc, x0, x1, y0, y1, z0, z1, off);
-    uint2 t[20];
+    axis_tap(px, sc.gs[0], x0, w);
+    axis_tap(py, sc.gs[1], y0, w);
+    axis_tap(pz, sc.gs[2], zi, w);
+    uint32_t off[4];
+    grid_corner_offsets<true>(sc, x0, min(x0 + 1, sc.G[0] - 1), y0, min(y0 + 1, sc.G[1] - 1), zi, off);
+    uint4 t[10];
 #pragma unroll
-    for (int q = 0; q < 8; q++) t[q] = __ldg(sc.grid + off[q]);
-    axis_tap(px, sc.xy_s[0], sc.xy_n[0], a0, a1, w);
-    axis_tap(py, sc.xy_s[1], sc.xy_n[1], b0, b1, w);
-    plane_taps(sc.pxy, sc.xy_n[1], a0, a1, b0, b1, t + 8);
-    axis_tap(px, sc.xz_s[0], sc.xz_n[0], a0, a1, w);
-    axis_tap(pz, sc.xz_s[1], sc.xz_n[1], b0, b1, w);
-    plane_taps(sc.pxz, sc.xz_n[1], a0, a1, b0, b1, t + 12);
-    axis_tap(py, sc.yz_s[0], sc.yz_n[0], a0, a1, w);
-    axis_tap(pz, sc.yz_s[1], sc.yz_n[1], b0, b1, w);
-    plane_taps(sc.pyz, sc.yz_n[1], a0, a1, b0, b1, t + 16);
+    for (int q = 0; q < 4; q++) t[q] = __ldg(sc.grid + off[q]);
+    axis_tap(px, sc.xy_s[0], xa, w);
+    axis_tap(py, sc.xy_s[1], ya, w);
+    axis_tap(px, sc.xz_s[0], xb, w);
+    axis_tap(pz, sc.xz_s[1], za, w);
+    axis_tap(py, sc.yz_s[0], yb, w);
+    axis_tap(pz, sc.yz_s[1], zb, w);
+    const uint32_t Nxy = (uint32_t)sc.xy_n[1], Nxz = (uint32_t)sc.xz_rows, Nyz = (uint32_t)sc.yz_rows;
+    const uint32_t zr = (uint32_t)(za - sc.xz_zoff), zs = (uint32_t)(zb - sc.yz_zoff);
+    t[4] = __ldg(sc.pxy + ((uint32_t)xa * Nxy + (uint32_t)ya));
+    t[5] = __ldg(sc.pxy + ((uint32_t)min(xa + 1, sc.xy_n[0] - 1) * Nxy + (uint32_t)ya));
+    t[6] = __ldg(sc.pxz + ((uint32_t)xb * Nxz + zr));
+    t[7] = __ldg(sc.pxz + ((uint32_t)min(xb + 1, sc.xz_n[0] - 1) * Nxz + zr));
+    t[8] = __ldg(sc.pyz + ((uint32_t)yb * Nyz + zs));
+    t[9] = __ldg(sc.pyz + ((uint32_t)min(yb + 1, sc.yz_n[0] - 1) * Nyz + zs));
     uint32_t x = 0;
 #pragma unroll
-    for (int q = 0; q < 20; q++) x ^= t[q].x + t[q].y;
+    for (int q = 0; q < 10; q++) x ^= (t[q].x + t[q].y) ^ (t[q].z + t[q].w);
     sink[i] = x;
 }
 

@@ -73,9 +73,11 @@ __global__ void __launch_bounds__(1024) sparse_scan_kernel(const uint32_t *__res
     if (t == 1023) *n_alloc = sums[1023];
 }
 
-// one CTA per block of the block grid; allocated blocks copy their B^3 texels (zeros past the grid edge)
+// one CTA per block of the block grid; allocated blocks copy their B^3 ENTRIES (zeros past the grid edge).  An entry is
+// the texel pair (z, min(z + 1, Gz - 1)) of the dense array (S0 layout, omerf_build.cu): the second texel of a block's last
+// z layer comes from the block above, so the trilinear gather needs one table lookup per corner column.
 __global__ void sparse_copy_kernel(const uint2 *__restrict__ dense, int Gx, int Gy, int Gz, int shift, int nby, int nbz,
-                                   const int32_t *__restrict__ table, uint2 *__restrict__ atlas)
+                                   const int32_t *__restrict__ table, uint4 *__restrict__ atlas)
 {
     const int32_t id = table[blockIdx.x];
     if (id < 0) return;
@@ -84,15 +86,20 @@ __global__ void sparse_copy_kernel(const uint2 *__restrict__ dense, int Gx, int 
     for (int v = threadIdx.x; v < vox; v += blockDim.x) {
         const int z = v & m, y = (v >> shift) & m, x = v >> (2 * shift);
         const int gx = (bx << shift) + x, gy = (by << shift) + y, gz = (bz << shift) + z;
-        uint2 t = make_uint2(0u, 0u);
-        if (gx < Gx && gy < Gy && gz < Gz) t = dense[((size_t)gx * Gy + gy) * Gz + gz];
+        uint4 t = make_uint4(0u, 0u, 0u, 0u);
+        if (gx < Gx && gy < Gy && gz < Gz) {
+            const size_t col = ((size_t)gx * Gy + gy) * Gz;
+            const uint2 a = dense[col + gz], b = dense[col + min(gz + 1, Gz - 1)];
+            t = make_uint4(a.x, a.y, b.x, b.y);
+        }
         atlas[(size_t)id * vox + v] = t;
     }
 }
 
 } // namespace
 
-// Replaces the dense grid *d_dense (freed here) by (block table, atlas); fills the sparse fields of s->dev.
+// Builds (block table, atlas) from the raw dense texels *d_dense ([Gx][Gy][Gz] of 8 bytes; freed here and replaced by the
+// atlas); fills the sparse fields of s->dev.
 int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream_t st)
 {
     DevScene &v = s->dev;
@@ -131,10 +138,10 @@ int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream
             break;
         }
         void *atlas = nullptr;
-        SP_CUDA(cudaMalloc(&atlas, (texels ? texels : 1) * sizeof(uint2)));
+        SP_CUDA(cudaMalloc(&atlas, (texels ? texels : 1) * sizeof(uint4)));
         if (n_alloc)
             sparse_copy_kernel<<<(unsigned int)nb, 256, 0, st>>>((const uint2 *)*d_dense, v.G[0], v.G[1], v.G[2], shift, nby, nbz,
-                                                                 (const int32_t *)s->d_blk_table, (uint2 *)atlas);
+                                                                 (const int32_t *)s->d_blk_table, (uint4 *)atlas);
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
         if (e != cudaSuccess) {
@@ -145,14 +152,14 @@ int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream
 #undef SP_CUDA
         cudaFree(*d_dense);
         *d_dense = atlas;
-        v.grid = (const uint2 *)atlas;
+        v.grid = (const uint4 *)atlas;
         v.blk_shift = shift;
         v.nby = nby;
         v.nbz = nbz;
         v.blk_table = (const int32_t *)s->d_blk_table;
         s->blocks_total = nb;
         s->blocks_allocated = n_alloc;
-        s->grid_bytes = texels * sizeof(uint2) + nb * sizeof(int32_t);
+        s->grid_bytes = texels * sizeof(uint4) + nb * sizeof(int32_t);
     } while (0);
     cudaFree(mark);
     cudaFree(d_n);

@@ -134,7 +134,7 @@ def test_config1_sparse_block_grid(omerf, city):
     with omerf.scene_create(city, grid_block=8) as h:
         info = omerf.scene_info(h)
         assert np.array_equal(omerf.block_table(h), S.table.ravel())
-        assert info["grid_blocks_allocated"] == S.n_alloc and info["grid_bytes"] < 128 << 20
+        assert info["grid_blocks_allocated"] == S.n_alloc and info["grid_bytes"] < 0.75 * 2 * city.grid.nbytes   # dense V on the device: 16-byte entries
         rgb, ns = omerf.render(h, cams, W, H)
         torch.cuda.synchronize()
         rgb, ns = rgb.cpu().numpy(), ns.cpu().numpy().view(np.uint32)
@@ -176,3 +176,25 @@ def test_config1_soft_mask_whole_frame(omerf, city):
     assert np.array_equal(ns[vuv[:, 0], vuv[:, 2], vuv[:, 1]], ref["nsamples"])
     assert np.abs(rgb[vuv[:, 0], vuv[:, 2], vuv[:, 1]].astype(np.float64) - ref["rgb"]).max() <= RGB_TOL
     assert np.abs(ref["rgb"] - hard["rgb"]).max() > 1e-2
+
+
+def test_config1_lowz_bake_whole_frame(omerf, city):
+    """SURVEY 8(f).1 second half at full size: the band is the oracle's, the side planes shrink, and the
+    whole frame equals the UNCROPPED oracle's."""
+    import torch
+
+    import oracle
+    cams = synth.make_cameras(1)
+    W, H = synth.config_resolution(1)
+    O = oracle.OracleScene(city)
+    bx, by = oracle.LowZBand(O, "xz", crop=False), oracle.LowZBand(O, "yz", crop=False)
+    with omerf.scene_create(city, lowz_bake=True) as h:
+        info = omerf.scene_info(h)
+        rgb, ns = omerf.render(h, cams, W, H)
+        torch.cuda.synchronize()
+        rgb, ns = rgb.cpu().numpy(), ns.cpu().numpy().view(np.uint32)
+    assert info["xz_band"] == (bx.b_lo, bx.b_hi) and info["yz_band"] == (by.b_lo, by.b_hi)
+    side_full = 2 * (city.plane_xz.nbytes + city.plane_yz.nbytes)
+    side_now = info["plane_bytes"] - 2 * city.plane_xy.nbytes
+    assert side_now == 16 * (city.plane_xz.shape[0] * bx.rows + city.plane_yz.shape[0] * by.rows) < side_full
+    _check_whole_views(rgb, ns, city, cams, W, H, 0, [0])

@@ -309,7 +309,7 @@ def test_sparse_block_grid_matches_oracle_bake_and_dense_render(omerf, oracle, B
     with omerf.scene_create(sc, grid_block=B) as h:
         info = omerf.scene_info(h)
         assert info["grid_blocks_total"] == S.table.size and info["grid_blocks_allocated"] == S.n_alloc
-        assert info["grid_bytes"] == S.n_alloc * B ** 3 * 8 + S.table.size * 4
+        assert info["grid_bytes"] == S.n_alloc * B ** 3 * 16 + S.table.size * 4     # 16-byte entries (texel pairs along z)
         assert np.array_equal(omerf.block_table(h), S.table.ravel())
         rgb, ns = omerf.render(h, cams, 72, 56)
         torch.cuda.synchronize()
@@ -390,3 +390,107 @@ def test_heatmap_is_bit_exact(omerf, oracle):
             assert np.array_equal(hm.cpu().numpy(), oracle.heatmap(ns.cpu().numpy().view(np.uint32), n_max))
     with pytest.raises(omerf.OmerfError):
         omerf.heatmap(ns, 0)
+
+
+def test_device_block_table_against_the_plain_definition(omerf, oracle):
+    """The DEVICE bake judged against the plain definition, not against the oracle's formula: on a tiny scene the voxels
+    that a dense sampling of the slab really touches (brute force over points that pass Eq. 7) must all lie in blocks
+    the device allocated (soundness), and every allocated block must hold a voxel within one voxel of a touched one
+    (tightness: the rule may over-mark by its stated padding only)."""
+    import math
+    from scipy.ndimage import binary_dilation
+    rng = np.random.default_rng(7)
+    hf, G, box, B = 9, (10, 9, 8), (8.0, 8.0, 4.0), 2
+    lo = (0.5 + 2.0 * rng.random((hf, hf))).astype(np.float32)
+    hi = (lo + 0.05 + 1.0 * rng.random((hf, hf))).astype(np.float32)
+    kill = rng.random((hf, hf)) < 0.2
+    hi[kill] = lo[kill] - 1.0
+    sc = synth.custom_scene(box=box, hf_n=(hf, hf), h_lo=lo, h_up=hi, grid_n=G, seed=7, smooth=False)
+    O = oracle.OracleScene(sc)
+    touched = np.zeros(G, dtype=bool)
+    xs = np.linspace(0.0, 8.0, 161, dtype=np.float32)[:-1] + np.float32(0.013)
+    zs = np.linspace(0.0, 4.0, 201, dtype=np.float32)[:-1] + np.float32(0.007)
+    for x in xs:
+        for y in xs:
+            ix, iy = int(math.floor(x + 0.5)), int(math.floor(y + 0.5))
+            for z in zs[(zs >= sc.h_lo[ix, iy]) & (zs <= sc.h_up[ix, iy])]:
+                c = oracle.grid_corners(O, np.array([x, y, z], dtype=np.float32))
+                touched[c[0]:c[1] + 1, c[2]:c[3] + 1, c[4]:c[5] + 1] = True
+    assert touched.sum() > 50
+    with omerf.scene_create(sc, grid_block=B) as h:
+        nb = tuple((g + B - 1) // B for g in G)
+        alloc = omerf.block_table(h).reshape(nb) >= 0
+    vox_alloc = np.repeat(np.repeat(np.repeat(alloc, B, 0), B, 1), B, 2)[:G[0], :G[1], :G[2]]
+    assert not (touched & ~vox_alloc).any()                                    # soundness
+    near = binary_dilation(touched, structure=np.ones((3, 3, 3), bool))
+    pad = np.zeros(tuple(n * B for n in nb), dtype=bool)
+    pad[:G[0], :G[1], :G[2]] = near
+    blocks_near = pad.reshape(nb[0], B, nb[1], B, nb[2], B).any(axis=(1, 3, 5))
+    assert not (alloc & ~blocks_near).any()                                    # tightness
+    assert 0 < alloc.sum() < alloc.size
+
+
+# ----------------------------------------------------------------------------- SURVEY 8(f).1, second half: low-z triplane bake
+def _lowz_scene(seed, m=21, lo_rng=(2.2, 3.0), thick=(0.05, 1.5), empty=0.2, **kw):
+    rng = np.random.default_rng(seed)
+    lo = (lo_rng[0] + (lo_rng[1] - lo_rng[0]) * rng.random((m, m))).astype(np.float32)
+    hi = (lo + thick[0] + (thick[1] - thick[0]) * rng.random((m, m))).astype(np.float32)
+    kill = rng.random((m, m)) < empty
+    lo[kill], hi[kill] = 7.5, 0.2                                  # empty columns must not widen the band
+    return synth.custom_scene(box=(14.0, 13.0, 8.0), hf_n=(m, m), h_lo=lo, h_up=hi, grid_n=(20, 18, 12), xy_n=(64, 60),
+                              xz_n=(64, 48), yz_n=(60, 40), seed=seed, step=0.15, smooth=False, bias_amp=0.2, **kw)
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_lowz_bake_band_is_the_oracles_and_the_image_is_unchanged(omerf, oracle, seed):
+    """PAPER.md:186 / DESIGN.md R27: the device keeps exactly the oracle's band of z rows (bit-exact integers), stores
+    fewer plane bytes, and renders the UNCROPPED oracle's image (same texels fetched), alone and with sparse blocks + soft mask."""
+    import torch
+    sc = _lowz_scene(seed)
+    cams = np.stack([synth.look_at_camera((7.0, -8.0, 15.0), (7.0, 6.5, 2.0), 72, 56),
+                     synth.look_at_camera((1.0, 1.5, 3.0), (13.0, 12.0, 2.6), 72, 56)])
+    O = oracle.OracleScene(sc)
+    bands = {w: oracle.LowZBand(O, w, crop=False) for w in ("xz", "yz")}
+    with omerf.scene_create(sc) as h:
+        full = omerf.scene_info(h)
+    assert full["xz_band"] == (0, 47) and full["yz_band"] == (0, 39)
+    with omerf.scene_create(sc, lowz_bake=True) as h:
+        info = omerf.scene_info(h)
+        rgb, ns = omerf.render(h, cams, 72, 56)
+        torch.cuda.synchronize()
+        probe = omerf.gather_probe(h, cams[0], 72, 56, repeats=1, flush_l2=False)
+    assert info["xz_band"] == (bands["xz"].b_lo, bands["xz"].b_hi) and info["yz_band"] == (bands["yz"].b_lo, bands["yz"].b_hi)
+    assert bands["xz"].rows < 48 and bands["yz"].rows < 40
+    assert full["plane_bytes"] - info["plane_bytes"] == 16 * (64 * (48 - bands["xz"].rows) + 60 * (40 - bands["yz"].rows))
+    ref = O.render(cams, 72, 56, mode="brute")
+    assert ref["nsamples"].sum() > 3000
+    _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, "low-z bake")
+    assert probe["samples"] == int(ref["nsamples"][0].sum())
+    with omerf.scene_create(sc, lowz_bake=True, grid_block=4, soft_eps=0.3) as h:
+        rgb, ns = omerf.render(h, cams, 72, 56)
+        torch.cuda.synchronize()
+    ref = oracle.OracleScene(sc, soft_eps=0.3).render(cams, 72, 56, mode="brute")
+    _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32), ref, "low-z + sparse + soft")
+
+
+def test_lowz_bake_degenerate_scenes_and_rejections(omerf, oracle):
+    import torch
+    cam = synth.look_at_camera((4.0, -6.0, 9.0), (4.0, 4.0, 2.0), 40, 30)
+    for lo, hi, want in ((3.0, 1.0, (0, 0)),        # no occupied column: one row is kept, nothing is ever fetched
+                         (-2.0, 9.0, (0, 31)),      # slab larger than the box: the whole plane
+                         (1.0, 1.0, None)):         # zero-thickness slab
+        sc = synth.custom_scene(box=(8.0, 8.0, 4.0), hf_n=(9, 9), h_lo=lo, h_up=hi, xz_n=(16, 32), yz_n=(16, 32), seed=3)
+        O = oracle.OracleScene(sc)
+        Bd = oracle.LowZBand(O, "xz", crop=False)
+        with omerf.scene_create(sc, lowz_bake=True) as h:
+            info = omerf.scene_info(h)
+            rgb, ns = omerf.render(h, cam, 40, 30)
+            torch.cuda.synchronize()
+        assert info["xz_band"] == (Bd.b_lo, Bd.b_hi) == info["yz_band"]
+        if want is not None:
+            assert info["xz_band"] == want
+        _assert_parity(rgb.cpu().numpy().astype(np.float64), ns.cpu().numpy().view(np.uint32),
+                       O.render(cam, 40, 30, mode="brute"), f"low-z, slab [{lo}, {hi}]")
+    sc = synth.custom_scene(occ_n=(8, 8, 8))
+    with pytest.raises(omerf.OmerfError):
+        omerf.scene_create(sc, sampler=1, lowz_bake=True)     # the grid sampler's voxels are a superset of the slab
