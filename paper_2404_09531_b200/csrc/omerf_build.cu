@@ -335,9 +335,10 @@ __global__ void mlp_pack_kernel(const float *__restrict__ W0, const float *__res
     if (tile < OMERF_MLP_TILES) {
         float w0 = 0.0f, w1 = 0.0f;
         if (tile < 10) {
-            const int s = tile >> 1, q = tile & 1, n = 8 * q + g, k0 = 8 * s + t, k1 = 8 * s + t + 4;
-            if (k0 < OMERF_MLP_IN) w0 = W0[n * OMERF_MLP_IN + k0];
-            if (k1 < OMERF_MLP_IN) w1 = W0[n * OMERF_MLP_IN + k1];
+            // layer-1 columns are permuted (omerf_mlp.cuh: mlp_orig_of_col); padding columns carry weight 0
+            const int s = tile >> 1, q = tile & 1, n = 8 * q + g, k0 = mlp_orig_of_col(8 * s + t), k1 = mlp_orig_of_col(8 * s + t + 4);
+            if (k0 >= 0) w0 = W0[n * OMERF_MLP_IN + k0];
+            if (k1 >= 0) w1 = W0[n * OMERF_MLP_IN + k1];
         } else if (tile < 14) {
             const int s = (tile - 10) >> 1, q = (tile - 10) & 1, n = 8 * q + g;
             w0 = W1[n * OMERF_MLP_HID + 8 * s + 2 * t];

@@ -13,6 +13,24 @@
 #define OMERF_MLP_BIAS_OFF (OMERF_MLP_TILES * 2 * 32)
 #define OMERF_MLP_TAB_LEN (OMERF_MLP_BIAS_OFF + 5 * 32)
 
+// Column order of the deferred MLP's layer-1 input matrix (explained in omerf_mlp.cuh): column -> input index of Eq. 4
+// in the order of DESIGN.md R13 (-1: padding column, weight 0), and its inverse.
+__host__ __device__ constexpr inline int mlp_orig_of_col(int col)
+{
+    const int s = col >> 3, r = col & 7, t = r & 3, i = 2 * s + (r >> 2);
+    if (t == 3) return i < 4 ? 3 + i : -1;
+    if (i == 0) return 7 + t;
+    if (i == 9) return t;
+    return 10 + (3 * ((i - 1) >> 1) + t) * 2 + ((i - 1) & 1);
+}
+__host__ __device__ constexpr inline int mlp_col(int j) // inverse: the column that holds input j
+{
+    for (int col = 0; col < 40; col++)
+        if (mlp_orig_of_col(col) == j) return col;
+    return -1;
+}
+
+
 // Everything a render kernel needs, passed by value as a __grid_constant__ kernel parameter so that
 // scalars and the 883 MLP weights are read through the constant bank (no loads in the MLP).
 struct DevScene {

@@ -38,38 +38,62 @@ __device__ __forceinline__ void mma_x3(float c[4], const uint32_t ahi[4], const 
     mma_tf32(c, ahi, bhi.x, bhi.y);
 }
 
-// MLP input of one ray: [sum w c^d (3), sum w f (4), d (3), sin/cos(2^j d) j = 0..3 (24)]  (R13)
+// Column order of the layer-1 input matrix (K = 34, padded to 40).  An m16n8k8 A fragment gives lane (g, t) the columns
+// 8s + t and 8s + t + 4 of k-step s, i.e. ten values v[2s], v[2s + 1] per row.  The 34 inputs of Eq. 4 (R13:
+// sum w c^d (3), sum w f (4), d (3), sin/cos(2^j d), j = 0..3) are laid out so that one lane can produce its ten values
+// from ONE direction component (no staging through shared memory):
+//   t = 0,1,2 (component c = t):  v = [d_c, sin d_c, cos d_c, sin 2d_c, cos 2d_c, sin 4d_c, cos 4d_c, sin 8d_c, cos 8d_c, acc_t]
+//   t = 3:                        v = [acc_3, acc_4, acc_5, acc_6, -, -, -, -, -, -]   (- : weight 0, any finite value)
+// mlp_pack_kernel (omerf_build.cu) permutes the columns of W0 with mlp_orig_of_col (omerf_device.cuh), so the network is
+// unchanged.
+// d, then sin/cos(2^j d), j = 0..3, of one direction component: v[0..8]
 // FAST: sin/cos of d through the MUFU intrinsics (absolute error 2^-21.4 on [-pi, pi], about 3e-6 after the three angle
 // doublings, i.e. <= 4e-6 on an output colour): used by the renderer (budget 2e-3), not by the smoothness term, which
 // differences G.
 template <bool FAST>
-__device__ __forceinline__ void mlp_input(const float acc[7], float dx, float dy, float dz, float in[OMERF_MLP_IN])
+__device__ __forceinline__ void mlp_encode_component(float d, float v[9])
+{
+    float s, co;
+    if (FAST) __sincosf(d, &s, &co);
+    else sincosf(d, &s, &co); // |d| <= 1: no range-reduction slow path
+    v[0] = d;
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        v[1 + 2 * j] = s;
+        v[2 + 2 * j] = co;
+        const float s2 = 2.0f * s * co, c2 = 1.0f - 2.0f * s * s; // double angle: sin/cos(2^(j+1) d)
+        s = s2;
+        co = c2;
+    }
+}
+
+// All 40 columns of one row (padding columns 0), for kernels that stage rows through shared memory.
+template <bool FAST>
+__device__ __forceinline__ void mlp_input(const float acc[7], float dx, float dy, float dz, float in[40])
 {
 #pragma unroll
-    for (int i = 0; i < 7; i++) in[i] = acc[i];
+    for (int i = 0; i < 40; i++) in[i] = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 7; i++) in[mlp_col(i)] = acc[i];
     const float d[3] = {dx, dy, dz};
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-        in[7 + c] = d[c];
-        float s, co;
-        if (FAST) __sincosf(d[c], &s, &co);
-        else sincosf(d[c], &s, &co); // |d| <= 1: no range-reduction slow path
+        float v[9];
+        mlp_encode_component<FAST>(d[c], v);
+        in[mlp_col(7 + c)] = v[0];
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-            in[10 + (3 * j + c) * 2] = s;
-            in[10 + (3 * j + c) * 2 + 1] = co;
-            const float s2 = 2.0f * s * co, c2 = 1.0f - 2.0f * s * s; // double angle: sin/cos(2^(j+1) d)
-            s = s2;
-            co = c2;
+            in[mlp_col(10 + (3 * j + c) * 2)] = v[1 + 2 * j];
+            in[mlp_col(10 + (3 * j + c) * 2 + 1)] = v[2 + 2 * j];
         }
     }
 }
 
-// Evaluates G for the rays staged by lanes [16*half, 16*half+16) and returns this lane's share of the output
-// C fragment: out[0], out[1] = row g cols 2t, 2t+1; out[2], out[3] = row g+8 (pre-sigmoid; cols >= 3 unused).
-__device__ __forceinline__ void mlp_half(const float2 *__restrict__ tab, const float *X, int lane, float out[4])
+// Evaluates G for 16 rows given as register fragments: v0 = this lane's ten layer-1 values of row g, v1 = of row g + 8
+// (column order above).  Returns this lane's share of the output C fragment: out[0], out[1] = row g cols 2t, 2t+1;
+// out[2], out[3] = row g+8 (pre-sigmoid; cols >= 3 unused).
+__device__ __forceinline__ void mlp_tiles(const float2 *__restrict__ tab, const float v0[10], const float v1[10], int lane, float out[4])
 {
-    const int g = lane >> 2, t = lane & 3;
     float c1[2][4], c2[2][4];
 #pragma unroll
     for (int q = 0; q < 2; q++) {
@@ -83,10 +107,10 @@ __device__ __forceinline__ void mlp_half(const float2 *__restrict__ tab, const f
 #pragma unroll
     for (int s = 0; s < 5; s++) {
         uint32_t ahi[4], alo[4];
-        split_tf32(X[g * OMERF_XS + 8 * s + t], ahi[0], alo[0]);
-        split_tf32(X[(g + 8) * OMERF_XS + 8 * s + t], ahi[1], alo[1]);
-        split_tf32(X[g * OMERF_XS + 8 * s + t + 4], ahi[2], alo[2]);
-        split_tf32(X[(g + 8) * OMERF_XS + 8 * s + t + 4], ahi[3], alo[3]);
+        split_tf32(v0[2 * s], ahi[0], alo[0]);
+        split_tf32(v1[2 * s], ahi[1], alo[1]);
+        split_tf32(v0[2 * s + 1], ahi[2], alo[2]);
+        split_tf32(v1[2 * s + 1], ahi[3], alo[3]);
 #pragma unroll
         for (int q = 0; q < 2; q++) mma_x3(c1[q], ahi, alo, tab, s * 2 + q, lane);
     }
@@ -114,6 +138,21 @@ __device__ __forceinline__ void mlp_half(const float2 *__restrict__ tab, const f
         split_tf32(fmaxf(c2[s][3], 0.0f), ahi[3], alo[3]);
         mma_x3(out, ahi, alo, tab, 14 + s, lane);
     }
+}
+
+// The same for 16 rows staged in shared memory (row stride OMERF_XS, all 40 columns written).
+__device__ __forceinline__ void mlp_half(const float2 *__restrict__ tab, const float *X, int lane, float out[4])
+{
+    const int g = lane >> 2, t = lane & 3;
+    float v0[10], v1[10];
+#pragma unroll
+    for (int s = 0; s < 5; s++) {
+        v0[2 * s] = X[g * OMERF_XS + 8 * s + t];
+        v1[2 * s] = X[(g + 8) * OMERF_XS + 8 * s + t];
+        v0[2 * s + 1] = X[g * OMERF_XS + 8 * s + t + 4];
+        v1[2 * s + 1] = X[(g + 8) * OMERF_XS + 8 * s + t + 4];
+    }
+    mlp_tiles(tab, v0, v1, lane, out);
 }
 
 } // namespace

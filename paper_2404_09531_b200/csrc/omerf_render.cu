@@ -432,12 +432,11 @@ constexpr int OMERF_ENDGAME_BUSY = 32;   // in the endgame a warp takes a new ti
 
 struct WarpPool {
     uint32_t meta[OMERF_POOL]; // status (bits 0-1) | pyramid level (bits 2-6) | view (bits 8-31)
-    float dx[OMERF_POOL], dy[OMERF_POOL], dz[OMERF_POOL];
+    float d[3][OMERF_POOL];    // ray direction
     int k[OMERF_POOL], k1[OMERF_POOL];
     uint32_t Q[OMERF_POOL], n[OMERF_POOL], pix[OMERF_POOL];
     float acc[7][OMERF_POOL];
     uint8_t list[OMERF_POOL]; // slots in the picked state, in slot order (phases other than traversal use the first 32)
-    float X[16 * OMERF_XS]; // staged MLP inputs of 16 rays
 };
 
 __device__ __forceinline__ uint32_t pack_meta(int status, int lvl, uint32_t view)
@@ -486,9 +485,9 @@ __device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P,
     L.view = m >> 8;
     L.k = P.k[s_];
     L.k1 = P.k1[s_];
-    L.r.dx = P.dx[s_];
-    L.r.dy = P.dy[s_];
-    L.r.dz = P.dz[s_];
+    L.r.dx = P.d[0][s_];
+    L.r.dy = P.d[1][s_];
+    L.r.dz = P.d[2][s_];
     ray_origin(oc, cams, L.view, L.r);
     L.r.ix = L.r.dx != 0.0f ? __fdividef(1.0f, L.r.dx) : INFINITY;
     L.r.iy = L.r.dy != 0.0f ? __fdividef(1.0f, L.r.dy) : INFINITY;
@@ -645,9 +644,9 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                     int k, k1;
                     if (setup_ray(sc, cam, u, v, r, k, k1)) {
                         P.meta[slot] = pack_meta(ST_TRAV, start_lvl, view);
-                        P.dx[slot] = r.dx;
-                        P.dy[slot] = r.dy;
-                        P.dz[slot] = r.dz;
+                        P.d[0][slot] = r.dx;
+                        P.d[1][slot] = r.dy;
+                        P.d[2][slot] = r.dz;
                         P.k[slot] = k;
                         P.k1[slot] = k1;
                         P.Q[slot] = 0;
@@ -683,9 +682,9 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                 k1 = P.k1[s_];
                 Q = P.Q[s_];
                 n = P.n[s_];
-                r.dx = P.dx[s_];
-                r.dy = P.dy[s_];
-                r.dz = P.dz[s_];
+                r.dx = P.d[0][s_];
+                r.dy = P.d[1][s_];
+                r.dz = P.d[2][s_];
                 ray_origin(oc, cams, view, r);
 #pragma unroll
                 for (int c = 0; c < 7; c++) acc[c] = P.acc[c][s_];
@@ -772,25 +771,23 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 #pragma unroll 1
             for (int half = 0; half < 2; half++) {
                 if (half * 16 >= n_act) break;
-                if ((lane >> 4) == half) { // stage the inputs of this half's rays (zeros for unused rows)
-                    float in[OMERF_MLP_IN];
+                // layer-1 A fragments straight from the pool (column order of omerf_mlp.cuh): lane (g, t) makes its ten
+                // values of rays g and g + 8 of this half from direction component t (t = 3: the four feature sums)
+                float v[2][10], o[4];
 #pragma unroll
-                    for (int i = 0; i < OMERF_MLP_IN; i++) in[i] = 0.0f;
-                    if (active) {
-                        float acc[7];
-#pragma unroll
-                        for (int c = 0; c < 7; c++) acc[c] = P.acc[c][slot];
-                        mlp_input<true>(acc, P.dx[slot], P.dy[slot], P.dz[slot], in);
+                for (int rr = 0; rr < 2; rr++) {
+                    const int ray = half * 16 + (lane >> 2) + 8 * rr, tq = lane & 3;
+                    const int sl = ray < n_act ? (int)P.list[ray] : slot; // unused rows: any finite values
+                    mlp_encode_component<true>(P.d[min(tq, 2)][sl], v[rr]);
+                    v[rr][9] = P.acc[tq][sl];
+                    if (tq == 3) {
+                        v[rr][0] = v[rr][9];
+                        v[rr][1] = P.acc[4][sl];
+                        v[rr][2] = P.acc[5][sl];
+                        v[rr][3] = P.acc[6][sl];
                     }
-                    float4 *row = reinterpret_cast<float4 *>(P.X + (lane & 15) * OMERF_XS);
-#pragma unroll
-                    for (int i = 0; i < 8; i++) row[i] = make_float4(in[4 * i], in[4 * i + 1], in[4 * i + 2], in[4 * i + 3]);
-                    row[8] = make_float4(in[32], in[33], 0.0f, 0.0f);
-                    row[9] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
                 }
-                __syncwarp();
-                float o[4];
-                mlp_half(sc.mlp_tab, P.X, lane, o);
+                mlp_tiles(sc.mlp_tab, v[0], v[1], lane, o);
                 // lane (g, t): t = 0 holds colours 0,1 and t = 1 colour 2 of rays g and g+8 of this half
                 const int g = lane >> 2, t = lane & 3;
                 if (t < 2) {

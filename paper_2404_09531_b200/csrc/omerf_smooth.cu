@@ -63,9 +63,9 @@ omerf_smooth_kernel(const float2 *__restrict__ mlp_tab, long long n, int S, cons
         for (int p = 0; p < passes; p++) {
             // ---- stage 32 rows: row j = 32 p + lane; j = 0 is the unperturbed direction
             const int j = p * 32 + lane;
-            float in[OMERF_MLP_IN];
+            float in[40];
 #pragma unroll
-            for (int q = 0; q < OMERF_MLP_IN; q++) in[q] = 0.0f;
+            for (int q = 0; q < 40; q++) in[q] = 0.0f;
             float cosv = 0.0f;
             if (j < rows_total) {
                 float sx = dx, sy = dy, sz = dz;
@@ -88,9 +88,7 @@ omerf_smooth_kernel(const float2 *__restrict__ mlp_tab, long long n, int S, cons
             }
             float4 *xr = reinterpret_cast<float4 *>(Xs[w][half] + row * OMERF_XS);
 #pragma unroll
-            for (int q = 0; q < 8; q++) xr[q] = make_float4(in[4 * q], in[4 * q + 1], in[4 * q + 2], in[4 * q + 3]);
-            xr[8] = make_float4(in[32], in[33], 0.0f, 0.0f);
-            xr[9] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            for (int q = 0; q < 10; q++) xr[q] = make_float4(in[4 * q], in[4 * q + 1], in[4 * q + 2], in[4 * q + 3]);
             Ws[w][half][row] = cosv;
             __syncwarp();
             // ---- two tiles of 16 rows through G
