@@ -179,8 +179,8 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
         v.xz_rows = s->band[1] - s->band[0] + 1;
         v.yz_zoff = s->band[2];
         v.yz_rows = s->band[3] - s->band[2] + 1;
-        // S0: features.  8 channels per texel = 8 bytes; stored as 16-byte entries of two texels adjacent along the fastest
-        // axis (omerf_build.cu: pair_layout_kernel).  Only the kept z band of xz / yz is uploaded at all.
+        // S0: features.  8 channels per texel = 8 bytes; stored as 16-byte entries of two texels adjacent along y (V) or the
+        // second axis (planes) (omerf_build.cu: pair_layout_kernel).  Only the kept z band of xz / yz is uploaded at all.
         struct {
             const uint8_t *host;
             size_t rows;
@@ -212,7 +212,9 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
                 rc = omerf_cuda_fail(e, "feature layout");
                 break;
             }
-            if ((rc = omerf_launch_pair_layout(d_raw, *arr[a].dst, arr[a].rows, arr[a].n, 0))) break;
+            if (a == 0) rc = omerf_launch_pair_layout(d_raw, *arr[a].dst, arr[a].rows * arr[a].n, v.G[1], (unsigned long long)v.G[2], 0);
+            else rc = omerf_launch_pair_layout(d_raw, *arr[a].dst, arr[a].rows * arr[a].n, arr[a].n, 1ull, 0);
+            if (rc) break;
             if ((e = cudaDeviceSynchronize()) != cudaSuccess) {
                 rc = omerf_cuda_fail(e, "feature layout");
                 break;

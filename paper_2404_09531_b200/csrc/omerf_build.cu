@@ -9,29 +9,29 @@
 #include "omerf_device.cuh"
 
 // ------------------------------------------------------------------------------------------ S0: gather layout
-// Every feature array is stored as ENTRIES of two texels adjacent along its fastest axis:
-//     dst[r][j] = (src[r][j], src[r][min(j + 1, n - 1)]),   8 + 8 = 16 bytes,
-// so that the two taps a bilinear / trilinear footprint takes along that axis (z for V, the second axis for the planes)
-// arrive with ONE 16-byte load instead of two 8-byte loads: 10 gathers per sample instead of 20 for twice the memory
-// (PAPER.md:186 stores the features as textures; SURVEY 8(a) S0 "re-lay out for gathers").  The clamp reproduces
-// clamp-to-edge addressing (R10) at the last texel; the first texel needs none (omerf_render.cu: axis_tap).
-__global__ void pair_layout_kernel(const uint2 *__restrict__ src, uint4 *__restrict__ dst, unsigned long long rows, int n)
+// Every feature array is stored as ENTRIES of two texels adjacent along one of its axes (y for V, the second axis for the
+// planes):  dst[e] = pair_entry(src[e], src[e + stride]) (the texel itself again at the last index of that axis),
+// 8 + 8 = 16 bytes with the two texels' bytes interleaved channel by channel (omerf_device.cuh: pair_entry).
+// The two taps a bilinear / trilinear footprint takes along that axis arrive with ONE 16-byte load, already in the operand
+// order of the 16-bit x 8-bit dot products that filter them: 10 gathers per sample instead of 20, no byte shuffles, for
+// twice the memory (PAPER.md:186 stores the features as textures; SURVEY 8(a) S0 "re-lay out for gathers").  The repeated
+// texel reproduces clamp-to-edge addressing (R10) at the last index; the first index needs none (omerf_render.cu: axis_tap).
+__global__ void pair_layout_kernel(const uint2 *__restrict__ src, uint4 *__restrict__ dst, unsigned long long total, int n,
+                                   unsigned long long stride)
 {
-    const unsigned long long total = rows * (unsigned long long)n;
     for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < total;
          e += (unsigned long long)gridDim.x * blockDim.x) {
-        const int j = (int)(e % (unsigned long long)n);
-        const uint2 a = src[e], b = src[j + 1 < n ? e + 1 : e];
-        dst[e] = make_uint4(a.x, a.y, b.x, b.y);
+        const int j = (int)((e / stride) % (unsigned long long)n); // coordinate along the paired axis
+        dst[e] = pair_entry(src[e], src[j + 1 < n ? e + stride : e]);
     }
 }
 
-int omerf_launch_pair_layout(const void *d_src, void *d_dst, unsigned long long rows, int n, cudaStream_t st)
+// `total` texels; the paired axis has n texels and element stride `stride` (1: the fastest axis)
+int omerf_launch_pair_layout(const void *d_src, void *d_dst, unsigned long long total, int n, unsigned long long stride, cudaStream_t st)
 {
-    if (rows == 0 || n <= 0) return OMERF_OK;
-    const unsigned long long total = rows * (unsigned long long)n;
+    if (total == 0 || n <= 0) return OMERF_OK;
     const unsigned int blocks = (unsigned int)((total + 255) / 256 < (1u << 20) ? (total + 255) / 256 : (1u << 20));
-    pair_layout_kernel<<<blocks, 256, 0, st>>>((const uint2 *)d_src, (uint4 *)d_dst, rows, n);
+    pair_layout_kernel<<<blocks, 256, 0, st>>>((const uint2 *)d_src, (uint4 *)d_dst, total, n, stride);
     OMERF_CUDA(cudaGetLastError());
     return OMERF_OK;
 }

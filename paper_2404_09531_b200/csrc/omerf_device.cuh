@@ -42,11 +42,13 @@ struct DevScene {
     int n_levels;
     const float2 *pyr;     // all levels, (min of h_lo, max of h_up) per node, [nx][ny] row-major
     int lvl_off[OMERF_MAX_LEVELS], lvl_nx[OMERF_MAX_LEVELS], lvl_ny[OMERF_MAX_LEVELS];
-    // features: 8 uint8 channels per texel = 8 bytes; every array ENTRY is a pair of texels adjacent along the array's
-    // fastest axis, (t[i], t[min(i+1, N-1)]) = one 16-byte word, so the two taps of that axis come with one load (S0 layout)
+    // features: 8 uint8 channels per texel = 8 bytes; every array ENTRY is a pair of texels adjacent along ONE axis of the
+    // array, (t[i], t[min(i+1, N-1)]), with the bytes of the two texels interleaved channel by channel (pair_entry below):
+    // one 16-byte load brings both taps of that axis, already in the operand order of the IDP.2A dot products (S0 layout).
+    // Paired axis: y for V, the second axis for the planes.
     int G[3];
     float gs[3];           // G/box per axis
-    const uint4 *grid;     // dense: [Gx][Gy][Gz] entries (pairs along z); sparse blocks: atlas [id][B][B][B] (omerf_sparse.cu)
+    const uint4 *grid;     // dense: [Gx][Gy][Gz] entries (pairs along y); sparse blocks: atlas [id][B][B][B] (omerf_sparse.cu)
     int blk_shift;         // 0 = dense grid, else log2 of the block edge B
     int nby, nbz;          // block-grid dims along y and z
     const int32_t *blk_table; // [nbx][nby][nbz] block id or -1
@@ -77,6 +79,13 @@ struct DevScene {
     // (k-step*2 + n-tile), 10..13 layer 2, 14..15 layer 3; then 5 bias tiles (layer 1 n-tiles 0,1; layer 2; layer 3).
     const float2 *mlp_tab;
 };
+
+// S0 entry of two texels a, b (8 channels each): bytes (a.c0, b.c0, a.c1, b.c1 | a.c2, b.c2, a.c3, b.c3 | ... c4..c7)
+__device__ __forceinline__ uint4 pair_entry(uint2 a, uint2 b)
+{
+    return make_uint4(__byte_perm(a.x, b.x, 0x5140), __byte_perm(a.x, b.x, 0x7362), __byte_perm(a.y, b.y, 0x5140),
+                      __byte_perm(a.y, b.y, 0x7362));
+}
 
 struct omerf_scene {
     DevScene dev;
@@ -117,7 +126,7 @@ int omerf_cuda_fail(cudaError_t e, const char *what);
 // kernels' host launchers
 int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, cudaStream_t st);
 int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st);
-int omerf_launch_pair_layout(const void *d_src, void *d_dst, unsigned long long rows, int n, cudaStream_t st);
+int omerf_launch_pair_layout(const void *d_src, void *d_dst, unsigned long long total, int n, unsigned long long stride, cudaStream_t st);
 int omerf_lowz_band(const omerf_scene *s, const float *d_lo, const float *d_up, int n_xz, int n_yz, int *band, cudaStream_t st);
 int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream_t st);
 int omerf_launch_mlp_pack(omerf_scene *s, const omerf_scene_desc *d, cudaStream_t st);

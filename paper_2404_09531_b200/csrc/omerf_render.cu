@@ -206,10 +206,10 @@ __device__ __forceinline__ void axis_tap(float p, float s, int &i, uint32_t &w)
 }
 
 // Bilinear footprints as 16-bit x 8-bit dot products (IDP.2A, fma pipe, full rate): the four weights
-// w_ab = (256 - w_a | w_a)(256 - w_b | w_b) are packed as two u16 pairs, the texel bytes of one channel of two
-// texels are brought side by side with one PRMT per two channels.  Only w_00 can reach 2^16 (w_a = w_b = 0; the taps
-// never carry a weight of 256, see axis_tap): it is then stored as 65535 and the missing unit of texel (a0, b0) is added
-// by the caller (`ovf`, a rare branch): the sum stays the exact integer of R9.
+// w_ab = (256 - w_a | w_a)(256 - w_b | w_b) are packed as two u16 pairs (pairs along axis b), and an S0 entry already holds
+// the bytes of texels b0 and b1 side by side per channel (pair_entry), so a channel costs one IDP.2A per row and no byte
+// shuffle.  Only w_00 can reach 2^16 (w_a = w_b = 0; the taps never carry a weight of 256, see axis_tap): it is then
+// stored as 65535 and the missing unit of texel (a0, b0) is added (`ovf`, a rare branch): the sum stays the exact integer of R9.
 struct BiW {
     uint32_t w0, w1; // (w00 | w01 << 16), (w10 | w11 << 16): pairs along axis b for rows a0 and a1
     bool ovf;
@@ -226,68 +226,55 @@ __device__ __forceinline__ BiW bilinear_weights(uint32_t wa, uint32_t wb)
     return r;
 }
 
-// acc[0..7] += sum over the 2x2 footprint of w_ab * texel_ab[c]; ra = texels (a0,b0),(a0,b1), rb = (a1,b0),(a1,b1)
-// (8 channels = 2 words per texel: .x/.y the first texel of the pair, .z/.w the second)
-__device__ __forceinline__ void bilinear8_dp(const uint32_t a0x, const uint32_t a0y, const uint32_t a1x, const uint32_t a1y,
-                                             const uint32_t b0x, const uint32_t b0y, const uint32_t b1x, const uint32_t b1y,
-                                             const BiW w, uint32_t acc[8])
+// acc[0..7] += sum over the 2x2 footprint of w_ab * texel_ab[c]; e0 = entry of row a0 (texels b0, b1), e1 = of row a1
+__device__ __forceinline__ void bilinear8_dp(const uint4 e0, const uint4 e1, const BiW w, uint32_t acc[8])
 {
-    // a0* = texel (a0,b0), a1* = texel (a0,b1), b0* = texel (a1,b0), b1* = texel (a1,b1)
-    uint32_t p, q;
-    p = __byte_perm(a0x, a1x, 0x5140);
-    q = __byte_perm(b0x, b1x, 0x5140);
-    acc[0] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[0]));
-    acc[1] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[1]));
-    p = __byte_perm(a0x, a1x, 0x7362);
-    q = __byte_perm(b0x, b1x, 0x7362);
-    acc[2] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[2]));
-    acc[3] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[3]));
-    p = __byte_perm(a0y, a1y, 0x5140);
-    q = __byte_perm(b0y, b1y, 0x5140);
-    acc[4] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[4]));
-    acc[5] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[5]));
-    p = __byte_perm(a0y, a1y, 0x7362);
-    q = __byte_perm(b0y, b1y, 0x7362);
-    acc[6] = __dp2a_lo(w.w1, q, __dp2a_lo(w.w0, p, acc[6]));
-    acc[7] = __dp2a_hi(w.w1, q, __dp2a_hi(w.w0, p, acc[7]));
-    if (w.ovf) { // w_00 = 2^16 was stored as 2^16 - 1 (probability 2^-16 per footprint)
-        acc[0] += a0x & 255u; acc[1] += (a0x >> 8) & 255u; acc[2] += (a0x >> 16) & 255u; acc[3] += a0x >> 24;
-        acc[4] += a0y & 255u; acc[5] += (a0y >> 8) & 255u; acc[6] += (a0y >> 16) & 255u; acc[7] += a0y >> 24;
+    acc[0] = __dp2a_lo(w.w1, e1.x, __dp2a_lo(w.w0, e0.x, acc[0]));
+    acc[1] = __dp2a_hi(w.w1, e1.x, __dp2a_hi(w.w0, e0.x, acc[1]));
+    acc[2] = __dp2a_lo(w.w1, e1.y, __dp2a_lo(w.w0, e0.y, acc[2]));
+    acc[3] = __dp2a_hi(w.w1, e1.y, __dp2a_hi(w.w0, e0.y, acc[3]));
+    acc[4] = __dp2a_lo(w.w1, e1.z, __dp2a_lo(w.w0, e0.z, acc[4]));
+    acc[5] = __dp2a_hi(w.w1, e1.z, __dp2a_hi(w.w0, e0.z, acc[5]));
+    acc[6] = __dp2a_lo(w.w1, e1.w, __dp2a_lo(w.w0, e0.w, acc[6]));
+    acc[7] = __dp2a_hi(w.w1, e1.w, __dp2a_hi(w.w0, e0.w, acc[7]));
+    if (w.ovf) { // w_00 = 2^16 was stored as 2^16 - 1 (probability 2^-16 per footprint): one more unit of texel (a0, b0)
+        acc[0] += e0.x & 255u; acc[1] += (e0.x >> 16) & 255u; acc[2] += e0.y & 255u; acc[3] += (e0.y >> 16) & 255u;
+        acc[4] += e0.z & 255u; acc[5] += (e0.z >> 16) & 255u; acc[6] += e0.w & 255u; acc[7] += (e0.w >> 16) & 255u;
     }
 }
 
-// Entry indices of the 4 (x,y) corner columns of V at tap z, order x0y0, x0y1, x1y0, x1y1; every entry holds the texels
-// (z, z+1) of its column (S0 layout, omerf_build.cu).  Dense layout: row-major [Gx][Gy][Gz]; sparse blocks (8(f).1):
-// one block-table lookup per corner column, then the entry inside the atlas block (the z+1 texel of an entry was
-// copied from the neighbouring block at bake time, so one lookup serves both z taps).
+// Entry indices of the four (x, z) corners of V at tap y, order x0z0, x0z1, x1z0, x1z1; every entry holds the texels
+// (y, y+1) of its (x, z) (S0 layout, omerf_build.cu).  Dense layout: row-major [Gx][Gy][Gz]; sparse blocks (8(f).1):
+// one block-table lookup per corner, then the entry inside the atlas block (the y+1 texel of an entry was copied from the
+// neighbouring block at bake time, so one lookup serves both y taps).
 template <bool GENERAL>
-__device__ __forceinline__ void grid_corner_offsets(const DevScene &sc, int x0, int x1, int y0, int y1, int z, uint32_t off[4])
+__device__ __forceinline__ void grid_corner_offsets(const DevScene &sc, int x0, int x1, int y, int z0, int z1, uint32_t off[4])
 {
     if (!GENERAL || sc.blk_shift == 0) {
         const uint32_t Gy = (uint32_t)sc.G[1], Gz = (uint32_t)sc.G[2];
-        const uint32_t c0 = (uint32_t)x0 * Gy, c1 = (uint32_t)x1 * Gy;
-        off[0] = (c0 + (uint32_t)y0) * Gz + (uint32_t)z;
-        off[1] = (c0 + (uint32_t)y1) * Gz + (uint32_t)z;
-        off[2] = (c1 + (uint32_t)y0) * Gz + (uint32_t)z;
-        off[3] = (c1 + (uint32_t)y1) * Gz + (uint32_t)z;
+        const uint32_t c0 = ((uint32_t)x0 * Gy + (uint32_t)y) * Gz, c1 = ((uint32_t)x1 * Gy + (uint32_t)y) * Gz;
+        off[0] = c0 + (uint32_t)z0;
+        off[1] = c0 + (uint32_t)z1;
+        off[2] = c1 + (uint32_t)z0;
+        off[3] = c1 + (uint32_t)z1;
     } else {
         const int s = sc.blk_shift, m = (1 << s) - 1;
-        const int xs[2] = {x0, x1}, ys[2] = {y0, y1};
+        const int xs[2] = {x0, x1}, zs[2] = {z0, z1};
 #pragma unroll
         for (int a = 0; a < 2; a++)
 #pragma unroll
             for (int b = 0; b < 2; b++) {
                 // every corner of a sample inside the slab lies in an allocated block (R24); max() only guards memory
-                const int id = max(__ldg(sc.blk_table + ((xs[a] >> s) * sc.nby + (ys[b] >> s)) * sc.nbz + (z >> s)), 0);
-                off[a * 2 + b] = ((uint32_t)id << (3 * s)) + (uint32_t)(((((xs[a] & m) << s) + (ys[b] & m)) << s) + (z & m));
+                const int id = max(__ldg(sc.blk_table + ((xs[a] >> s) * sc.nby + (y >> s)) * sc.nbz + (zs[b] >> s)), 0);
+                off[a * 2 + b] = ((uint32_t)id << (3 * s)) + (uint32_t)(((((xs[a] & m) << s) + (y & m)) << s) + (zs[b] & m));
             }
     }
 }
 
-// The 10 gathers of one sample: every load fetches a PAIR of texels that are adjacent along the array's fastest axis
-// (z for V, the second axis for the planes) as one 16-byte word.
+// The 10 gathers of one sample: every load fetches a PAIR of texels adjacent along y (V) or the second axis (planes) as
+// one 16-byte entry.
 struct Footprints {
-    uint4 g[4];  // V: corner columns x0y0, x0y1, x1y0, x1y1, each (z0 | z1)
+    uint4 g[4];  // V: corners x0z0, x0z1, x1z0, x1z1, each (y0 | y1)
     uint4 p[6];  // xy rows a0, a1; xz rows a0, a1; yz rows a0, a1, each (b0 | b1)
 };
 
@@ -295,16 +282,16 @@ template <bool GENERAL>
 __device__ __forceinline__ void gather_features(const DevScene &sc, float px, float py, float pz, uint32_t I[8])
 {
     // taps and weights of all four sources first, then all 10 loads, then the arithmetic
-    int x0, y0, zi;
+    int x0, y0, z0;
     uint32_t wx, wy, wz;
     axis_tap(px, sc.gs[0], x0, wx);
     axis_tap(py, sc.gs[1], y0, wy);
-    axis_tap(pz, sc.gs[2], zi, wz);
-    const int x1 = min(x0 + 1, sc.G[0] - 1), y1 = min(y0 + 1, sc.G[1] - 1);
+    axis_tap(pz, sc.gs[2], z0, wz);
+    const int x1 = min(x0 + 1, sc.G[0] - 1), z1 = min(z0 + 1, sc.G[2] - 1);
     Footprints f;
     {
         uint32_t off[4];
-        grid_corner_offsets<GENERAL>(sc, x0, x1, y0, y1, zi, off);
+        grid_corner_offsets<GENERAL>(sc, x0, x1, y0, z0, z1, off);
 #pragma unroll
         for (int c = 0; c < 4; c++) f.g[c] = __ldg(sc.grid + off[c]);
     }
@@ -342,15 +329,15 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
     uint32_t A[8], B[8];
 #pragma unroll
     for (int c = 0; c < 8; c++) A[c] = B[c] = 0u;
-    // V: bilinear in (x,y) on the z-slices z0 (.x/.y of every corner column) and z1 (.z/.w)
-    bilinear8_dp(f.g[0].x, f.g[0].y, f.g[1].x, f.g[1].y, f.g[2].x, f.g[2].y, f.g[3].x, f.g[3].y, wg, A);
-    bilinear8_dp(f.g[0].z, f.g[0].w, f.g[1].z, f.g[1].w, f.g[2].z, f.g[2].w, f.g[3].z, f.g[3].w, wg, B);
+    // V: bilinear in (x,y) on the z-slices z0 (entries x0z0, x1z0) and z1 (x0z1, x1z1)
+    bilinear8_dp(f.g[0], f.g[2], wg, A);
+    bilinear8_dp(f.g[1], f.g[3], wg, B);
     // the z lerp rounds once (R9): (256 - wz) A + wz B < 2^32
 #pragma unroll
     for (int c = 0; c < 8; c++) I[c] = ((256u - wz) * A[c] + wz * B[c] + 128u) >> 8;
-    bilinear8_dp(f.p[0].x, f.p[0].y, f.p[0].z, f.p[0].w, f.p[1].x, f.p[1].y, f.p[1].z, f.p[1].w, w1, I);
-    bilinear8_dp(f.p[2].x, f.p[2].y, f.p[2].z, f.p[2].w, f.p[3].x, f.p[3].y, f.p[3].z, f.p[3].w, w2, I);
-    bilinear8_dp(f.p[4].x, f.p[4].y, f.p[4].z, f.p[4].w, f.p[5].x, f.p[5].y, f.p[5].z, f.p[5].w, w3, I);
+    bilinear8_dp(f.p[0], f.p[1], w1, I);
+    bilinear8_dp(f.p[2], f.p[3], w2, I);
+    bilinear8_dp(f.p[4], f.p[5], w3, I);
 }
 
 // per-sample activations (Eq. 3, colour path only): sigmoid(2x) = 1/2 + 1/2 tanh(x) with one MUFU.TANH; the caller
@@ -838,13 +825,13 @@ omerf_gather_probe_kernel(const __grid_constant__ DevScene sc, const omerf_camer
     float px, py, pz;
     lattice_point(r, sc.step, (int)e.y, px, py, pz);
     // the same 10 sixteen-byte loads as gather_features (addresses only; weights are not needed)
-    int x0, y0, zi, xa, ya, za, xb, yb, zb;
+    int x0, y0, z0, xa, ya, za, xb, yb, zb;
     uint32_t w;
     axis_tap(px, sc.gs[0], x0, w);
     axis_tap(py, sc.gs[1], y0, w);
-    axis_tap(pz, sc.gs[2], zi, w);
+    axis_tap(pz, sc.gs[2], z0, w);
     uint32_t off[4];
-    grid_corner_offsets<true>(sc, x0, min(x0 + 1, sc.G[0] - 1), y0, min(y0 + 1, sc.G[1] - 1), zi, off);
+    grid_corner_offsets<true>(sc, x0, min(x0 + 1, sc.G[0] - 1), y0, z0, min(z0 + 1, sc.G[2] - 1), off);
     uint4 t[10];
 #pragma unroll
     for (int q = 0; q < 4; q++) t[q] = __ldg(sc.grid + off[q]);

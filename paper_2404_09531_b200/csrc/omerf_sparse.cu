@@ -74,8 +74,8 @@ __global__ void __launch_bounds__(1024) sparse_scan_kernel(const uint32_t *__res
 }
 
 // one CTA per block of the block grid; allocated blocks copy their B^3 ENTRIES (zeros past the grid edge).  An entry is
-// the texel pair (z, min(z + 1, Gz - 1)) of the dense array (S0 layout, omerf_build.cu): the second texel of a block's last
-// z layer comes from the block above, so the trilinear gather needs one table lookup per corner column.
+// the texel pair (y, min(y + 1, Gy - 1)) of the dense array (S0 layout, omerf_build.cu): the second texel of a block's last
+// y layer comes from the neighbouring block, so the trilinear gather needs one table lookup per (x, z) corner pair.
 __global__ void sparse_copy_kernel(const uint2 *__restrict__ dense, int Gx, int Gy, int Gz, int shift, int nby, int nbz,
                                    const int32_t *__restrict__ table, uint4 *__restrict__ atlas)
 {
@@ -88,9 +88,8 @@ __global__ void sparse_copy_kernel(const uint2 *__restrict__ dense, int Gx, int 
         const int gx = (bx << shift) + x, gy = (by << shift) + y, gz = (bz << shift) + z;
         uint4 t = make_uint4(0u, 0u, 0u, 0u);
         if (gx < Gx && gy < Gy && gz < Gz) {
-            const size_t col = ((size_t)gx * Gy + gy) * Gz;
-            const uint2 a = dense[col + gz], b = dense[col + min(gz + 1, Gz - 1)];
-            t = make_uint4(a.x, a.y, b.x, b.y);
+            const size_t row = (size_t)gx * Gy;
+            t = pair_entry(dense[(row + gy) * Gz + gz], dense[(row + min(gy + 1, Gy - 1)) * Gz + gz]);
         }
         atlas[(size_t)id * vox + v] = t;
     }
