@@ -1,140 +1,139 @@
 // omerf_smooth.cu — view-direction smoothness term (Eq. 9-10) as a batched
 // workload of the deferred MLP G (Eq. 4):
 //     l(d) = sum_s S(d, s) || G(F, s) - G(F, d) ||^2,   s = d + delta,   S = cosine similarity.
-// One warp per viewing direction; its 1 + S evaluations of G run as 16-row tensor-core tiles (omerf_mlp.cuh),
-// two tiles per pass (lanes 0-15 stage one, lanes 16-31 the other).  Row 0 of the first tile is G(F, d).
-// The perturbed direction goes into the encoding as it is (R25).
+// One warp per viewing direction; its 1 + S evaluations of G run as 16-row tensor-core tiles (omerf_mlp.cuh), row 0 of
+// the first tile being G(F, d).  Lane (g, t) builds its layer-1 A fragment of rows g and g + 8 in registers from ONE
+// component of s (column order of omerf_mlp.cuh): nothing is staged through shared memory.  The perturbed direction goes
+// into the encoding as it is (R25).
 #include "omerf_device.cuh"
 #include "omerf_mlp.cuh"
 
 namespace {
 
-#ifndef SMOOTH_WARPS
-#define SMOOTH_WARPS 4
-#endif
+constexpr int SMOOTH_WARPS = 4;
+constexpr int SMOOTH_MIN_BLOCKS = 6; // 80 registers, 24 warps per SM: measured 0.97 ms against 1.13 ms at 4 blocks (121 registers)
 
-#ifndef SMOOTH_MIN_BLOCKS
-#define SMOOTH_MIN_BLOCKS 5
-#endif
+struct SmoothDir {          // what a lane keeps of one direction
+    float d[3];             // the direction
+    float f9, f1, f2, f3;   // F[t] (t = 3: F[3]); F[4..6] for lanes t = 3
+};
+
+__device__ __forceinline__ void smooth_fetch(long long i, int t, const float *__restrict__ F, const float *__restrict__ dir, SmoothDir &q)
+{
+    q.d[0] = __ldg(dir + i * 3 + 0);
+    q.d[1] = __ldg(dir + i * 3 + 1);
+    q.d[2] = __ldg(dir + i * 3 + 2);
+    q.f9 = __ldg(F + i * 7 + t);
+    q.f1 = __ldg(F + i * 7 + 4);
+    q.f2 = __ldg(F + i * 7 + 5);
+    q.f3 = __ldg(F + i * 7 + 6);
+}
+
+// One tile of 16 rows j = 16 tile + (0..15) of direction i (row 0 = d itself): returns this lane's two rows' colours
+// (sigmoid applied; c[0], c[1] = row g cols 2t, 2t+1; c[2], c[3] = row g + 8) and their weights S(d, s) (0 for row 0 and
+// for rows past S).
+__device__ __forceinline__ void smooth_tile(const float2 *__restrict__ tab, const SmoothDir &q, long long i, int S, int tile,
+                                            const float *__restrict__ delta, int lane, float c[4], float w[2])
+{
+    const int g = lane >> 2, t = lane & 3, comp = min(t, 2);
+    float v[2][10];
+#pragma unroll
+    for (int rr = 0; rr < 2; rr++) {
+        const int j = tile * 16 + g + 8 * rr;
+        float sx = q.d[0], sy = q.d[1], sz = q.d[2];
+        w[rr] = 0.0f;
+        if (j > 0 && j <= S) {
+            const float *dl = delta + (i * S + (j - 1)) * 3;
+            sx = __fadd_rn(sx, __ldg(dl + 0));
+            sy = __fadd_rn(sy, __ldg(dl + 1));
+            sz = __fadd_rn(sz, __ldg(dl + 2));
+            const float dot = q.d[0] * sx + q.d[1] * sy + q.d[2] * sz;
+            const float nn = (q.d[0] * q.d[0] + q.d[1] * q.d[1] + q.d[2] * q.d[2]) * (sx * sx + sy * sy + sz * sz);
+            w[rr] = nn > 0.0f ? dot * rsqrtf(nn) : 0.0f;
+        }
+        mlp_encode_component<false>(comp == 0 ? sx : (comp == 1 ? sy : sz), v[rr]);
+        v[rr][9] = q.f9;
+        if (t == 3) {
+            v[rr][0] = q.f9;
+            v[rr][1] = q.f1;
+            v[rr][2] = q.f2;
+            v[rr][3] = q.f3;
+        }
+    }
+    float o[4];
+    mlp_tiles(tab, v[0], v[1], lane, o);
+#pragma unroll
+    for (int k = 0; k < 4; k++) c[k] = sigmoid_fast(o[k]);
+}
+
+// loss terms of this lane's two rows of a tile; lane (g, t): t = 0 holds colours 0,1 and t = 1 colour 2
+__device__ __forceinline__ float smooth_terms(const float c[4], const float w[2], const float G0[3], long long i, int S, int tile,
+                                              int lane, float *__restrict__ out_G)
+{
+    const int g = lane >> 2, t = lane & 3;
+    float loss = 0.0f;
+    if (t < 2) {
+#pragma unroll
+        for (int rr = 0; rr < 2; rr++) {
+            const int j = tile * 16 + g + 8 * rr;
+            if (j <= S) {
+                if (t == 0) {
+                    const float a = c[2 * rr] - G0[0], b = c[2 * rr + 1] - G0[1];
+                    loss += w[rr] * (a * a + b * b);
+                } else {
+                    const float a = c[2 * rr] - G0[2];
+                    loss += w[rr] * a * a;
+                }
+                if (out_G) {
+                    float *og = out_G + (i * (S + 1) + j) * 3;
+                    if (t == 0) {
+                        og[0] = c[2 * rr];
+                        og[1] = c[2 * rr + 1];
+                    } else {
+                        og[2] = c[2 * rr];
+                    }
+                }
+            }
+        }
+    }
+    return loss;
+}
+
+// G(F, d) = row 0 of tile 0: lane 0 holds colours 0,1, lane 1 colour 2
+__device__ __forceinline__ void smooth_G0(const float c[4], float G0[3])
+{
+    const unsigned FULL = 0xffffffffu;
+    G0[0] = __shfl_sync(FULL, c[0], 0);
+    G0[1] = __shfl_sync(FULL, c[1], 0);
+    G0[2] = __shfl_sync(FULL, c[0], 1);
+}
+
+__device__ __forceinline__ float warp_sum(float x)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+
 __global__ void __launch_bounds__(32 * SMOOTH_WARPS, SMOOTH_MIN_BLOCKS)
 omerf_smooth_kernel(const float2 *__restrict__ mlp_tab, long long n, int S, const float *__restrict__ F,
                     const float *__restrict__ dir, const float *__restrict__ delta, float *__restrict__ out_loss,
                     float *__restrict__ out_G)
 {
-    __shared__ float Xs[SMOOTH_WARPS][2][16 * OMERF_XS];
-    __shared__ float Ws[SMOOTH_WARPS][2][16]; // S(d, s) of every staged row (0 for padding rows and for row 0)
-    const unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int half = lane >> 4, row = lane & 15;
-    const long long warps = (long long)gridDim.x * SMOOTH_WARPS;
-    const int rows_total = S + 1, passes = (rows_total + 31) / 32;
-    const int g = lane >> 2, t = lane & 3;
-
-    // inputs of the first pass are fetched one direction ahead, so their DRAM latency overlaps the previous tiles
-    struct In {
-        float f7[7], dx, dy, dz, lx, ly, lz;
-    };
-    auto fetch = [&](long long i, In &q) {
-        if (i >= n) return;
-#pragma unroll
-        for (int c = 0; c < 7; c++) q.f7[c] = __ldg(F + i * 7 + c);
-        q.dx = __ldg(dir + i * 3 + 0);
-        q.dy = __ldg(dir + i * 3 + 1);
-        q.dz = __ldg(dir + i * 3 + 2);
-        q.lx = q.ly = q.lz = 0.0f;
-        if (lane > 0 && lane < rows_total) {
-            const float *dl = delta + (i * S + (lane - 1)) * 3;
-            q.lx = __ldg(dl + 0);
-            q.ly = __ldg(dl + 1);
-            q.lz = __ldg(dl + 2);
+    const int lane = threadIdx.x & 31, t = lane & 3;
+    const long long warps = (long long)gridDim.x * SMOOTH_WARPS, w0 = (long long)blockIdx.x * SMOOTH_WARPS + (threadIdx.x >> 5);
+    const int tiles = (S + 16) / 16;
+    for (long long i = w0; i < n; i += warps) {
+        SmoothDir q;
+        smooth_fetch(i, t, F, dir, q);
+        float G0[3] = {0.0f, 0.0f, 0.0f}, loss = 0.0f;
+        for (int tile = 0; tile < tiles; tile++) {
+            float c[4], w[2];
+            smooth_tile(mlp_tab, q, i, S, tile, delta, lane, c, w);
+            if (tile == 0) smooth_G0(c, G0);
+            loss += smooth_terms(c, w, G0, i, S, tile, lane, out_G);
         }
-    };
-    In cur, nxt;
-    fetch((long long)blockIdx.x * SMOOTH_WARPS + w, nxt);
-    for (long long i = (long long)blockIdx.x * SMOOTH_WARPS + w; i < n; i += warps) {
-        cur = nxt;
-        fetch(i + warps, nxt);
-        float f7[7];
-#pragma unroll
-        for (int c = 0; c < 7; c++) f7[c] = cur.f7[c];
-        const float dx = cur.dx, dy = cur.dy, dz = cur.dz;
-        float G0[3] = {0.f, 0.f, 0.f};
-        float loss = 0.0f;
-        for (int p = 0; p < passes; p++) {
-            // ---- stage 32 rows: row j = 32 p + lane; j = 0 is the unperturbed direction
-            const int j = p * 32 + lane;
-            float in[40];
-#pragma unroll
-            for (int q = 0; q < 40; q++) in[q] = 0.0f;
-            float cosv = 0.0f;
-            if (j < rows_total) {
-                float sx = dx, sy = dy, sz = dz;
-                if (j > 0) {
-                    float lx = cur.lx, ly = cur.ly, lz = cur.lz;
-                    if (p > 0) {
-                        const float *dl = delta + (i * S + (j - 1)) * 3;
-                        lx = __ldg(dl + 0);
-                        ly = __ldg(dl + 1);
-                        lz = __ldg(dl + 2);
-                    }
-                    sx = __fadd_rn(dx, lx);
-                    sy = __fadd_rn(dy, ly);
-                    sz = __fadd_rn(dz, lz);
-                    const float dot = dx * sx + dy * sy + dz * sz;
-                    const float nn = (dx * dx + dy * dy + dz * dz) * (sx * sx + sy * sy + sz * sz);
-                    cosv = nn > 0.0f ? dot * rsqrtf(nn) : 0.0f;
-                }
-                mlp_input<false>(f7, sx, sy, sz, in);
-            }
-            float4 *xr = reinterpret_cast<float4 *>(Xs[w][half] + row * OMERF_XS);
-#pragma unroll
-            for (int q = 0; q < 10; q++) xr[q] = make_float4(in[4 * q], in[4 * q + 1], in[4 * q + 2], in[4 * q + 3]);
-            Ws[w][half][row] = cosv;
-            __syncwarp();
-            // ---- two tiles of 16 rows through G
-#pragma unroll 1
-            for (int tile = 0; tile < 2; tile++) {
-                if (p * 32 + tile * 16 >= rows_total) break;
-                float o[4];
-                mlp_half(mlp_tab, Xs[w][tile], lane, o);
-                // lane (g, t): t = 0 holds colours 0,1 and t = 1 colour 2 of rows g and g + 8 of this tile
-                float c[4];
-#pragma unroll
-                for (int q = 0; q < 4; q++) c[q] = sigmoid_fast(o[q]);
-                if (p == 0 && tile == 0) { // row 0 lives in lanes g = 0 (lane 0: colours 0,1; lane 1: colour 2)
-                    G0[0] = __shfl_sync(FULL, c[0], 0);
-                    G0[1] = __shfl_sync(FULL, c[1], 0);
-                    G0[2] = __shfl_sync(FULL, c[0], 1);
-                }
-#pragma unroll
-                for (int rr = 0; rr < 2; rr++) {
-                    const int r16 = g + 8 * rr;
-                    const int jj = p * 32 + tile * 16 + r16;
-                    if (jj < rows_total && t < 2) {
-                        const float wgt = Ws[w][tile][r16];
-                        if (t == 0) {
-                            const float a = c[2 * rr] - G0[0], b = c[2 * rr + 1] - G0[1];
-                            loss += wgt * (a * a + b * b);
-                        } else {
-                            const float a = c[2 * rr] - G0[2];
-                            loss += wgt * a * a;
-                        }
-                        if (out_G) {
-                            float *og = out_G + (i * rows_total + jj) * 3;
-                            if (t == 0) {
-                                og[0] = c[2 * rr];
-                                og[1] = c[2 * rr + 1];
-                            } else {
-                                og[2] = c[2 * rr];
-                            }
-                        }
-                    }
-                }
-            }
-            __syncwarp();
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) loss += __shfl_xor_sync(FULL, loss, o);
+        loss = warp_sum(loss);
         if (lane == 0) out_loss[i] = loss;
     }
 }
