@@ -85,11 +85,10 @@ __device__ __forceinline__ bool in_box(const DevScene &sc, float px, float py, f
     return px >= 0.0f && px < sc.box[0] && py >= 0.0f && py < sc.box[1] && pz >= 0.0f && pz < sc.box[2];
 }
 
-__device__ __forceinline__ int cell_index(float p, float s, int M)
-{
-    const int i = floor_int(__fmaf_rn(p, s, 0.5f));
-    return min(max(i, 0), M - 1);
-}
+// Nearest grid point of P_o (Eq. 7) for a point INSIDE the box (0 <= p < X): p s < M - 1 exactly (s = fl((M-1)/X),
+// p <= X (1 - 2^-24)), so the rounded fma lies in [1/2, M - 1/2] and the clamp of R1 to [0, M-1] is the identity.  Every
+// lattice index a ray keeps lies inside the box (setup_ray), which is what lets the march drop the clamps and box tests.
+__device__ __forceinline__ int cell_index_in_box(float p, float s) { return floor_int(__fmaf_rn(p, s, 0.5f)); }
 
 __device__ __forceinline__ int voxel_index(float p, float s, int N)
 {
@@ -105,41 +104,60 @@ __device__ __forceinline__ int index_before(float t_end, float inv_step, int k1)
 }
 
 // ---------------------------------------------------------------------------------- S4: one traversal step
+// Per-ray constants of the occupancy-plane traversal (proposals only: they set where a jump is tried, never whether it
+// is taken).  The exit parameter of the node boundary at level-0 cell index b is
+//     t = ((b - 1/2) cell - o) / d = fma((float)b, a, c),   a = cell / d,  c = (-cell / 2 - o) / d   (d = 0: a = 0, c = +inf).
+struct PlaneTrav {
+    float ax, cx, ay, cy;
+    int sx, sy; // 1 if the ray moves towards larger indices, else 0: the boundary a node is left through
+};
+
+__device__ __forceinline__ void plane_trav_setup(const DevScene &sc, const Ray &r, PlaneTrav &q)
+{
+    q.ax = r.dx != 0.0f ? sc.cell_x * r.ix : 0.0f;
+    q.cx = r.dx != 0.0f ? (-0.5f * sc.cell_x - r.ox) * r.ix : INFINITY;
+    q.ay = r.dy != 0.0f ? sc.cell_y * r.iy : 0.0f;
+    q.cy = r.dy != 0.0f ? (-0.5f * sc.cell_y - r.oy) * r.iy : INFINITY;
+    q.sx = r.dx > 0.0f ? 1 : 0;
+    q.sy = r.dy > 0.0f ? 1 : 0;
+}
+
 // sampler PLANE.  One step for a ray in state ST_TRAV (any other status passes through): advances (k, lvl) and returns
 // ST_READY when lattice sample k passes the predicate (Eq. 7), ST_FIN when no sample is left, ST_TRAV otherwise.
-//   inside the node's [min,max]:  level 0 -> the sample is occupied if it is in the box, else k+1; level > 0 -> descend 2
+//   inside the node's [min,max]:  level 0 -> the sample is occupied; level > 0 -> descend
 //   outside:  propose a jump to the node's xy exit or to where z reaches the range; if the last index before that
 //             (kk) is verified to lie in the same node on the same side, k = kk+1 and the level follows the boundary
 //             crossed (entering the z-range: descend OMERF_LVL_ENTER; an xy boundary: ascend OMERF_LVL_UP);
 //             otherwise descend OMERF_LVL_FAIL levels, or k+1 at level 0.
+// Every index in [k, k1] is inside the box (setup_ray), so cell indices need no clamp and the predicate no box test.
 // Written without branches (selects only): the warp does not serialise the inside / jump / descend paths.
-__device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl, int status)
+__device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r, const PlaneTrav &q, int &k, int k1, int &lvl,
+                                               int status)
 {
     const bool run = status == ST_TRAV && k <= k1;
-    float px, py, pz;
-    lattice_point(r, sc.step, k, px, py, pz);
-    const int top = sc.n_levels - 1;
-    const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
-    const int nx = ix >> lvl, ny = iy >> lvl;
-    const float2 h = __ldg(sc.pyr + sc.lvl_off[lvl] + nx * sc.lvl_ny[lvl] + ny);
-    const bool above = pz > h.y, below = pz < h.x, inside = !above && !below;
-    const int bxi = nx + (r.dx > 0.0f ? 1 : 0), byi = ny + (r.dy > 0.0f ? 1 : 0);
-    const float xb = fmaf((float)(bxi << lvl), sc.cell_x, -0.5f * sc.cell_x);
-    const float yb = fmaf((float)(byi << lvl), sc.cell_y, -0.5f * sc.cell_y);
-    const float tx = r.dx != 0.0f ? (xb - r.ox) * r.ix : INFINITY;
-    const float ty = r.dy != 0.0f ? (yb - r.oy) * r.iy : INFINITY;
-    float tz = INFINITY;
-    if (above && !below && r.dz < 0.0f) tz = (h.y - r.oz) * r.iz;
-    if (below && !above && r.dz > 0.0f) tz = (h.x - r.oz) * r.iz;
+    const float t = __fmul_rn(__fadd_rn(__int2float_rn(k), 0.5f), sc.step);
+    const float px = __fmaf_rn(t, r.dx, r.ox), py = __fmaf_rn(t, r.dy, r.oy), pz = __fmaf_rn(t, r.dz, r.oz);
+    const int nx = cell_index_in_box(px, sc.sx) >> lvl, ny = cell_index_in_box(py, sc.sy) >> lvl;
+    float2 h = make_float2(0.0f, 0.0f);
+    if (run) h = __ldg(sc.pyr + (uint32_t)(sc.lvl_off[lvl] + nx * sc.lvl_ny[lvl] + ny)); // lanes without a ray load nothing
+    const bool above = pz > h.y, below = pz < h.x, inside = !(above || below);
+    const float tx = fmaf((float)((nx + q.sx) << lvl), q.ax, q.cx);
+    const float ty = fmaf((float)((ny + q.sy) << lvl), q.ay, q.cy);
+    // where z reaches the side of the range the point is outside of; in the past (or NaN / -inf when dz = 0): never
+    const float tzr = ((above ? h.y : h.x) - r.oz) * r.iz;
+    const float tz = tzr > t ? tzr : INFINITY;
     const float txy = fminf(tx, ty);
     const int kk = index_before(fminf(txy, tz), sc.inv_step, k1);
     float qx, qy, qz;
     lattice_point(r, sc.step, kk, qx, qy, qz);
-    const int jx = cell_index(qx, sc.sx, sc.Mx) >> lvl, jy = cell_index(qy, sc.sy, sc.My) >> lvl;
-    const bool same_side = (above ? qz > h.y : true) && (below ? qz < h.x : true);
+    const int jx = cell_index_in_box(qx, sc.sx) >> lvl, jy = cell_index_in_box(qy, sc.sy) >> lvl; // kk in (k, k1] when it counts
+    // z is monotone along the ray: both ends above the node's maximum (or both below its minimum) and in the node means
+    // every index between them is too.  For an empty node (max < min) "above" alone proves it.
+    const bool same_side = above ? qz > h.y : qz < h.x;
     const bool jump = !inside && kk > k && jx == nx && jy == ny && same_side;
-    const bool ready = run && inside && lvl == 0 && in_box(sc, px, py, pz);
+    const bool ready = run && inside && lvl == 0;
     // next (k, lvl)
+    const int top = sc.n_levels - 1;
     const int lvl_jump = tz <= txy ? max(lvl - OMERF_LVL_ENTER, 0) : min(lvl + OMERF_LVL_UP, top);
     const int lvl_next = inside ? max(lvl - OMERF_LVL_INSIDE, 0) : (jump ? lvl_jump : max(lvl - OMERF_LVL_FAIL, 0));
     const int k_next = jump ? kk + 1 : ((lvl == 0 && !ready) ? k + 1 : k); // level 0 and the predicate is false at k
@@ -397,6 +415,56 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
     const float fb = ceilf(t1 * sc.inv_step - 0.5f) + 2.0f;
     k = fa > 0.0f ? (int)fminf(fa, 1.0e9f) : 0;
     k1 = (int)fminf(fb, 1.0e9f);
+    if (k > k1) return false;
+    // The exact index range inside the box.  Every component of the lattice point is monotone in the index (rounding is
+    // monotone), so "entered the box" (per axis: past the face the ray comes in through) is false..false true..true and
+    // "not yet left" is true..true false..false: the indices inside the box are [first entered, last not yet left].
+    // A few linear probes (the padding is 2 indices), then bisection (rays that graze a face).
+    auto entered = [&](int i) {
+        float px, py, pz;
+        lattice_point(r, sc.step, i, px, py, pz);
+        return (r.dx >= 0.0f ? px >= 0.0f : px < sc.box[0]) && (r.dy >= 0.0f ? py >= 0.0f : py < sc.box[1]) &&
+               (r.dz >= 0.0f ? pz >= 0.0f : pz < sc.box[2]);
+    };
+    auto not_left = [&](int i) {
+        float px, py, pz;
+        lattice_point(r, sc.step, i, px, py, pz);
+        return (r.dx >= 0.0f ? px < sc.box[0] : px >= 0.0f) && (r.dy >= 0.0f ? py < sc.box[1] : py >= 0.0f) &&
+               (r.dz >= 0.0f ? pz < sc.box[2] : pz >= 0.0f);
+    };
+    if (!entered(k1) || !not_left(k)) return false;
+    {
+        int lo = k; // first entered index is in [lo, hi]
+        int hi = k1;
+#pragma unroll 1
+        for (int it = 0; it < 4 && lo < hi; it++) {
+            if (entered(lo)) hi = lo;
+            else lo++;
+        }
+#pragma unroll 1
+        while (lo < hi) {
+            const int mid = lo + ((hi - lo) >> 1);
+            if (entered(mid)) hi = mid;
+            else lo = mid + 1;
+        }
+        k = lo;
+    }
+    {
+        int lo = k - 1; // last index not yet left is in [lo, hi]; lo = k - 1 stands for "none at or after k"
+        int hi = k1;
+#pragma unroll 1
+        for (int it = 0; it < 4 && lo < hi; it++) {
+            if (not_left(hi)) lo = hi;
+            else hi--;
+        }
+#pragma unroll 1
+        while (lo < hi) {
+            const int mid = hi - ((hi - lo) >> 1);
+            if (not_left(mid)) lo = mid;
+            else hi = mid - 1;
+        }
+        k1 = hi;
+    }
     return k <= k1;
 }
 
@@ -457,6 +525,7 @@ __device__ __forceinline__ void ray_origin(OriginCache &oc, const omerf_camera *
 
 struct TravLane {
     Ray r;
+    PlaneTrav q;
     int k, k1, lvl, status, slot; // slot < 0: the lane holds no ray
     uint32_t view;
 };
@@ -479,6 +548,7 @@ __device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P,
     L.r.ix = L.r.dx != 0.0f ? __fdividef(1.0f, L.r.dx) : INFINITY;
     L.r.iy = L.r.dy != 0.0f ? __fdividef(1.0f, L.r.dy) : INFINITY;
     L.r.iz = L.r.dz != 0.0f ? __fdividef(1.0f, L.r.dz) : INFINITY;
+    plane_trav_setup(sc, L.r, L.q);
 }
 
 __device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, const TravLane &L, float *__restrict__ out_rgb,
@@ -510,7 +580,7 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
 #pragma unroll 1
     for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
         if (SAMPLER == OMERF_SAMPLER_PLANE) {
-            L.status = trav_step_plane(sc, L.r, L.k, L.k1, L.lvl, L.status);
+            L.status = trav_step_plane(sc, L.r, L.q, L.k, L.k1, L.lvl, L.status);
         } else {
             L.status = trav_step_grid(sc, L.r, L.k, L.k1, L.lvl, L.status);
         }
@@ -701,16 +771,18 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                     if (SAMPLER == OMERF_SAMPLER_PLANE) {
                         float qx, qy, qz;
                         lattice_point(r, sc.step, k + 1, qx, qy, qz);
-                        const int ix = cell_index(qx, sc.sx, sc.Mx), iy = cell_index(qy, sc.sy, sc.My);
-                        const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
-                        next_ready = k < k1 && h.x <= qz && qz <= h.y && in_box(sc, qx, qy, qz);
+                        if (k < k1) { // k + 1 is inside the box then (setup_ray): no clamp, no box test
+                            const int ix = cell_index_in_box(qx, sc.sx), iy = cell_index_in_box(qy, sc.sy);
+                            const float2 h = __ldg(sc.pyr + (uint32_t)(ix * sc.My + iy));
+                            next_ready = h.x <= qz && qz <= h.y;
+                        }
                     }
                     float soft_m = 1.0f;
                     if (GENERAL && SAMPLER == OMERF_SAMPLER_PLANE && sc.soft_eps > 0.0f) {
                         // Eq. 6 (q = 2) at the nearest grid point of P_o (Eq. 7): the sample is inside [z_min, z_max],
                         // so M = min(1, ((z - z_min)/eps)^2, ((z_max - z)/eps)^2); it weights the colours only (Eq. 8)
-                        const int ix = cell_index(px, sc.sx, sc.Mx), iy = cell_index(py, sc.sy, sc.My);
-                        const float2 h = __ldg(sc.pyr + ix * sc.My + iy);
+                        const int ix = cell_index_in_box(px, sc.sx), iy = cell_index_in_box(py, sc.sy);
+                        const float2 h = __ldg(sc.pyr + (uint32_t)(ix * sc.My + iy));
                         const float m = __saturatef(fminf(pz - h.x, h.y - pz) * sc.inv_soft_eps);
                         soft_m = m * m;
                     }
