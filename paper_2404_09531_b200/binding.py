@@ -25,7 +25,7 @@ EXPORTS = (
     "omerf_scene_create", "omerf_render", "omerf_render_tiles", "omerf_render_host", "omerf_gather_probe", "omerf_mlp_smoothness", "omerf_heatmap",
     "omerf_last_launch_count",
     "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield", "omerf_scene_get_block_table",
-    "omerf_scene_destroy", "omerf_last_error", "omerf_version",
+    "omerf_scene_destroy", "omerf_last_error", "omerf_version", "omerf_check_errors",
 )
 
 
@@ -74,6 +74,7 @@ def load_library() -> C.CDLL:
     L = C.CDLL(LIB_PATH)
     L.omerf_last_error.restype = C.c_char_p
     L.omerf_version.restype = C.c_char_p
+    L.omerf_check_errors.restype = C.c_uint32
     L.omerf_scene_create.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
     L.omerf_render.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
     L.omerf_render_host.argtypes = L.omerf_render.argtypes

@@ -226,7 +226,13 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
             else s->plane_bytes += raw_bytes * 2;
         }
         if (rc) break;
-        if (!d->grid_block) v.grid = (const uint4 *)s->d_grid;
+        if (!d->grid_block) {
+            v.grid = (const uint4 *)s->d_grid;
+            v.n_grid = (uint32_t)((size_t)v.G[0] * v.G[1] * v.G[2]);
+        }
+        v.n_pxy = (uint32_t)((size_t)v.xy_n[0] * v.xy_n[1]);
+        v.n_pxz = (uint32_t)((size_t)v.xz_n[0] * v.xz_rows);
+        v.n_pyz = (uint32_t)((size_t)v.yz_n[0] * v.yz_rows);
         v.pxy = (const uint4 *)s->d_pxy;
         v.pxz = (const uint4 *)s->d_pxz;
         v.pyz = (const uint4 *)s->d_pyz;

@@ -161,6 +161,7 @@ int omerf_launch_pyramid(omerf_scene *s, const float *d_lo, const float *d_up, c
         return OMERF_ERR_INVALID;
     }
     v.n_levels = L;
+    v.n_pyr = (uint32_t)total;
     OMERF_CUDA(cudaMalloc(&s->d_pyr, total * sizeof(float2)));
     s->device_bytes += total * sizeof(float2);
     v.pyr = (const float2 *)s->d_pyr;
@@ -289,6 +290,7 @@ int omerf_launch_bitfield(omerf_scene *s, cudaStream_t st)
         nz = (nz + 1) / 2;
     }
     v.occ_levels = L;
+    v.n_occ_words = total_words;
     OMERF_CUDA(cudaMalloc(&s->d_occ, total_words * 4 + 16));
     s->device_bytes += total_words * 4;
     v.occ = (const uint32_t *)s->d_occ;

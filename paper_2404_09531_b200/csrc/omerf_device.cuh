@@ -78,6 +78,9 @@ struct DevScene {
     // (omerf_build.cu: mlp_pack_kernel).  tab[(tile*2 + part)*32 + lane], part 0 = hi, 1 = lo; tiles 0..9 layer 1
     // (k-step*2 + n-tile), 10..13 layer 2, 14..15 layer 3; then 5 bias tiles (layer 1 n-tiles 0,1; layer 2; layer 3).
     const float2 *mlp_tab;
+    // element counts of the arrays above, for the range checks of the OMERF_CHECKED build (omerf_render.cu)
+    uint32_t n_pyr, n_grid, n_pxy, n_pxz, n_pyz, n_blk;
+    unsigned long long n_occ_words;
 };
 
 // S0 entry of two texels a, b (8 channels each): bytes (a.c0, b.c0, a.c1, b.c1 | a.c2, b.c2, a.c3, b.c3 | ... c4..c7)

@@ -31,6 +31,39 @@
 #include "omerf_device.cuh"
 #include "omerf_mlp.cuh"
 
+// OMERF_CHECKED build (libomerf_checked.so; paper_2404_09531_b200/build.py: build(checked=True)): every global-memory
+// index and every pool slot the render kernels use is range-checked on the device.  A violation sets a bit of
+// omerf_check_word (read and cleared by omerf_check_errors) and the access goes to element 0 instead, so the run
+// completes and reports.  This is the stand-in for compute-sanitizer memcheck, which is closed on the GPU pool
+// (profiles/r02_checked_build.md); the shipped library compiles the checks away.
+enum : int { CHK_PYR = 0, CHK_GRID, CHK_PXY, CHK_PXZ, CHK_PYZ, CHK_BLK, CHK_OCC, CHK_VIEW, CHK_PIXEL, CHK_SLOT, CHK_LIST };
+#ifdef OMERF_CHECKED
+__device__ unsigned int omerf_check_word = 0u;
+template <typename T>
+__device__ __forceinline__ T chk(T i, unsigned long long n, int code)
+{
+    if ((unsigned long long)i >= n) {
+        atomicOr(&omerf_check_word, 1u << code);
+        return (T)0;
+    }
+    return i;
+}
+#else
+#define chk(i, n, code) (i)
+#endif
+
+extern "C" unsigned int omerf_check_errors(void)
+{
+#ifdef OMERF_CHECKED
+    unsigned int w = 0xffffffffu, zero = 0u;
+    if (cudaDeviceSynchronize() != cudaSuccess || cudaMemcpyFromSymbol(&w, omerf_check_word, sizeof w) != cudaSuccess) return 0xffffffffu;
+    cudaMemcpyToSymbol(omerf_check_word, &zero, sizeof zero);
+    return w;
+#else
+    return 0u;
+#endif
+}
+
 namespace {
 
 enum : int { ST_IDLE = 0, ST_TRAV = 1, ST_READY = 2, ST_FIN = 3 };
@@ -139,7 +172,7 @@ __device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r,
     const float px = __fmaf_rn(t, r.dx, r.ox), py = __fmaf_rn(t, r.dy, r.oy), pz = __fmaf_rn(t, r.dz, r.oz);
     const int nx = cell_index_in_box(px, sc.sx) >> lvl, ny = cell_index_in_box(py, sc.sy) >> lvl;
     float2 h = make_float2(0.0f, 0.0f);
-    if (run) h = __ldg(sc.pyr + (uint32_t)(sc.lvl_off[lvl] + nx * sc.lvl_ny[lvl] + ny)); // lanes without a ray load nothing
+    if (run) h = __ldg(sc.pyr + chk((uint32_t)(sc.lvl_off[lvl] + nx * sc.lvl_ny[lvl] + ny), sc.n_pyr, CHK_PYR)); // lanes without a ray load nothing
     const bool above = pz > h.y, below = pz < h.x, inside = !(above || below);
     const float tx = fmaf((float)((nx + q.sx) << lvl), q.ax, q.cx);
     const float ty = fmaf((float)((ny + q.sy) << lvl), q.ay, q.cy);
@@ -171,7 +204,7 @@ __device__ __forceinline__ int trav_step_plane(const DevScene &sc, const Ray &r,
 __device__ __forceinline__ bool occ_test(const DevScene &sc, int lvl, int jx, int jy, int jz)
 {
     unsigned long long idx = ((unsigned long long)jx * sc.occ_ny[lvl] + jy) * sc.occ_nz[lvl] + jz;
-    return (__ldg(sc.occ + sc.occ_off[lvl] + (idx >> 5)) >> (idx & 31)) & 1u;
+    return (__ldg(sc.occ + chk(sc.occ_off[lvl] + (idx >> 5), sc.n_occ_words, CHK_OCC)) >> (idx & 31)) & 1u;
 }
 
 // sampler GRID (config-4 comparator): multi-resolution binary occupancy grid, DDA-style skipping.
@@ -283,7 +316,7 @@ __device__ __forceinline__ void grid_corner_offsets(const DevScene &sc, int x0, 
 #pragma unroll
             for (int b = 0; b < 2; b++) {
                 // every corner of a sample inside the slab lies in an allocated block (R24); max() only guards memory
-                const int id = max(__ldg(sc.blk_table + ((xs[a] >> s) * sc.nby + (y >> s)) * sc.nbz + (zs[b] >> s)), 0);
+                const int id = max(__ldg(sc.blk_table + chk((uint32_t)(((xs[a] >> s) * sc.nby + (y >> s)) * sc.nbz + (zs[b] >> s)), sc.n_blk, CHK_BLK)), 0);
                 off[a * 2 + b] = ((uint32_t)id << (3 * s)) + (uint32_t)(((((xs[a] & m) << s) + (y & m)) << s) + (zs[b] & m));
             }
     }
@@ -311,7 +344,7 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
         uint32_t off[4];
         grid_corner_offsets<GENERAL>(sc, x0, x1, y0, z0, z1, off);
 #pragma unroll
-        for (int c = 0; c < 4; c++) f.g[c] = __ldg(sc.grid + off[c]);
+        for (int c = 0; c < 4; c++) f.g[c] = __ldg(sc.grid + chk(off[c], sc.n_grid, CHK_GRID));
     }
     // triplanes: xy sampled with (x,y), xz with (x,z), yz with (y,z).  When the planes share their resolution per
     // world axis (every config: xy A x A, xz and yz A x B) a tap computed for one plane is the other plane's tap too
@@ -334,12 +367,12 @@ __device__ __forceinline__ void gather_features(const DevScene &sc, float px, fl
         const uint32_t xa1 = (uint32_t)min(xa + 1, sc.xy_n[0] - 1), xb1 = (uint32_t)min(xb + 1, sc.xz_n[0] - 1),
                        yb1 = (uint32_t)min(yb + 1, sc.yz_n[0] - 1);
         const uint32_t zr = (uint32_t)(za - sc.xz_zoff), zs = (uint32_t)(zb - sc.yz_zoff); // low-z bake: rows below the band are not stored
-        f.p[0] = __ldg(sc.pxy + ((uint32_t)xa * Nxy + (uint32_t)ya));
-        f.p[1] = __ldg(sc.pxy + (xa1 * Nxy + (uint32_t)ya));
-        f.p[2] = __ldg(sc.pxz + ((uint32_t)xb * Nxz + zr));
-        f.p[3] = __ldg(sc.pxz + (xb1 * Nxz + zr));
-        f.p[4] = __ldg(sc.pyz + ((uint32_t)yb * Nyz + zs));
-        f.p[5] = __ldg(sc.pyz + (yb1 * Nyz + zs));
+        f.p[0] = __ldg(sc.pxy + chk((uint32_t)xa * Nxy + (uint32_t)ya, sc.n_pxy, CHK_PXY));
+        f.p[1] = __ldg(sc.pxy + chk(xa1 * Nxy + (uint32_t)ya, sc.n_pxy, CHK_PXY));
+        f.p[2] = __ldg(sc.pxz + chk((uint32_t)xb * Nxz + zr, sc.n_pxz, CHK_PXZ));
+        f.p[3] = __ldg(sc.pxz + chk(xb1 * Nxz + zr, sc.n_pxz, CHK_PXZ));
+        f.p[4] = __ldg(sc.pyz + chk((uint32_t)yb * Nyz + zs, sc.n_pyz, CHK_PYZ));
+        f.p[5] = __ldg(sc.pyz + chk(yb1 * Nyz + zs, sc.n_pyz, CHK_PYZ));
     }
     const BiW wg = bilinear_weights(wx, wy);
     const BiW w1 = bilinear_weights(xw, yw), w2 = bilinear_weights(xbw, zw), w3 = bilinear_weights(ybw, zbw);
@@ -506,17 +539,22 @@ __device__ __forceinline__ uint32_t pack_meta(int status, int lvl, uint32_t view
 // visit ends when the list is exhausted and fewer than OMERF_TRAV_KEEP lanes still traverse, or after
 // OMERF_TRAV_STEPS steps (occupied rays then get their samples).
 // per-lane cache of the camera origin of the view last used (rays of one lane almost always share the view)
+struct LaunchBounds { // what the OMERF_CHECKED build checks views and pixels against
+    uint32_t n_views;
+    unsigned long long n_pix;
+};
 struct OriginCache {
     uint32_t view;
     float ox, oy, oz;
 };
-__device__ __forceinline__ void ray_origin(OriginCache &oc, const omerf_camera *__restrict__ cams, uint32_t view, Ray &r)
+__device__ __forceinline__ void ray_origin(OriginCache &oc, const omerf_camera *__restrict__ cams, const LaunchBounds &lb, uint32_t view, Ray &r)
 {
     if (view != oc.view) {
         oc.view = view;
-        oc.ox = __ldg(&cams[view].origin[0]);
-        oc.oy = __ldg(&cams[view].origin[1]);
-        oc.oz = __ldg(&cams[view].origin[2]);
+        const omerf_camera *cam = cams + chk(view, lb.n_views, CHK_VIEW);
+        oc.ox = __ldg(&cam->origin[0]);
+        oc.oy = __ldg(&cam->origin[1]);
+        oc.oz = __ldg(&cam->origin[2]);
     }
     r.ox = oc.ox;
     r.oy = oc.oy;
@@ -531,10 +569,10 @@ struct TravLane {
 };
 
 __device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P, const omerf_camera *__restrict__ cams,
-                                          OriginCache &oc, int slot, TravLane &L)
+                                          const LaunchBounds &lb, OriginCache &oc, int slot, TravLane &L)
 {
     L.slot = slot;
-    const int s_ = slot < 0 ? 0 : slot; // idle lanes read slot 0 and step nothing
+    const int s_ = slot < 0 ? 0 : chk(slot, OMERF_POOL, CHK_SLOT); // idle lanes read slot 0 and step nothing
     const uint32_t m = P.meta[s_];
     L.status = slot < 0 ? ST_IDLE : ST_TRAV;
     L.lvl = (int)((m >> 2) & 31u);
@@ -544,20 +582,20 @@ __device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P,
     L.r.dx = P.d[0][s_];
     L.r.dy = P.d[1][s_];
     L.r.dz = P.d[2][s_];
-    ray_origin(oc, cams, L.view, L.r);
+    ray_origin(oc, cams, lb, L.view, L.r);
     L.r.ix = L.r.dx != 0.0f ? __fdividef(1.0f, L.r.dx) : INFINITY;
     L.r.iy = L.r.dy != 0.0f ? __fdividef(1.0f, L.r.dy) : INFINITY;
     L.r.iz = L.r.dz != 0.0f ? __fdividef(1.0f, L.r.dz) : INFINITY;
     plane_trav_setup(sc, L.r, L.q);
 }
 
-__device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, const TravLane &L, float *__restrict__ out_rgb,
-                                           uint32_t *__restrict__ out_n)
+__device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, const LaunchBounds &lb, const TravLane &L,
+                                           float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
 {
-    const int s_ = L.slot;
+    const int s_ = chk(L.slot, OMERF_POOL, CHK_SLOT);
     int st_ = L.status;
     if (st_ == ST_FIN && P.n[s_] == 0) { // no sample at all: background exactly, MLP skipped (R14)
-        const size_t pix = P.pix[s_];
+        const size_t pix = chk((size_t)P.pix[s_], lb.n_pix, CHK_PIXEL);
         out_rgb[pix * 3 + 0] = sc.bg[0];
         out_rgb[pix * 3 + 1] = sc.bg[1];
         out_rgb[pix * 3 + 2] = sc.bg[2];
@@ -569,13 +607,13 @@ __device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, cons
 }
 
 template <int SAMPLER>
-__device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, const omerf_camera *__restrict__ cams,
+__device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, const omerf_camera *__restrict__ cams, const LaunchBounds &lb,
                                            OriginCache &oc, int lane, int n_sel, int keep, float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
 {
     const unsigned FULL = 0xffffffffu;
     const unsigned lt_mask = (1u << lane) - 1u;
     TravLane L;
-    trav_load(sc, P, cams, oc, lane < n_sel ? (int)P.list[lane] : -1, L);
+    trav_load(sc, P, cams, lb, oc, lane < n_sel ? (int)P.list[lane] : -1, L);
     int next = min(n_sel, 32); // first list entry not yet taken
 #pragma unroll 1
     for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
@@ -591,9 +629,9 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
             const unsigned fm = ~going;
             if (__popc(fm) >= OMERF_TRAV_SWAP) {
                 if (free_lane) {
-                    if (L.slot >= 0) trav_store(sc, P, L, out_rgb, out_n);
+                    if (L.slot >= 0) trav_store(sc, P, lb, L, out_rgb, out_n);
                     const int idx = next + __popc(fm & lt_mask);
-                    trav_load(sc, P, cams, oc, idx < n_sel ? (int)P.list[idx] : -1, L);
+                    trav_load(sc, P, cams, lb, oc, idx < n_sel ? (int)P.list[idx] : -1, L);
                 }
                 next = min(next + __popc(fm), n_sel);
             }
@@ -601,7 +639,7 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
             break;
         }
     }
-    if (L.slot >= 0) trav_store(sc, P, L, out_rgb, out_n);
+    if (L.slot >= 0) trav_store(sc, P, lb, L, out_rgb, out_n);
 }
 
 constexpr int OMERF_MIN_BLOCKS = 5;
@@ -628,6 +666,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
     for (int j = 0; j < OMERF_PJ; j++) P.meta[lane + 32 * j] = ST_IDLE;
     __syncwarp();
     bool more = true;
+    const LaunchBounds lb = {(uint32_t)n_views, (unsigned long long)n_views * (unsigned long long)W * (unsigned long long)H};
     OriginCache oc = {0xffffffffu, 0.0f, 0.0f, 0.0f};
     // Endgame: a warp's pool holds about three tiles of work, which would all drain at falling utilisation once the
     // tile counter runs out.  For the last tiles, warps refill only when (nearly) empty, so the remaining work
@@ -673,14 +712,14 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 #pragma unroll
             for (int j = 0; j < OMERF_PJ; j++) {
                 const int pos = base + __popc(b[j] & lt_mask);
-                if ((b[j] >> lane) & 1u) P.list[pos] = (uint8_t)(lane + 32 * j);
+                if ((b[j] >> lane) & 1u) P.list[chk(pos, OMERF_POOL, CHK_LIST)] = (uint8_t)(lane + 32 * j);
                 base += __popc(b[j]);
             }
         }
         __syncwarp();
         const int n_act = min(n_sel, 32);
         const bool active = lane < n_act;
-        const int slot = active ? (int)P.list[lane] : 0;
+        const int slot = active ? chk((int)P.list[lane], OMERF_POOL, CHK_SLOT) : 0;
 
         if (phase == ST_IDLE) {
             // ---- refill: one 8x4 tile -> 32 new rays (S2, S3)
@@ -695,8 +734,8 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                 const int ty = (int)(tv / (unsigned)tiles_x), tx = (int)(tv - (unsigned)ty * tiles_x);
                 const int u = tx * 8 + (lane & 7), v = ty * 4 + (lane >> 3);
                 if (u < W && v < H) {
-                    const omerf_camera cam = cams[view];
-                    const size_t pix = ((size_t)view * H + v) * W + u;
+                    const omerf_camera cam = cams[chk(view, lb.n_views, CHK_VIEW)];
+                    const size_t pix = chk(((size_t)view * H + v) * W + u, lb.n_pix, CHK_PIXEL);
                     Ray r;
                     int k, k1;
                     if (setup_ray(sc, cam, u, v, r, k, k1)) {
@@ -722,7 +761,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
         } else if (phase == ST_TRAV) {
             // ---- traversal visit (S4).  (Two rays per lane, interleaved dependency chains, was measured slower on
             // B200 at every threshold: 0.80-0.86 ms against 0.76 ms per configs[1] frame.)
-            trav_visit<SAMPLER>(sc, P, cams, oc, lane, n_sel, (more && !endgame) ? OMERF_TRAV_KEEP : OMERF_DRAIN_TRAV_KEEP, out_rgb, out_n);
+            trav_visit<SAMPLER>(sc, P, cams, lb, oc, lane, n_sel, (more && !endgame) ? OMERF_TRAV_KEEP : OMERF_DRAIN_TRAV_KEEP, out_rgb, out_n);
         } else if (phase == ST_READY) {
             // ---- samples: gather, activations, compositing (S5, S6, S7) for the rays listed in P.list[0 .. n_sel);
             // lanes whose ray left the READY state take the next listed rays, OMERF_SAMPLE_SWAP lanes at a time
@@ -732,7 +771,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             Ray r;
             auto load_ray = [&](int s_new) {
                 sslot = s_new;
-                const int s_ = s_new < 0 ? 0 : s_new;
+                const int s_ = s_new < 0 ? 0 : chk(s_new, OMERF_POOL, CHK_SLOT);
                 view = P.meta[s_] >> 8;
                 status = s_new < 0 ? ST_IDLE : ST_READY;
                 k = P.k[s_];
@@ -742,7 +781,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                 r.dx = P.d[0][s_];
                 r.dy = P.d[1][s_];
                 r.dz = P.d[2][s_];
-                ray_origin(oc, cams, view, r);
+                ray_origin(oc, cams, lb, view, r);
 #pragma unroll
                 for (int c = 0; c < 7; c++) acc[c] = P.acc[c][s_];
             };
@@ -773,7 +812,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                         lattice_point(r, sc.step, k + 1, qx, qy, qz);
                         if (k < k1) { // k + 1 is inside the box then (setup_ray): no clamp, no box test
                             const int ix = cell_index_in_box(qx, sc.sx), iy = cell_index_in_box(qy, sc.sy);
-                            const float2 h = __ldg(sc.pyr + (uint32_t)(ix * sc.My + iy));
+                            const float2 h = __ldg(sc.pyr + chk((uint32_t)(ix * sc.My + iy), sc.n_pyr, CHK_PYR));
                             next_ready = h.x <= qz && qz <= h.y;
                         }
                     }
@@ -782,7 +821,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                         // Eq. 6 (q = 2) at the nearest grid point of P_o (Eq. 7): the sample is inside [z_min, z_max],
                         // so M = min(1, ((z - z_min)/eps)^2, ((z_max - z)/eps)^2); it weights the colours only (Eq. 8)
                         const int ix = cell_index_in_box(px, sc.sx), iy = cell_index_in_box(py, sc.sy);
-                        const float2 h = __ldg(sc.pyr + (uint32_t)(ix * sc.My + iy));
+                        const float2 h = __ldg(sc.pyr + chk((uint32_t)(ix * sc.My + iy), sc.n_pyr, CHK_PYR));
                         const float m = __saturatef(fminf(pz - h.x, h.y - pz) * sc.inv_soft_eps);
                         soft_m = m * m;
                     }
@@ -836,7 +875,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 #pragma unroll
                 for (int rr = 0; rr < 2; rr++) {
                     const int ray = half * 16 + (lane >> 2) + 8 * rr, tq = lane & 3;
-                    const int sl = ray < n_act ? (int)P.list[ray] : slot; // unused rows: any finite values
+                    const int sl = ray < n_act ? chk((int)P.list[ray], OMERF_POOL, CHK_SLOT) : slot; // unused rows: their outputs are not read
                     mlp_encode_component<true>(P.d[min(tq, 2)][sl], v[rr]);
                     v[rr][9] = P.acc[tq][sl];
                     if (tq == 3) {
@@ -854,8 +893,8 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                     for (int rr = 0; rr < 2; rr++) {
                         const int ray = half * 16 + g + 8 * rr;
                         if (ray < n_act) {
-                            const int sl = (int)P.list[ray];
-                            const size_t pix = P.pix[sl];
+                            const int sl = chk((int)P.list[ray], OMERF_POOL, CHK_SLOT);
+                            const size_t pix = chk((size_t)P.pix[sl], lb.n_pix, CHK_PIXEL);
                             const float T_end = __expf(-(float)P.Q[sl] * (1.0f / 1048576.0f));
                             if (t == 0) {
                                 out_rgb[pix * 3 + 0] = __saturatef(P.acc[0][sl] + sigmoid_fast(o[2 * rr]) + T_end * sc.bg[0]);
@@ -906,7 +945,7 @@ omerf_gather_probe_kernel(const __grid_constant__ DevScene sc, const omerf_camer
     grid_corner_offsets<true>(sc, x0, min(x0 + 1, sc.G[0] - 1), y0, z0, min(z0 + 1, sc.G[2] - 1), off);
     uint4 t[10];
 #pragma unroll
-    for (int q = 0; q < 4; q++) t[q] = __ldg(sc.grid + off[q]);
+    for (int q = 0; q < 4; q++) t[q] = __ldg(sc.grid + chk(off[q], sc.n_grid, CHK_GRID));
     axis_tap(px, sc.xy_s[0], xa, w);
     axis_tap(py, sc.xy_s[1], ya, w);
     axis_tap(px, sc.xz_s[0], xb, w);
@@ -915,12 +954,12 @@ omerf_gather_probe_kernel(const __grid_constant__ DevScene sc, const omerf_camer
     axis_tap(pz, sc.yz_s[1], zb, w);
     const uint32_t Nxy = (uint32_t)sc.xy_n[1], Nxz = (uint32_t)sc.xz_rows, Nyz = (uint32_t)sc.yz_rows;
     const uint32_t zr = (uint32_t)(za - sc.xz_zoff), zs = (uint32_t)(zb - sc.yz_zoff);
-    t[4] = __ldg(sc.pxy + ((uint32_t)xa * Nxy + (uint32_t)ya));
-    t[5] = __ldg(sc.pxy + ((uint32_t)min(xa + 1, sc.xy_n[0] - 1) * Nxy + (uint32_t)ya));
-    t[6] = __ldg(sc.pxz + ((uint32_t)xb * Nxz + zr));
-    t[7] = __ldg(sc.pxz + ((uint32_t)min(xb + 1, sc.xz_n[0] - 1) * Nxz + zr));
-    t[8] = __ldg(sc.pyz + ((uint32_t)yb * Nyz + zs));
-    t[9] = __ldg(sc.pyz + ((uint32_t)min(yb + 1, sc.yz_n[0] - 1) * Nyz + zs));
+    t[4] = __ldg(sc.pxy + chk((uint32_t)xa * Nxy + (uint32_t)ya, sc.n_pxy, CHK_PXY));
+    t[5] = __ldg(sc.pxy + chk((uint32_t)min(xa + 1, sc.xy_n[0] - 1) * Nxy + (uint32_t)ya, sc.n_pxy, CHK_PXY));
+    t[6] = __ldg(sc.pxz + chk((uint32_t)xb * Nxz + zr, sc.n_pxz, CHK_PXZ));
+    t[7] = __ldg(sc.pxz + chk((uint32_t)min(xb + 1, sc.xz_n[0] - 1) * Nxz + zr, sc.n_pxz, CHK_PXZ));
+    t[8] = __ldg(sc.pyz + chk((uint32_t)yb * Nyz + zs, sc.n_pyz, CHK_PYZ));
+    t[9] = __ldg(sc.pyz + chk((uint32_t)min(yb + 1, sc.yz_n[0] - 1) * Nyz + zs, sc.n_pyz, CHK_PYZ));
     uint32_t x = 0;
 #pragma unroll
     for (int q = 0; q < 10; q++) x ^= (t[q].x + t[q].y) ^ (t[q].z + t[q].w);

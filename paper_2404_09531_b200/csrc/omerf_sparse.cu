@@ -156,6 +156,8 @@ int omerf_bake_sparse_grid(omerf_scene *s, void **d_dense, int block, cudaStream
         v.nby = nby;
         v.nbz = nbz;
         v.blk_table = (const int32_t *)s->d_blk_table;
+        v.n_blk = (uint32_t)nb;
+        v.n_grid = (uint32_t)texels;
         s->blocks_total = nb;
         s->blocks_allocated = n_alloc;
         s->grid_bytes = texels * sizeof(uint4) + nb * sizeof(int32_t);

@@ -31,6 +31,16 @@ def test_every_declared_symbol_is_exported(omerf):
     assert b"sm_100a" in L.omerf_version()
 
 
+def test_range_checked_flavour_builds_and_exports_the_same_symbols(omerf):
+    """libomerf_checked.so (-DOMERF_CHECKED, tests/test_gpu_checked.py): same C-ABI as the shipped library"""
+    from paper_2404_09531_b200 import build as b
+    L = C.CDLL(b.build(checked=True))
+    for name in omerf.EXPORTS:
+        assert getattr(L, name) is not None
+    L.omerf_check_errors.restype = C.c_uint32
+    assert omerf.load_library().omerf_check_errors() == 0          # the shipped library has no checks: always 0
+
+
 def test_struct_layout_matches_header(omerf, tmp_path):
     """ctypes mirrors vs the real header, through gcc's offsetof/sizeof."""
     import subprocess
