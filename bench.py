@@ -39,9 +39,9 @@ if ROOT not in sys.path:
 
 import synth  # noqa: E402
 
-BYTES_PER_SAMPLE = 168   # 20 texels x 8 B (64 B grid + 96 B planes) + one (z_min, z_max) pair of 8 B
+BYTES_PER_SAMPLE = 168   # 20 distinct texels x 8 B (64 B grid + 96 B planes) + one (z_min, z_max) pair of 8 B
 BYTES_PER_PIXEL = 16     # 12 B rgb + 4 B sample count written
-TEXEL_BYTES_PER_SAMPLE = 160   # what the gather requests: 20 texels x 8 B
+TEXEL_BYTES_PER_SAMPLE = 160   # the distinct texels a sample needs: 20 x 8 B (fetched as 10 entries of 16 B)
 # Figures of ONE march-kernel launch on configs[1] from the committed `ncu --set full` capture (profiles/r02_march_kernel.md,
 # which names the command and the commit it was taken at); cited constants, not measured by this run:
 NCU_CAPTURE = {"profile": "profiles/r02_march_kernel.md", "commit": "8a6b660",
@@ -391,7 +391,7 @@ def run_ours(args):
                     "pixels_where_counts_differ": int((n2 != out_n).sum().item())}
         omerf.scene_destroy(h2)
 
-    # gather calibration: the same frame's 20 texel loads per sample replayed with no arithmetic
+    # gather calibration: the same frame's 10 entry loads per sample replayed with no arithmetic
     probe = omerf.gather_probe(h, cams[0], W, H, repeats=10, flush_l2=True) if rank == 0 else None
 
     # e2e through the C-ABI with HOST buffers (pinned), copies inside the timed region
