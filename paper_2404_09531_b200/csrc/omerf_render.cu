@@ -28,6 +28,8 @@
 // in k in every component (rounding is monotone), so cell indices and z are monotone in k.  If samples k
 // and kk both lie in one pyramid node and both are on the same side outside its [min,max] z-range, so
 // does every sample between them: all of them fail the predicate and may be skipped.
+#include <type_traits>
+
 #include "omerf_device.cuh"
 #include "omerf_mlp.cuh"
 
@@ -113,21 +115,10 @@ __device__ __forceinline__ void lattice_point(const Ray &r, float step, int k, f
     pz = __fmaf_rn(t, r.dz, r.oz);
 }
 
-__device__ __forceinline__ bool in_box(const DevScene &sc, float px, float py, float pz)
-{
-    return px >= 0.0f && px < sc.box[0] && py >= 0.0f && py < sc.box[1] && pz >= 0.0f && pz < sc.box[2];
-}
-
 // Nearest grid point of P_o (Eq. 7) for a point INSIDE the box (0 <= p < X): p s < M - 1 exactly (s = fl((M-1)/X),
 // p <= X (1 - 2^-24)), so the rounded fma lies in [1/2, M - 1/2] and the clamp of R1 to [0, M-1] is the identity.  Every
 // lattice index a ray keeps lies inside the box (setup_ray), which is what lets the march drop the clamps and box tests.
 __device__ __forceinline__ int cell_index_in_box(float p, float s) { return floor_int(__fmaf_rn(p, s, 0.5f)); }
-
-__device__ __forceinline__ int voxel_index(float p, float s, int N)
-{
-    const int j = floor_int(__fmul_rn(p, s));
-    return min(max(j, 0), N - 1);
-}
 
 // last lattice index whose parameter is below t_end (proposal only; verified by the caller)
 __device__ __forceinline__ int index_before(float t_end, float inv_step, int k1)
@@ -208,32 +199,56 @@ __device__ __forceinline__ bool occ_test(const DevScene &sc, int lvl, int jx, in
 }
 
 // sampler GRID (config-4 comparator): multi-resolution binary occupancy grid, DDA-style skipping.
-__device__ __forceinline__ int trav_step_grid(const DevScene &sc, const Ray &r, int &k, int k1, int &lvl, int status)
+// Voxel index of R18 for a point inside the box: floor(p N/X) >= 0; the product can round up to N just below the far
+// face, so the upper clamp stays.
+__device__ __forceinline__ int voxel_index_in_box(float p, float s, int N) { return min(floor_int(__fmul_rn(p, s)), N - 1); }
+
+// Per-ray constants (proposals only): exit parameter of the voxel boundary at level-0 index b along an axis,
+// t = (b vox - o) / d = fma((float)b, vox / d, -o / d)   (d = 0: a = 0, c = +inf).
+struct GridTrav {
+    float a[3], c[3];
+    int s[3];
+};
+
+__device__ __forceinline__ void grid_trav_setup(const DevScene &sc, const Ray &r, GridTrav &q)
 {
-    // same shape as trav_step_plane: branch-free, status other than ST_TRAV passes through
+    const float d[3] = {r.dx, r.dy, r.dz}, o[3] = {r.ox, r.oy, r.oz}, id[3] = {r.ix, r.iy, r.iz};
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        q.a[i] = d[i] != 0.0f ? sc.vox[i] * id[i] : 0.0f;
+        q.c[i] = d[i] != 0.0f ? -o[i] * id[i] : INFINITY;
+        q.s[i] = d[i] > 0.0f ? 1 : 0;
+    }
+}
+
+// Same shape as trav_step_plane: branch-free, a status other than ST_TRAV passes through, every index in [k, k1] is
+// inside the box.  An empty node is left through its nearest face (verified: index kk still lies in the node); the level
+// then rises as far as the face crossed is aligned.
+__device__ __forceinline__ int trav_step_grid(const DevScene &sc, const Ray &r, const GridTrav &q, int &k, int k1, int &lvl, int status)
+{
     const bool run = status == ST_TRAV && k <= k1;
     float px, py, pz;
     lattice_point(r, sc.step, k, px, py, pz);
-    const bool inb = in_box(sc, px, py, pz); // the 2-index padding outside the box is walked one index at a time
     const int top = sc.occ_levels - 1;
-    const int nx = voxel_index(px, sc.ns[0], sc.N[0]) >> lvl, ny = voxel_index(py, sc.ns[1], sc.N[1]) >> lvl,
-              nz = voxel_index(pz, sc.ns[2], sc.N[2]) >> lvl;
-    const bool occ = occ_test(sc, lvl, nx, ny, nz);
-    const int bxi = nx + (r.dx > 0.0f ? 1 : 0), byi = ny + (r.dy > 0.0f ? 1 : 0), bzi = nz + (r.dz > 0.0f ? 1 : 0);
-    const float tx = r.dx != 0.0f ? ((float)(bxi << lvl) * sc.vox[0] - r.ox) * r.ix : INFINITY;
-    const float ty = r.dy != 0.0f ? ((float)(byi << lvl) * sc.vox[1] - r.oy) * r.iy : INFINITY;
-    const float tz = r.dz != 0.0f ? ((float)(bzi << lvl) * sc.vox[2] - r.oz) * r.iz : INFINITY;
+    const int nx = voxel_index_in_box(px, sc.ns[0], sc.N[0]) >> lvl, ny = voxel_index_in_box(py, sc.ns[1], sc.N[1]) >> lvl,
+              nz = voxel_index_in_box(pz, sc.ns[2], sc.N[2]) >> lvl;
+    bool occ = false;
+    if (run) occ = occ_test(sc, lvl, nx, ny, nz); // lanes without a ray load nothing
+    const int bxi = nx + q.s[0], byi = ny + q.s[1], bzi = nz + q.s[2];
+    const float tx = fmaf((float)(bxi << lvl), q.a[0], q.c[0]);
+    const float ty = fmaf((float)(byi << lvl), q.a[1], q.c[1]);
+    const float tz = fmaf((float)(bzi << lvl), q.a[2], q.c[2]);
     const int kk = index_before(fminf(fminf(tx, ty), tz), sc.inv_step, k1);
     float qx, qy, qz;
     lattice_point(r, sc.step, kk, qx, qy, qz);
-    const bool same = (voxel_index(qx, sc.ns[0], sc.N[0]) >> lvl) == nx && (voxel_index(qy, sc.ns[1], sc.N[1]) >> lvl) == ny &&
-                      (voxel_index(qz, sc.ns[2], sc.N[2]) >> lvl) == nz;
-    const bool jump = inb && !occ && kk > k && same;
-    const bool ready = run && inb && occ && lvl == 0;
+    const bool same = (voxel_index_in_box(qx, sc.ns[0], sc.N[0]) >> lvl) == nx && (voxel_index_in_box(qy, sc.ns[1], sc.N[1]) >> lvl) == ny &&
+                      (voxel_index_in_box(qz, sc.ns[2], sc.N[2]) >> lvl) == nz;
+    const bool jump = !occ && kk > k && same;
+    const bool ready = run && occ && lvl == 0;
     const int crossed = (tx <= ty && tx <= tz) ? bxi : (ty <= tz ? byi : bzi);
     const int up = crossed == 0 ? 2 : min(__ffs(crossed) - 1, 2); // leaving 2^up-aligned parents: ascend that far
-    const int lvl_next = !inb ? lvl : (occ ? max(lvl - OMERF_GRID_LVL_INSIDE, 0) : (jump ? min(lvl + up, top) : max(lvl - OMERF_GRID_LVL_FAIL, 0)));
-    const int k_next = !inb ? k + 1 : (jump ? kk + 1 : ((lvl == 0 && !ready) ? k + 1 : k));
+    const int lvl_next = occ ? max(lvl - OMERF_GRID_LVL_INSIDE, 0) : (jump ? min(lvl + up, top) : max(lvl - OMERF_GRID_LVL_FAIL, 0));
+    const int k_next = jump ? kk + 1 : ((lvl == 0 && !ready) ? k + 1 : k);
     if (run) {
         k = k_next;
         lvl = lvl_next;
@@ -465,39 +480,26 @@ __device__ __forceinline__ bool setup_ray(const DevScene &sc, const omerf_camera
         return (r.dx >= 0.0f ? px < sc.box[0] : px >= 0.0f) && (r.dy >= 0.0f ? py < sc.box[1] : py >= 0.0f) &&
                (r.dz >= 0.0f ? pz < sc.box[2] : pz >= 0.0f);
     };
-    if (!entered(k1) || !not_left(k)) return false;
-    {
-        int lo = k; // first entered index is in [lo, hi]
-        int hi = k1;
+    // smallest index in [lo, hi] for which a monotone (false..false true..true) predicate holds, hi + 1 if none: probes
+    // next to the estimate first (it is usually right or off by one), then bisection (rays that graze a face)
+    auto first_true = [&](auto pred, int lo, int hi, int guess) {
+        int L = lo, H = hi + 1, p = min(max(guess, lo), hi);
 #pragma unroll 1
-        for (int it = 0; it < 4 && lo < hi; it++) {
-            if (entered(lo)) hi = lo;
-            else lo++;
+        for (int it = 0; L < H; it++) {
+            const bool t = pred(p);
+            if (t) H = p;
+            else L = p + 1;
+            p = it < 3 ? (t ? p - 1 : p + 1) : L + ((H - 1 - L) >> 1);
+            p = min(max(p, L), max(H - 1, L));
         }
-#pragma unroll 1
-        while (lo < hi) {
-            const int mid = lo + ((hi - lo) >> 1);
-            if (entered(mid)) hi = mid;
-            else lo = mid + 1;
-        }
-        k = lo;
-    }
-    {
-        int lo = k - 1; // last index not yet left is in [lo, hi]; lo = k - 1 stands for "none at or after k"
-        int hi = k1;
-#pragma unroll 1
-        for (int it = 0; it < 4 && lo < hi; it++) {
-            if (not_left(hi)) lo = hi;
-            else hi--;
-        }
-#pragma unroll 1
-        while (lo < hi) {
-            const int mid = hi - ((hi - lo) >> 1);
-            if (not_left(mid)) lo = mid;
-            else hi = mid - 1;
-        }
-        k1 = hi;
-    }
+        return L;
+    };
+    const int ge = (int)fminf(ceilf(t0 * sc.inv_step - 0.5f), 1.0e9f), gl = (int)fminf(floorf(t1 * sc.inv_step - 0.5f), 1.0e9f) + 1;
+    const int ka = first_true(entered, k, k1, ge);                                     // first index past the entry faces
+    if (ka > k1) return false;
+    const int kb = first_true([&](int i) { return !not_left(i); }, ka, k1, gl) - 1;     // last index before the exit faces
+    k = ka;
+    k1 = kb;
     return k <= k1;
 }
 
@@ -561,15 +563,22 @@ __device__ __forceinline__ void ray_origin(OriginCache &oc, const omerf_camera *
     r.oz = oc.oz;
 }
 
+struct NoTrav {};
+template <int SAMPLER>
 struct TravLane {
     Ray r;
-    PlaneTrav q;
+    typename std::conditional<SAMPLER == OMERF_SAMPLER_PLANE, PlaneTrav, NoTrav>::type q;
+    typename std::conditional<SAMPLER == OMERF_SAMPLER_PLANE, NoTrav, GridTrav>::type g;
     int k, k1, lvl, status, slot; // slot < 0: the lane holds no ray
     uint32_t view;
 };
 
+__device__ __forceinline__ void plane_trav_setup(const DevScene &, const Ray &, NoTrav &) {}
+__device__ __forceinline__ void grid_trav_setup(const DevScene &, const Ray &, NoTrav &) {}
+
+template <int SAMPLER>
 __device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P, const omerf_camera *__restrict__ cams,
-                                          const LaunchBounds &lb, OriginCache &oc, int slot, TravLane &L)
+                                          const LaunchBounds &lb, OriginCache &oc, int slot, TravLane<SAMPLER> &L)
 {
     L.slot = slot;
     const int s_ = slot < 0 ? 0 : chk(slot, OMERF_POOL, CHK_SLOT); // idle lanes read slot 0 and step nothing
@@ -587,9 +596,11 @@ __device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P,
     L.r.iy = L.r.dy != 0.0f ? __fdividef(1.0f, L.r.dy) : INFINITY;
     L.r.iz = L.r.dz != 0.0f ? __fdividef(1.0f, L.r.dz) : INFINITY;
     plane_trav_setup(sc, L.r, L.q);
+    grid_trav_setup(sc, L.r, L.g);
 }
 
-__device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, const LaunchBounds &lb, const TravLane &L,
+template <int SAMPLER>
+__device__ __forceinline__ void trav_store(const DevScene &sc, WarpPool &P, const LaunchBounds &lb, const TravLane<SAMPLER> &L,
                                            float *__restrict__ out_rgb, uint32_t *__restrict__ out_n)
 {
     const int s_ = chk(L.slot, OMERF_POOL, CHK_SLOT);
@@ -612,15 +623,15 @@ __device__ __forceinline__ void trav_visit(const DevScene &sc, WarpPool &P, cons
 {
     const unsigned FULL = 0xffffffffu;
     const unsigned lt_mask = (1u << lane) - 1u;
-    TravLane L;
+    TravLane<SAMPLER> L;
     trav_load(sc, P, cams, lb, oc, lane < n_sel ? (int)P.list[lane] : -1, L);
     int next = min(n_sel, 32); // first list entry not yet taken
 #pragma unroll 1
     for (int it = 0; it < OMERF_TRAV_STEPS; it++) {
-        if (SAMPLER == OMERF_SAMPLER_PLANE) {
+        if constexpr (SAMPLER == OMERF_SAMPLER_PLANE) {
             L.status = trav_step_plane(sc, L.r, L.q, L.k, L.k1, L.lvl, L.status);
         } else {
-            L.status = trav_step_grid(sc, L.r, L.k, L.k1, L.lvl, L.status);
+            L.status = trav_step_grid(sc, L.r, L.g, L.k, L.k1, L.lvl, L.status);
         }
         const unsigned going = __ballot_sync(FULL, L.status == ST_TRAV);
         if (next < n_sel) {
@@ -815,6 +826,13 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
                             const float2 h = __ldg(sc.pyr + chk((uint32_t)(ix * sc.My + iy), sc.n_pyr, CHK_PYR));
                             next_ready = h.x <= qz && qz <= h.y;
                         }
+                    } else {
+                        // the comparator's predicate at the next lattice point: its level-0 voxel bit (R18)
+                        float qx, qy, qz;
+                        lattice_point(r, sc.step, k + 1, qx, qy, qz);
+                        if (k < k1)
+                            next_ready = occ_test(sc, 0, voxel_index_in_box(qx, sc.ns[0], sc.N[0]), voxel_index_in_box(qy, sc.ns[1], sc.N[1]),
+                                                  voxel_index_in_box(qz, sc.ns[2], sc.N[2]));
                     }
                     float soft_m = 1.0f;
                     if (GENERAL && SAMPLER == OMERF_SAMPLER_PLANE && sc.soft_eps > 0.0f) {
