@@ -494,3 +494,42 @@ def test_lowz_bake_degenerate_scenes_and_rejections(omerf, oracle):
     sc = synth.custom_scene(occ_n=(8, 8, 8))
     with pytest.raises(omerf.OmerfError):
         omerf.scene_create(sc, sampler=1, lowz_bake=True)     # the grid sampler's voxels are a superset of the slab
+
+
+# ----------------------------------------------------------------------------- the exact in-box index range (setup_ray)
+def _axis_camera(origin, fwd, up, W, H, f=20.0):
+    """camera row with an exactly axis-aligned frame (so rays through the principal point have zero components)"""
+    fwd = np.asarray(fwd, dtype=np.float64)
+    up = np.asarray(up, dtype=np.float64)
+    right = np.cross(fwd, up)
+    return np.concatenate([origin, right, up, fwd, [f, f, W / 2.0, H / 2.0]]).astype(np.float32)
+
+
+FACE_CAMS = [
+    ((0.0, 4.0, 2.0), (1, 0, 0), (0, 0, 1)),     # origin ON the face x = 0, looking in: first lattice points just inside
+    ((8.0, 4.0, 2.0), (-1, 0, 0), (0, 0, 1)),    # origin ON the far face x = X (p < X fails at t = 0), looking in
+    ((4.0, 4.0, 4.0), (0, 0, -1), (0, 1, 0)),    # origin ON the top face z = Z, straight down
+    ((4.0, 0.0, 0.0), (0, 1, 0), (0, 0, 1)),     # origin ON the edge y = 0, z = 0: rays along the bottom face
+    ((0.0, 0.0, 0.0), (1, 0, 0), (0, 0, 1)),     # origin ON a corner, along an edge of the box
+    ((-3.0, 8.0, 2.0), (1, 0, 0), (0, 0, 1)),    # in the plane y = Y (never inside: p.y < Y fails), grazing
+    ((-3.0, 7.999999, 3.9999998), (1, 0, 0), (0, 0, 1)),   # one ulp inside two faces, parallel to both
+    ((4.0, 4.0, 2.0), (1, 0, 0), (0, 0, 1)),     # inside, axis-parallel
+]
+
+
+@pytest.mark.parametrize("sampler", [0, 1])
+@pytest.mark.parametrize("origin,fwd,up", FACE_CAMS)
+def test_cameras_on_faces_edges_and_grazing_rays(omerf, oracle, origin, fwd, up, sampler):
+    """setup_ray searches the exact range of lattice indices inside the box and the march then drops every box test and
+    clamp: rays that start on a face, run inside a face plane, or are parallel to an axis (zero direction components,
+    odd image sizes put a pixel centre on the principal point) must still give the brute-force oracle's counts."""
+    rng = np.random.default_rng(3)
+    lo = rng.uniform(0.0, 1.5, (9, 9)).astype(np.float32)
+    hi = (lo + rng.uniform(-0.2, 2.6, (9, 9))).astype(np.float32)      # some empty columns, some reaching the top face
+    hi[2:4, 2:4] = 4.0
+    lo[5:7, 5:7] = 0.0
+    sc = synth.custom_scene(h_lo=lo, h_up=hi, seed=8, bias_amp=0.1, occ_n=(16, 16, 8) if sampler else (0, 0, 0))
+    W, H = 33, 21
+    cam = _axis_camera(origin, fwd, up, W, H)
+    rgb, ns, _ = _gpu_render(omerf, sc, cam, W, H, sampler=sampler)
+    _assert_parity(rgb, ns, oracle.OracleScene(sc, sampler=sampler).render(cam, W, H, mode="brute"), f"face camera {origin}")
