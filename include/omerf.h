@@ -36,7 +36,8 @@ extern "C" {
 
 typedef struct omerf_scene omerf_scene; /* opaque; owns all device memory of one baked scene */
 
-/* Baked scene on the HOST.  omerf_scene_create deep-copies everything. */
+/* Baked scene on the HOST.  omerf_scene_create deep-copies everything; on the device every feature array
+ * is re-laid out as 16-byte entries of two adjacent texels (twice the host bytes; omerf_scene_info.device_bytes). */
 typedef struct {
     float box[3];      /* X, Y, Z */
     int32_t hf_n[2];   /* Mx, My: grid points of the occupancy plane P_o; vertex-centred, spacing X/(Mx-1) */
@@ -133,9 +134,10 @@ int omerf_render_host(const omerf_scene *scene, const omerf_camera *cameras /*HO
 
 /* Gather calibration (SURVEY.md 8(d) "L2/L1 gather rate": the builder must calibrate the achievable rate of the
  * same load width over the same footprint).  Renders one frame of `camera` while logging every sample taken, then
- * times a kernel that only replays the 20 eight-byte texel loads of Eq. 2 for those samples - no
- * filtering, activations or compositing - once in frame order (pixel-coherent addresses) and once in a scattered
- * order.  160 B are requested per sample.  flush_l2 != 0 overwrites a 256 MiB buffer before every timed launch.
+ * times a kernel that only replays the feature loads of Eq. 2 for those samples - the 10 sixteen-byte
+ * entries (pairs of adjacent texels) that hold a sample's 20 texels in the scene's device layout - with no filtering,
+ * activations or compositing, once in frame order (pixel-coherent addresses) and once in a scattered order.  A sample
+ * needs 160 B of distinct texels.  flush_l2 != 0 overwrites a 256 MiB buffer before every timed launch.
  * Synchronous (device-wide); owns and frees its scratch.  HOST pointers. */
 typedef struct {
     uint64_t samples;       /* samples of the frame (= sum of out_nsamples) */

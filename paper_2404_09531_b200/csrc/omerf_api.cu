@@ -437,7 +437,7 @@ extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *camer
 
 
 // Gather calibration: logs the samples of one frame, then times kernels that only replay their
-// 20 texel loads, in frame order and in a scattered order.  Synchronous; allocates and frees its own buffers.
+// 10 entry loads (20 texels), in frame order and in a scattered order.  Synchronous; allocates and frees its own buffers.
 extern "C" int omerf_gather_probe(const omerf_scene *s, const omerf_camera *camera, int W, int H, int repeats,
                                   int flush_l2, omerf_gather_probe_result *out)
 {
