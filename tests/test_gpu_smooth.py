@@ -33,7 +33,11 @@ def _run(omerf, sc, F, d, delta, want_G=True):
     return out.cpu().numpy().astype(np.float64)
 
 
-@pytest.mark.parametrize("n,S,sigma", [(1000, 15, 0.05), (257, 31, 0.2), (33, 40, 0.1), (5, 1, 0.3), (64, 0, 0.1)])
+# sigma 3.0: perturbed directions up to |s| ~ 10, arguments of the encoding far outside [-pi, pi], negative cosines.
+# The 4e-6 bar is a statement about |s| = O(1) (unit directions plus perturbations): the 3xTF32 products keep 2^-21 of
+# the magnitude of every product, and s itself is a network input, so the error grows in proportion to max |s|.
+@pytest.mark.parametrize("n,S,sigma", [(1000, 15, 0.05), (257, 31, 0.2), (33, 40, 0.1), (5, 1, 0.3), (64, 0, 0.1),
+                                       (500, 15, 3.0)])
 def test_smoothness_parity(omerf, n, S, sigma):
     import oracle
     sc = synth.custom_scene(seed=3, bias_amp=0.4)
@@ -41,7 +45,10 @@ def test_smoothness_parity(omerf, n, S, sigma):
     loss, G = _run(omerf, sc, F, d, delta)
     ref_loss, ref_G = oracle.mlp_smoothness(oracle.OracleScene(sc), F, d, delta, want_G=True)
     assert np.abs(G - ref_G).max() <= 4e-6
-    tol = 2 * np.sqrt(3 * max(S, 1) * ref_loss) * 4e-6 + 3 * max(S, 1) * (4e-6) ** 2 + 1e-6 * ref_loss
+    # |w| <= 1, so sum_s |G_s - G_0|^2 bounds sum_s |w_s| |G_s - G_0|^2 (the two agree for small perturbations, where
+    # w ~ 1); with large perturbations the cosine can be negative and the loss itself is no bound
+    L = ((ref_G[:, 1:] - ref_G[:, :1]) ** 2).sum(axis=(1, 2)) if S else np.zeros(n)
+    tol = 2 * np.sqrt(3 * max(S, 1) * L) * 4e-6 + 3 * max(S, 1) * (4e-6) ** 2 + 1e-6 * L
     assert np.all(np.abs(loss - ref_loss) <= tol), float(np.abs(loss - ref_loss).max())
     if S == 0:
         assert np.array_equal(loss, np.zeros(n))
