@@ -44,10 +44,10 @@ BYTES_PER_PIXEL = 16     # 12 B rgb + 4 B sample count written
 TEXEL_BYTES_PER_SAMPLE = 160   # the distinct texels a sample needs: 20 x 8 B (fetched as 10 entries of 16 B)
 # Figures of ONE march-kernel launch on configs[1] from the committed `ncu --set full` capture (profiles/r02_march_kernel.md,
 # which names the command and the commit it was taken at); cited constants, not measured by this run:
-NCU_CAPTURE = {"profile": "profiles/r02_march_kernel.md", "commit": "8a6b660",
-               "dram_bytes": 177553664 + 18950400,          # dram__bytes_read.sum + dram__bytes_write.sum
-               "warp_instructions": 356805584,              # smsp__inst_executed.sum
-               "lanes_per_instruction": 28.37}              # smsp__thread_inst_executed_per_inst_executed.ratio
+NCU_CAPTURE = {"profile": "profiles/r02_march_kernel.md", "commit": "d5ceb67",
+               "dram_bytes": 177507072 + 18304512,          # dram__bytes_read.sum + dram__bytes_write.sum
+               "warp_instructions": 344547795,              # smsp__inst_executed.sum
+               "lanes_per_instruction": 28.23}              # smsp__thread_inst_executed_per_inst_executed.ratio
 
 
 def workload_name(cfg: int) -> str:
