@@ -11,7 +11,7 @@
 namespace {
 
 constexpr int SMOOTH_WARPS = 4;
-constexpr int SMOOTH_MIN_BLOCKS = 6; // 80 registers, 24 warps per SM: measured 0.97 ms against 1.13 ms at 4 blocks (121 registers)
+constexpr int SMOOTH_MIN_BLOCKS = 7; // 72 registers, 28 warps per SM: 0.924 ms; 6 blocks 0.970, 8 blocks (64 registers) 0.952, 4 blocks (121 registers) 1.13
 
 struct SmoothDir {          // what a lane keeps of one direction
     float d[3];             // the direction
