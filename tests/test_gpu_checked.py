@@ -92,3 +92,30 @@ def test_checked_build_edge_cameras_ragged_sizes_and_probe(libs):
         assert L.omerf_check_errors() == 0
     ref_rgb, ref_n = _render(scene, cams, 37, 23)
     assert np.array_equal(ns.cpu().numpy(), ref_n) and np.array_equal(rgb.cpu().numpy(), ref_rgb)
+
+
+def test_checked_build_at_the_timed_size(libs):
+    """configs[1] (1920x1080, 8.3 M samples) and configs[5]'s in-box cameras through the checked library: plain path,
+    sparse blocks + soft mask, low-z bake; no violation, counts equal to the shipped library's"""
+    import torch
+    import paper_2404_09531_b200 as omerf
+    scene = synth.make_scene(1)
+    runs = [(1, {}), (1, dict(grid_block=4, soft_eps=2.0)), (1, dict(lowz_bake=True)), (5, {})]
+    ref = []
+    for cfg, kw in runs:
+        cams = synth.make_cameras(cfg)
+        W, H = synth.config_resolution(cfg)
+        with omerf.scene_create(scene, **kw) as h:
+            _, ns = omerf.render(h, cams, W, H)
+            torch.cuda.synchronize()
+            ref.append(ns.cpu())
+    with libs() as L:
+        for (cfg, kw), want in zip(runs, ref):
+            cams = synth.make_cameras(cfg)
+            W, H = synth.config_resolution(cfg)
+            with omerf.scene_create(scene, **kw) as h:
+                _, ns = omerf.render(h, cams, W, H)
+                torch.cuda.synchronize()
+                omerf.gather_probe(h, cams[0], W, H, repeats=1, flush_l2=False)
+            assert L.omerf_check_errors() == 0, f"config {cfg} {kw}: a device index left its array"
+            assert torch.equal(ns.cpu(), want)
