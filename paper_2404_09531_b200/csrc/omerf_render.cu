@@ -10,16 +10,19 @@
 // kernel leaves two thirds of the lanes idle (measured: 10.5 of 32 lanes active; the pool runs at 27).
 //
 //   S2 ray generation          fp32, one correctly rounded operation per step (bit-exact with the CPU checker)
-//   S3 box clip                fp32 slab test, padded by 2 lattice indices (the exact per-sample predicate decides)
+//   S3 box clip                fp32 slab test padded by 2 lattice indices, then the EXACT range of indices inside the box
+//                              (the lattice is monotone: probes + bisection), so the march needs no box test or clamp
 //   S4 occupancy-plane march   hierarchical DDA over the min/max pyramid of (z_min, z_max): in empty space the
 //                              ray jumps to the exit of the coarsest empty node or to the start of the node's
 //                              z-interval; every jump is VERIFIED with the exact lattice
 //                              arithmetic, so skipping never changes which samples exist
-//   S5 gather                  trilinear grid + 3 bilinear planes, uint8 x 8 channels per 8-byte load,
-//                              8-bit fixed-point weights, exact integer sums as IDP.2A dot products (Eq. 2, R9)
+//   S5 gather                  trilinear grid + 3 bilinear planes as 10 sixteen-byte entries (two adjacent texels of
+//                              8 uint8 channels, bytes interleaved per channel), 8-bit fixed-point weights, exact integer
+//                              sums as IDP.2A dot products (Eq. 2, R9)
 //   S6 activations             exp (exp_q on the decision path), sigmoid through MUFU.TANH (Eq. 3)
 //   S7 compositing             front to back, integer optical depth decides termination (Eq. 1/8, R7/R8)
-//   S8 deferred MLP            34 -> 16 -> 16 -> 3 as 3xTF32 tensor-core tiles, 16 rays at a time (Eq. 4; omerf_mlp.cuh)
+//   S8 deferred MLP            34 -> 16 -> 16 -> 3 as 3xTF32 tensor-core tiles, 16 rays at a time, layer-1 fragments built
+//                              in registers from the pool (Eq. 4; omerf_mlp.cuh)
 //   S9 outputs                 rgb fp32 + per-pixel sample count (Fig. 1)
 // plus the gather calibration of SURVEY 8(d) (sample log + omerf_gather_probe_kernel) and, in the GENERAL
 // instantiation, the 8(f) variants (soft occupancy of Eq. 6-8, sparse-block grid).

@@ -5,7 +5,7 @@
 // (ix,iy) of P_o the corner ranges of the cell footprint (widened by 1/64 cell, exact integer arithmetic) and of
 // [z_min, z_max] (widened by 1/64 voxel, double with one rounding per operation) are marked.  A B^3 block is
 // allocated iff it holds a needed voxel; allocated blocks are numbered in C order of (bx,by,bz) by a scan and their
-// voxels copied into the atlas [id][B][B][B] (8-byte texels).  The render kernels then address V through the block
+// voxels copied into the atlas [id][B][B][B] (16-byte entries: the texel and its +y neighbour).  The render kernels then address V through the block
 // table (one indirection per corner) and fetch exactly the texels of the dense grid.
 #include "omerf_device.cuh"
 
