@@ -132,6 +132,32 @@ int omerf_render_tiles(const omerf_scene *scene, const omerf_camera *cameras /*H
 int omerf_render_host(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W,
                       int H, float *out_rgb /*HOST*/, uint32_t *out_nsamples /*HOST*/, void *stream);
 
+/* omerf_render for callers that must not allocate.  omerf_render keeps its per-call scratch - the device copy of the
+ * cameras and the head of the march kernel's work queue - in a ring it (re)allocates with cudaMalloc / cudaMallocHost
+ * behind a cudaDeviceSynchronize whenever a call brings more views than any call before it.  That is wrong for two kinds
+ * of caller: a render or serving loop with a frame deadline (an allocation synchronises the whole device and stalls every
+ * other stream of the process, at a moment the loop does not choose), and a plug-in inside a host program that has
+ * already claimed all device memory for its own pool or forbids driver allocations once start-up is over (cudaMalloc then
+ * fails, or breaks the host's memory accounting).  This entry point renders the same images with the same march kernel,
+ * but the kernel's scratch lives in ONE fixed array that is part of the library image: a file-scope __device__ array of
+ * 256 B (queue head) + OMERF_STATIC_MAX_VIEWS * 64 B (cameras) = 2304 B, which every GPU that loads the library holds
+ * until the process exits.  It calls no cudaMalloc, cudaMallocHost, cudaFree or any other allocating routine; the scene
+ * handle (an input, made earlier by whoever may allocate) and both outputs are still the caller's.
+ *   cameras       HOST [n_views], 0 <= n_views <= OMERF_STATIC_MAX_VIEWS (more: OMERF_ERR_INVALID with a message that
+ *                 names the limit; split the batch, or use omerf_render).  Passed to the GPU as launch arguments, so the
+ *                 array may be pageable and may be reused or freed as soon as the call returns.
+ *   out_rgb, out_nsamples, W, H, stream: as omerf_render.  There is no limit on W or H.
+ * Set-up: the first call on each device looks up the device address of the array (cudaGetSymbolAddress, with that device
+ * current) and keeps it; make that first call before any stream capture begins.  Later calls only launch.
+ * Sharing: there is one array per GPU, shared by every scene, stream and thread.  Calls are safe back to back on one
+ * stream (each call clears the queue head and rewrites the cameras in stream order; nothing is carried over from the
+ * previous call).  Two calls whose kernels can overlap on the GPU - different streams without an ordering between them -
+ * RACE on the array and give wrong images; order them with an event, or use omerf_render for one of them (its scratch
+ * is separate).  Same one-host-thread-per-scene rule as omerf_render; asynchronous on `stream`. */
+#define OMERF_STATIC_MAX_VIEWS 32
+int omerf_render_static(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W, int H,
+                        float *out_rgb /*DEVICE*/, uint32_t *out_nsamples /*DEVICE*/, void *stream);
+
 /* Gather calibration (SURVEY.md 8(d) "L2/L1 gather rate": the builder must calibrate the achievable rate of the
  * same load width over the same footprint).  Renders one frame of `camera` while logging every sample taken, then
  * times a kernel that only replays the feature loads of Eq. 2 for those samples - the 10 sixteen-byte

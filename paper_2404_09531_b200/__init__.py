@@ -10,6 +10,7 @@ All arithmetic runs in hand-written CUDA kernels (csrc/*.cu, sm_100a).  No CPU f
 from .binding import (  # noqa: F401
     SAMPLER_GRID,
     SAMPLER_PLANE,
+    STATIC_MAX_VIEWS,
     EXPORTS,
     LIB_PATH,
     OmerfError,
@@ -24,6 +25,7 @@ from .binding import (  # noqa: F401
     pyramid_level,
     render,
     render_host,
+    render_static,
     render_tiles,
     scene_create,
     scene_destroy,

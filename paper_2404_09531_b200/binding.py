@@ -20,9 +20,10 @@ _u32p = C.POINTER(C.c_uint32)
 
 SAMPLER_PLANE = 0
 SAMPLER_GRID = 1
+STATIC_MAX_VIEWS = 32           # OMERF_STATIC_MAX_VIEWS of include/omerf.h
 
 EXPORTS = (
-    "omerf_scene_create", "omerf_render", "omerf_render_tiles", "omerf_render_host", "omerf_gather_probe", "omerf_mlp_smoothness", "omerf_heatmap",
+    "omerf_scene_create", "omerf_render", "omerf_render_tiles", "omerf_render_host", "omerf_render_static", "omerf_gather_probe", "omerf_mlp_smoothness", "omerf_heatmap",
     "omerf_last_launch_count",
     "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield", "omerf_scene_get_block_table",
     "omerf_scene_destroy", "omerf_last_error", "omerf_version", "omerf_check_errors",
@@ -78,6 +79,7 @@ def load_library() -> C.CDLL:
     L.omerf_scene_create.argtypes = [C.POINTER(SceneDesc), C.POINTER(C.c_void_p)]
     L.omerf_render.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
     L.omerf_render_host.argtypes = L.omerf_render.argtypes
+    L.omerf_render_static.argtypes = L.omerf_render.argtypes
     L.omerf_render_tiles.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_uint32,
                                      C.c_uint32, C.c_void_p]
     L.omerf_gather_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
@@ -223,6 +225,26 @@ def render_tiles(h: SceneHandle, cameras, W: int, H: int, out_rgb, out_nsamples,
     st = torch.cuda.current_stream() if stream is None else stream
     _check(load_library().omerf_render_tiles(h.ptr, cams.ctypes.data, n, W, H, out_rgb.data_ptr(), out_nsamples.data_ptr(),
                                              int(tile_first), int(tile_end), st.cuda_stream), "omerf_render_tiles")
+    return out_rgb, out_nsamples
+
+
+def render_static(h: SceneHandle, cameras, W: int, H: int, out_rgb, out_nsamples, stream=None):
+    """omerf_render_static: omerf_render for callers that must not allocate device memory - a frame loop that cannot
+    afford the device-wide stall of a cudaMalloc, or a plug-in whose host program owns all GPU memory.  The march
+    kernel's scratch (device cameras, work-queue head) is a fixed 2304-byte array inside the library instead of a
+    ring the call may have to grow, so at most STATIC_MAX_VIEWS (32) views per call; more raises OmerfError.  Both
+    outputs are the caller's DEVICE tensors (this wrapper does not create them either).  Every call on a GPU shares
+    the one array: back-to-back calls on one stream are fine, calls on unordered streams race.  The first call on a
+    device looks up the array's address; make it before any stream capture.  Asynchronous on `stream`."""
+    import torch
+    cams = _cams(cameras)
+    n = cams.shape[0]
+    assert out_rgb.is_cuda and out_rgb.is_contiguous() and out_rgb.dtype == torch.float32 and out_rgb.numel() == n * H * W * 3
+    assert out_nsamples.is_cuda and out_nsamples.is_contiguous() and out_nsamples.element_size() == 4 \
+        and out_nsamples.numel() == n * H * W
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(load_library().omerf_render_static(h.ptr, cams.ctypes.data, n, W, H, out_rgb.data_ptr(), out_nsamples.data_ptr(),
+                                              st.cuda_stream), "omerf_render_static")
     return out_rgb, out_nsamples
 
 

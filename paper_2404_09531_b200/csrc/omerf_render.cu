@@ -31,6 +31,8 @@
 // in k in every component (rounding is monotone), so cell indices and z are monotone in k.  If samples k
 // and kk both lie in one pyramid node and both are on the same side outside its [min,max] z-range, so
 // does every sample between them: all of them fail the predicate and may be skipped.
+#include <string.h>
+
 #include <type_traits>
 
 #include "omerf_device.cuh"
@@ -1047,4 +1049,108 @@ int omerf_query_persistent_blocks(int sampler, int *blocks)
         OMERF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, omerf_march_kernel<OMERF_SAMPLER_GRID, false, true>, 32 * OMERF_WARPS, 0));
     *blocks = sms * (per_sm > 0 ? per_sm : 1);
     return OMERF_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// omerf_render_static (include/omerf.h): the render call for callers that must not allocate.
+//
+// Who needs it: a frame loop with a deadline (cudaMalloc synchronises the whole device and stalls the process's other
+// streams whenever omerf_render's camera ring has to grow), and a plug-in whose host program owns all device memory or
+// forbids driver allocations after start-up.  What it does differently: the march kernel's scratch - the device copy of
+// the cameras and the work-queue head - is not a cudaMalloc'd ring slot but the fixed array below, which is part of the
+// library image.  Nothing in this section calls cudaMalloc, cudaMallocHost, cudaFree or an allocating library routine.
+//
+// The array: one per GPU that loads the library, 2304 B, held until the process exits, shared by every scene, stream and
+// thread.  It keeps whatever the last call left in it, so every call rewrites all it reads: the cameras by the staging
+// kernel, the queue head by the cudaMemsetAsync in omerf_launch_render - both in stream order ahead of the march kernel.
+// Calls whose kernels can overlap on the GPU (unordered streams) race on it; the header says so.
+//
+// Host code must not hand `omerf_static_scratch` itself to a kernel: in host code that name is only the host-side
+// stand-in of the symbol.  The device address comes from cudaGetSymbolAddress, asked once per device with that device
+// current (the first call on a device does it - before any stream capture, see the header) and kept in a table.
+namespace {
+struct StaticScratch {
+    unsigned int head[OMERF_COUNTER_WORDS];    // word 0: work-queue head of the march kernel
+    omerf_camera cams[OMERF_STATIC_MAX_VIEWS]; // device copy of the call's cameras
+};
+struct StaticCameraArgs {                      // the cameras travel as launch arguments (2 KiB): no staging buffer,
+    omerf_camera cam[OMERF_STATIC_MAX_VIEWS];  // pageable host memory is fine, read before the call returns
+};
+} // namespace
+
+static __device__ __align__(256) unsigned char omerf_static_scratch[sizeof(StaticScratch)];
+
+namespace {
+__global__ void __launch_bounds__(128)
+omerf_static_stage_kernel(const __grid_constant__ StaticCameraArgs args, int n_views, StaticScratch *scratch)
+{
+    const float *src = reinterpret_cast<const float *>(args.cam);
+    float *dst = reinterpret_cast<float *>(scratch->cams);
+    for (int i = (int)threadIdx.x; i < n_views * (int)(sizeof(omerf_camera) / sizeof(float)); i += (int)blockDim.x) dst[i] = src[i];
+}
+
+#define OMERF_STATIC_MAX_DEVICES 64
+StaticScratch *g_static_ptr[OMERF_STATIC_MAX_DEVICES]; // device address of omerf_static_scratch, per device ordinal
+} // namespace
+
+// Device address of the array on the CURRENT device `dev`; the first call per device asks the runtime for it.
+// Not locked: a scene handle is used by one host thread at a time, and two threads that race here store the same value.
+static int static_scratch_address(int dev, StaticScratch **out)
+{
+    if (dev < 0 || dev >= OMERF_STATIC_MAX_DEVICES) {
+        omerf_set_error("invalid argument: omerf_render_static supports device ordinals below %d", OMERF_STATIC_MAX_DEVICES);
+        return OMERF_ERR_INVALID;
+    }
+    StaticScratch *p = g_static_ptr[dev];
+    if (!p) {
+        OMERF_CUDA(cudaGetSymbolAddress((void **)&p, omerf_static_scratch));
+        g_static_ptr[dev] = p;
+    }
+    *out = p;
+    return OMERF_OK;
+}
+
+extern "C" int omerf_render_static(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
+                                   float *out_rgb, uint32_t *out_nsamples, void *stream)
+{
+    if (!s || !cameras || !out_rgb || !out_nsamples) {
+        omerf_set_error("invalid argument: null scene/cameras/output");
+        return OMERF_ERR_INVALID;
+    }
+    if (n_views < 0 || W <= 0 || H <= 0) {
+        omerf_set_error("invalid argument: n_views >= 0, W > 0, H > 0 required");
+        return OMERF_ERR_INVALID;
+    }
+    if (n_views > OMERF_STATIC_MAX_VIEWS) {
+        omerf_set_error("invalid argument: omerf_render_static takes at most %d views per call (got %d): its scratch is a "
+                        "fixed array; split the batch or use omerf_render",
+                        OMERF_STATIC_MAX_VIEWS, n_views);
+        return OMERF_ERR_INVALID;
+    }
+    if (((uintptr_t)out_rgb & 3) || ((uintptr_t)out_nsamples & 3)) {
+        omerf_set_error("invalid argument: misaligned output");
+        return OMERF_ERR_INVALID;
+    }
+    s->last_launches = 0;
+    if (n_views == 0) return OMERF_OK;
+    int dev = -1;
+    OMERF_CUDA(cudaGetDevice(&dev));
+    if (dev != s->device) {
+        omerf_set_error("invalid argument: scene lives on device %d but device %d is current", s->device, dev);
+        return OMERF_ERR_INVALID;
+    }
+    StaticScratch *scratch = nullptr;
+    int rc = static_scratch_address(dev, &scratch);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    StaticCameraArgs args;
+    memcpy(args.cam, cameras, (size_t)n_views * sizeof(omerf_camera));
+    memset(args.cam + n_views, 0, (size_t)(OMERF_STATIC_MAX_VIEWS - n_views) * sizeof(omerf_camera));
+    omerf_static_stage_kernel<<<1, 128, 0, st>>>(args, n_views, scratch);
+    OMERF_CUDA(cudaGetLastError());
+    int launches = 0;
+    // the existing launcher, given the static array instead of a ring slot; it clears the queue head on `st` first
+    rc = omerf_launch_render(s, scratch->cams, n_views, W, H, out_rgb, out_nsamples, st, scratch->head, &launches);
+    s->last_launches = 1 + launches;
+    return rc;
 }
