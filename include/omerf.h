@@ -212,9 +212,10 @@ void omerf_scene_destroy(omerf_scene *scene); /* NULL is a no-op */
 const char *omerf_last_error(void); /* thread-local, static storage; "" if none */
 const char *omerf_version(void);
 /* Diagnostic of the range-checked build (libomerf_checked.so: every device index of the render kernels is checked, a
- * violation is redirected to element 0 and recorded).  Synchronises the device, returns the bit mask of violations seen
- * since the last call (bit: 0 pyramid, 1 V, 2 xy, 3 xz, 4 yz, 5 block table, 6 bitfield, 7 view, 8 pixel, 9 pool slot,
- * 10 pool list; 0xffffffff: CUDA error) and clears it.  The shipped library compiles the checks away and returns 0. */
+ * violation is redirected to element 0 and recorded).  In that build it synchronises the device, returns the bit mask of
+ * violations seen since the last call (bit: 0 pyramid, 1 V, 2 xy, 3 xz, 4 yz, 5 block table, 6 bitfield, 7 view, 8 pixel,
+ * 9 pool slot, 10 pool list; 0xffffffff: CUDA error) and clears it.  The shipped library compiles the checks away: there
+ * the call touches no CUDA state (no synchronisation) and returns 0. */
 unsigned int omerf_check_errors(void);
 
 #ifdef __cplusplus

@@ -309,7 +309,7 @@ def test_sparse_block_grid_matches_oracle_bake_and_dense_render(omerf, oracle, B
     with omerf.scene_create(sc, grid_block=B) as h:
         info = omerf.scene_info(h)
         assert info["grid_blocks_total"] == S.table.size and info["grid_blocks_allocated"] == S.n_alloc
-        assert info["grid_bytes"] == S.n_alloc * B ** 3 * 16 + S.table.size * 4     # 16-byte entries (texel pairs along z)
+        assert info["grid_bytes"] == S.n_alloc * B ** 3 * 16 + S.table.size * 4     # 16-byte entries (texel pairs along y)
         assert np.array_equal(omerf.block_table(h), S.table.ravel())
         rgb, ns = omerf.render(h, cams, 72, 56)
         torch.cuda.synchronize()
