@@ -525,12 +525,16 @@ constexpr int OMERF_ENDGAME_WARPS = 2;   // endgame starts when fewer than this 
 constexpr int OMERF_ENDGAME_BUSY = 32;   // in the endgame a warp takes a new tile only with at most this many rays in flight
 #define OMERF_PJ (OMERF_POOL / 32)
 
+// Entry OMERF_NO_RAY of every per-ray array is the slot of a lane that holds no ray: written once at kernel start
+// (an idle ray of view 0 with direction 0 and an empty index range), never listed, never written again.  A lane that
+// takes no ray in a swap step loads from it, so it reads nothing another lane may be writing back in the same step.
+#define OMERF_NO_RAY OMERF_POOL
 struct WarpPool {
-    uint32_t meta[OMERF_POOL]; // status (bits 0-1) | pyramid level (bits 2-6) | view (bits 8-31)
-    float d[3][OMERF_POOL];    // ray direction
-    int k[OMERF_POOL], k1[OMERF_POOL];
-    uint32_t Q[OMERF_POOL], n[OMERF_POOL], pix[OMERF_POOL];
-    float acc[7][OMERF_POOL];
+    uint32_t meta[OMERF_POOL + 1]; // status (bits 0-1) | pyramid level (bits 2-6) | view (bits 8-31)
+    float d[3][OMERF_POOL + 1];    // ray direction
+    int k[OMERF_POOL + 1], k1[OMERF_POOL + 1];
+    uint32_t Q[OMERF_POOL + 1], n[OMERF_POOL + 1], pix[OMERF_POOL + 1];
+    float acc[7][OMERF_POOL + 1];
     uint8_t list[OMERF_POOL]; // slots in the picked state, in slot order (phases other than traversal use the first 32)
 };
 
@@ -586,7 +590,7 @@ __device__ __forceinline__ void trav_load(const DevScene &sc, const WarpPool &P,
                                           const LaunchBounds &lb, OriginCache &oc, int slot, TravLane<SAMPLER> &L)
 {
     L.slot = slot;
-    const int s_ = slot < 0 ? 0 : chk(slot, OMERF_POOL, CHK_SLOT); // idle lanes read slot 0 and step nothing
+    const int s_ = slot < 0 ? OMERF_NO_RAY : chk(slot, OMERF_POOL, CHK_SLOT); // lanes without a ray read the constant slot and step nothing
     const uint32_t m = P.meta[s_];
     L.status = slot < 0 ? ST_IDLE : ST_TRAV;
     L.lvl = (int)((m >> 2) & 31u);
@@ -680,6 +684,16 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
 
 #pragma unroll
     for (int j = 0; j < OMERF_PJ; j++) P.meta[lane + 32 * j] = ST_IDLE;
+    if (lane == 0) {
+        P.meta[OMERF_NO_RAY] = pack_meta(ST_IDLE, 0, 0u);
+        P.k[OMERF_NO_RAY] = 0;
+        P.k1[OMERF_NO_RAY] = -1;
+        P.Q[OMERF_NO_RAY] = P.n[OMERF_NO_RAY] = P.pix[OMERF_NO_RAY] = 0u;
+#pragma unroll
+        for (int c = 0; c < 3; c++) P.d[c][OMERF_NO_RAY] = 0.0f;
+#pragma unroll
+        for (int c = 0; c < 7; c++) P.acc[c][OMERF_NO_RAY] = 0.0f;
+    }
     __syncwarp();
     bool more = true;
     const LaunchBounds lb = {(uint32_t)n_views, (unsigned long long)n_views * (unsigned long long)W * (unsigned long long)H};
@@ -787,7 +801,7 @@ omerf_march_kernel(const __grid_constant__ DevScene sc, const omerf_camera *__re
             Ray r;
             auto load_ray = [&](int s_new) {
                 sslot = s_new;
-                const int s_ = s_new < 0 ? 0 : chk(s_new, OMERF_POOL, CHK_SLOT);
+                const int s_ = s_new < 0 ? OMERF_NO_RAY : chk(s_new, OMERF_POOL, CHK_SLOT);
                 view = P.meta[s_] >> 8;
                 status = s_new < 0 ? ST_IDLE : ST_READY;
                 k = P.k[s_];
