@@ -295,7 +295,7 @@ extern "C" void omerf_scene_destroy(omerf_scene *s)
 static int ensure_cams(const omerf_scene *s, int n_views)
 {
     if (n_views <= s->cam_capacity) return OMERF_OK;
-    cudaDeviceSynchronize();
+    OMERF_CUDA(cudaDeviceSynchronize()); // kernels of earlier calls still read the ring that is about to be freed
     cudaFree(s->d_cams);
     if (s->h_cams) cudaFreeHost(s->h_cams);
     s->d_cams = nullptr;
@@ -387,7 +387,7 @@ extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *camer
     }
     uint64_t px = (uint64_t)n_views * W * H;
     if (px > s->scratch_pixels) {
-        cudaDeviceSynchronize();
+        OMERF_CUDA(cudaDeviceSynchronize());
         cudaFree(s->d_scratch_rgb);
         cudaFree(s->d_scratch_n);
         s->d_scratch_rgb = nullptr;

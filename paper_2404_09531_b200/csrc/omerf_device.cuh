@@ -31,8 +31,9 @@ __host__ __device__ constexpr inline int mlp_col(int j) // inverse: the column t
 }
 
 
-// Everything a render kernel needs, passed by value as a __grid_constant__ kernel parameter so that
-// scalars and the 883 MLP weights are read through the constant bank (no loads in the MLP).
+// Everything a render kernel needs, passed by value as a __grid_constant__ kernel parameter, so scalars, sizes and
+// pointers are read through the constant bank.  The deferred MLP's weights are not in here: they sit in global memory
+// in tensor-core fragment order (mlp_tab below) and are read with __ldg by mma_x3 / mlp_tiles (omerf_mlp.cuh).
 struct DevScene {
     float box[3];
     // occupancy plane P_o and its min/max pyramid ("2D max pooling")

@@ -11,7 +11,6 @@ __device__ __forceinline__ float sigmoid_fast(float x) { return __fdividef(1.0f,
 // Warp-cooperative: the 34 -> 16 -> 16 -> 3 network of 16 rays at a time as m16n8k8 tensor-core tiles.
 // tf32 operands are split hi + lo (3 mma per tile product), so the result keeps fp32-level accuracy; hidden
 // activations stay in registers (the C fragment of one layer is the A fragment of the next, see mlp_pack_kernel).
-#define OMERF_XS 44 // row stride of the staged input tile in floats: conflict-free A-fragment loads
 
 // x = hi + lo with hi = x truncated to tf32 (10 explicit mantissa bits) and lo = x - hi exactly; the tensor core
 // reads only the tf32 part of lo, which leaves a relative error of about 2^-21 in the product sum
@@ -67,28 +66,6 @@ __device__ __forceinline__ void mlp_encode_component(float d, float v[9])
     }
 }
 
-// All 40 columns of one row (padding columns 0), for kernels that stage rows through shared memory.
-template <bool FAST>
-__device__ __forceinline__ void mlp_input(const float acc[7], float dx, float dy, float dz, float in[40])
-{
-#pragma unroll
-    for (int i = 0; i < 40; i++) in[i] = 0.0f;
-#pragma unroll
-    for (int i = 0; i < 7; i++) in[mlp_col(i)] = acc[i];
-    const float d[3] = {dx, dy, dz};
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        float v[9];
-        mlp_encode_component<FAST>(d[c], v);
-        in[mlp_col(7 + c)] = v[0];
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-            in[mlp_col(10 + (3 * j + c) * 2)] = v[1 + 2 * j];
-            in[mlp_col(10 + (3 * j + c) * 2 + 1)] = v[2 + 2 * j];
-        }
-    }
-}
-
 // Evaluates G for 16 rows given as register fragments: v0 = this lane's ten layer-1 values of row g, v1 = of row g + 8
 // (column order above).  Returns this lane's share of the output C fragment: out[0], out[1] = row g cols 2t, 2t+1;
 // out[2], out[3] = row g+8 (pre-sigmoid; cols >= 3 unused).
@@ -138,21 +115,6 @@ __device__ __forceinline__ void mlp_tiles(const float2 *__restrict__ tab, const 
         split_tf32(fmaxf(c2[s][3], 0.0f), ahi[3], alo[3]);
         mma_x3(out, ahi, alo, tab, 14 + s, lane);
     }
-}
-
-// The same for 16 rows staged in shared memory (row stride OMERF_XS, all 40 columns written).
-__device__ __forceinline__ void mlp_half(const float2 *__restrict__ tab, const float *X, int lane, float out[4])
-{
-    const int g = lane >> 2, t = lane & 3;
-    float v0[10], v1[10];
-#pragma unroll
-    for (int s = 0; s < 5; s++) {
-        v0[2 * s] = X[g * OMERF_XS + 8 * s + t];
-        v1[2 * s] = X[(g + 8) * OMERF_XS + 8 * s + t];
-        v0[2 * s + 1] = X[g * OMERF_XS + 8 * s + t + 4];
-        v1[2 * s + 1] = X[(g + 8) * OMERF_XS + 8 * s + t + 4];
-    }
-    mlp_tiles(tab, v0, v1, lane, out);
 }
 
 } // namespace
