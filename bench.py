@@ -42,12 +42,26 @@ import synth  # noqa: E402
 BYTES_PER_SAMPLE = 168   # 20 distinct texels x 8 B (64 B grid + 96 B planes) + one (z_min, z_max) pair of 8 B
 BYTES_PER_PIXEL = 16     # 12 B rgb + 4 B sample count written
 TEXEL_BYTES_PER_SAMPLE = 160   # the distinct texels a sample needs: 20 x 8 B (fetched as 10 entries of 16 B)
-# Figures of ONE march-kernel launch on configs[1] from the committed `ncu --set full` capture (profiles/r02_march_kernel.md,
+# Figures of ONE march-kernel launch on configs[1] from the committed `ncu --set full` capture (profiles/r03_march_kernel.md,
 # which names the command and the commit it was taken at); cited constants, not measured by this run:
-NCU_CAPTURE = {"profile": "profiles/r02_march_kernel.md", "commit": "d5ceb67",
-               "dram_bytes": 177507072 + 18304512,          # dram__bytes_read.sum + dram__bytes_write.sum
-               "warp_instructions": 344547795,              # smsp__inst_executed.sum
-               "lanes_per_instruction": 28.23}              # smsp__thread_inst_executed_per_inst_executed.ratio
+NCU_CAPTURE = {"profile": "profiles/r03_march_kernel.md", "commit": "c81844a",
+               "csrc_sha16": "7c09636cf84d70bf",            # csrc_sha16() of the kernel sources that were captured
+               "dram_bytes": 177669632 + 18324736,          # dram__bytes_read.sum + dram__bytes_write.sum
+               "warp_instructions": 344740301,              # smsp__inst_executed.sum
+               "lanes_per_instruction": 28.22}              # smsp__thread_inst_executed_per_inst_executed.ratio
+
+
+def csrc_sha16() -> str:
+    """First 16 hex digits of the SHA-256 over the kernel sources (csrc/*.cu, *.cuh, in name order).  The cited ncu
+    figures above describe one build of the kernels: when the sources differ from the captured ones the bench line
+    carries null instead of a stale figure."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2404_09531_b200", "csrc")
+    for path in sorted(glob.glob(os.path.join(d, "*.cu")) + glob.glob(os.path.join(d, "*.cuh"))):
+        h.update(os.path.basename(path).encode() + b"\0" + open(path, "rb").read() + b"\0")
+    return h.hexdigest()[:16]
 
 
 def workload_name(cfg: int) -> str:
@@ -429,7 +443,10 @@ def run_ours(args):
         if not args.no_cpu_baseline:
             cpu = oracle_bounded(scene, cams, W, H, sampler=1 if args.sampler == "grid" else 0, budget_s=15.0, soft_eps=args.soft_eps, count_sectors=True)
         # figures of the committed ncu capture apply to the workload that was captured only
-        captured = cfg == 1 and args.sampler == "plane" and not (args.soft_eps or args.grid_block or args.lowz)
+        # and to the kernel sources that were captured: a later kernel change turns them into null, not into a stale figure
+        sha = csrc_sha16()
+        captured = (cfg == 1 and args.sampler == "plane" and not (args.soft_eps or args.grid_block or args.lowz)
+                    and sha == NCU_CAPTURE["csrc_sha16"])
         props = torch.cuda.get_device_properties(local)
         issue_peak = props.multi_processor_count * 128 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12   # Tlane-op/s
         line = {
@@ -470,8 +487,16 @@ def run_ours(args):
             line["roofline"] = {
                 "bound": "gather (L2/L1 gather rate, SURVEY 8(d); calibrated live, not HBM)", "kernel": "omerf_march_kernel",
                 "achieved": view0 * TEXEL_BYTES_PER_SAMPLE, "peak": ceil_gs * TEXEL_BYTES_PER_SAMPLE, "unit": "GB/s",
+                "unit_note": "requested texel bytes (samples x 160 B, served by L1/L2), NOT DRAM traffic: that is `traffic`",
+                "peak_kind": "calibrated gather replay",
                 "frac": view0 / ceil_gs, "traffic": NCU_CAPTURE["dram_bytes"] if captured else None,
-                "traffic_source": NCU_CAPTURE["profile"],
+                "traffic_source": NCU_CAPTURE["profile"] if captured else
+                f"none: kernel sources {sha} are not the captured ones ({NCU_CAPTURE['csrc_sha16']}) or another workload",
+                # the same launch against the measured HBM copy rate, in SURVEY 8(d)'s algorithmic bytes (168 B per sample
+                # + 16 B per pixel): the figure that does not move with the calibration
+                "hbm_frac": achieved / hbm, "hbm_achieved_gbs": achieved, "hbm_peak_gbs": hbm,
+                "hbm_peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650",
+                "algorithmic_bytes_per_launch": alg_bytes, "compulsory_bytes_oracle": None,
                 "peak_source": "omerf_gather_probe in this run: the frame's texel loads replayed with no arithmetic, one sample "
                                "per thread, frame order, L2 flushed",
                 "march_gsamples_s": view0, "ceiling_gsamples_s": ceil_gs, "launch_ms": march_ms,
@@ -503,6 +528,8 @@ def run_ours(args):
                 line["gather_vs_hbm"]["compulsory_bytes_oracle"] = cpu["compulsory_bytes"]
                 line["gather_vs_hbm"]["compulsory_sectors_oracle"] = cpu["sectors"]
                 line["gather_vs_hbm"]["compulsory_ms_at_peak"] = cpu["compulsory_bytes"] / (hbm * 1e9) * 1e3
+                if line["roofline"] is not None:
+                    line["roofline"]["compulsory_bytes_oracle"] = cpu["compulsory_bytes"]
         print(json.dumps(line))
     omerf.scene_destroy(h)
     if world > 1:

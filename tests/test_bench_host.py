@@ -161,3 +161,15 @@ def test_reference_arm_other_ranks_exit_quietly():
                           "--steps", "1", "--warmup", "0", "--gpus", "2"], capture_output=True, text=True, timeout=120,
                          cwd=ROOT, env=env)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_cited_ncu_figures_are_keyed_on_the_kernel_sources():
+    """bench.NCU_CAPTURE (DRAM traffic, instruction counts of one committed ncu capture) names the hash of the kernel
+    sources it was taken at; bench.py prints the figures only while csrc_sha16() equals it and null otherwise, so a
+    kernel change can never be reported beside a stale capture.  The hash is over content: stable across calls, 16 hex
+    digits, and the profile it cites exists."""
+    import bench
+    h = bench.csrc_sha16()
+    assert h == bench.csrc_sha16() and len(h) == 16 and int(h, 16) >= 0
+    assert len(bench.NCU_CAPTURE["csrc_sha16"]) == 16
+    assert os.path.exists(os.path.join(bench.ROOT, bench.NCU_CAPTURE["profile"]))
