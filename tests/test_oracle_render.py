@@ -308,3 +308,36 @@ def test_grid_sampler_superset_and_occupancy_ratio():
     frac = float(((hi - lo) * area).sum() / area.sum() / 4.0)
     dz = 4.0 / 32
     assert frac <= ratio <= frac + 2 * dz / 4.0 + 1e-9
+
+
+def test_render_pixels_equals_render_on_random_pixels_of_a_batch():
+    """orc_render_pixels (the oracle's entry for scattered (view, u, v) triples, used by the full-size GPU tests where a
+    whole batch would take minutes) is the same per-pixel routine as orc_render: on random pixels of a 3-view batch -
+    cameras of different pose, a non-square image, repeated and border pixels - counts, colours and the auxiliary
+    outputs are bit-identical to the whole-image render, in both the brute-force and the clipped loop.  A wrong view
+    stride, swapped (u, v) or a camera taken from the wrong row fails it (W != H, three different poses)."""
+    sc = synth.make_scene(0)
+    W, H = 45, 31
+    cams = np.stack([synth.look_at_camera((10.0, -14.0, 30.0), (32.0, 32.0, 8.0), W, H),
+                     synth.look_at_camera((70.0, 70.0, 25.0), (32.0, 32.0, 6.0), W, H),
+                     synth.look_at_camera((32.0, 32.0, 60.0), (32.0, 32.5, 0.0), W, H)])
+    O = oracle.OracleScene(sc)
+    rng = np.random.default_rng(11)
+    m = 400
+    vuv = np.stack([rng.integers(0, 3, m), rng.integers(0, W, m), rng.integers(0, H, m)], axis=1).astype(np.int32)
+    vuv[:6] = [[0, 0, 0], [2, W - 1, H - 1], [1, 0, H - 1], [1, W - 1, 0], [2, 5, 7], [2, 5, 7]]
+    for mode in ("clipped", "brute"):
+        full = O.render(cams, W, H, mode=mode, aux=True)
+        got = O.render_pixels(cams, W, H, vuv, mode=mode, aux=True)
+        idx = (vuv[:, 0], vuv[:, 2], vuv[:, 1])             # images are indexed [view][row v][column u]
+        assert full["nsamples"].sum() > 10000 and len({int(x) for x in got["nsamples"]}) > 5
+        assert np.array_equal(got["nsamples"], full["nsamples"][idx])
+        assert np.array_equal(got["rgb"], full["rgb"][idx])
+        for key in ("T_end", "sum_w", "Q"):
+            assert np.array_equal(got[key], full[key][idx]), key
+    # the three views really differ at the sampled pixels (else a wrong camera row would go unnoticed)
+    assert not np.array_equal(full["nsamples"][0], full["nsamples"][1])
+    with pytest.raises(ValueError):
+        O.render_pixels(cams, W, H, [[3, 0, 0]])            # view out of range
+    with pytest.raises(ValueError):
+        O.render_pixels(cams, W, H, [[0, 0, H]])            # row out of range (u = 0 .. W-1, v = 0 .. H-1)
