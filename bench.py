@@ -245,10 +245,12 @@ def gather_shares(plans, rank, my_rgb, my_n, n_views, H, W, device):
     return rgb, ns
 
 
-def run_partitioned(omerf, h, cams, W, H, prev_n, world, rank, steps, timed, barrier, stream):
+def run_partitioned(omerf, h, cams, W, H, prev_n, world, rank, steps, timed, barrier, stream, comm_device="cuda"):
     """Strong scaling: the batch partitioned across the ranks by the previous frame's sample counts, timed
     like the main region (L2 flushed, CUDA events, max over ranks); then the shares are gathered on rank 0 and compared
-    bit for bit with this rank's own full render."""
+    bit for bit with this rank's own full render.  comm_device: where the tensors that torch.distributed moves live -
+    "cuda" under NCCL (one rank per GPU), "cpu" under gloo (shares staged through host memory; lets several ranks share
+    one GPU, tests/test_gpu_partition.py)."""
     import torch
 
     from paper_2404_09531_b200 import partition
@@ -279,20 +281,23 @@ def run_partitioned(omerf, h, cams, W, H, prev_n, world, rank, steps, timed, bar
         my_rgb, my_n = full_rgb.view(n_views * H, W, 3)[r0:r1], full_n.view(n_views * H, W)[r0:r1]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    got = gather_shares(plans, rank, my_rgb, my_n, n_views, H, W, "cuda")
+    if comm_device != "cuda":
+        torch.cuda.synchronize()
+        my_rgb, my_n = my_rgb.to(comm_device), my_n.to(comm_device)
+    got = gather_shares(plans, rank, my_rgb, my_n, n_views, H, W, comm_device)
     e1.record(stream)
     barrier()
-    total = max_over_ranks([float(np.sum(ms))], world, "cuda")[0]
+    total = max_over_ranks([float(np.sum(ms))], world, comm_device)[0]
     out = {"scaling": "strong", "mode": plan.mode, "ms_per_step": total / steps, "frames_per_s": n_views * steps / (total / 1e3),
            "mpixels_s": n_views * W * H * steps / (total / 1e3) / 1e6, "cost_imbalance": plan.imbalance,
            "sample_imbalance": plan.sample_imbalance, "samples_per_rank": [p.samples for p in plans],
            "gather_to_rank0_ms": e0.elapsed_time(e1), "parallelism": f"scene replicated x{world}, batch partitioned by {plan.mode}"}
     if rank == 0:
-        ref_rgb = torch.empty_like(got[0])
-        ref_n = torch.empty_like(got[1])
+        ref_rgb = torch.empty(got[0].shape, dtype=got[0].dtype, device="cuda")
+        ref_n = torch.empty(got[1].shape, dtype=got[1].dtype, device="cuda")
         omerf.render(h, cams, W, H, ref_rgb, ref_n, stream=stream)
         torch.cuda.synchronize()
-        out["stitched_equals_single_rank"] = bool(torch.equal(got[1], ref_n) and torch.equal(got[0], ref_rgb))
+        out["stitched_equals_single_rank"] = bool(torch.equal(got[1], ref_n.to(comm_device)) and torch.equal(got[0], ref_rgb.to(comm_device)))
     return out
 
 
