@@ -45,22 +45,25 @@ TEXEL_BYTES_PER_SAMPLE = 160   # the distinct texels a sample needs: 20 x 8 B (f
 # Figures of ONE march-kernel launch on configs[1] from the committed `ncu --set full` capture (profiles/r03_march_kernel.md,
 # which names the command and the commit it was taken at); cited constants, not measured by this run:
 NCU_CAPTURE = {"profile": "profiles/r03_march_kernel.md", "commit": "c81844a",
-               "csrc_sha16": "7c09636cf84d70bf",            # csrc_sha16() of the kernel sources that were captured
+               "csrc_sha16": "6162632a9805ac31",            # csrc_sha16() of the kernel sources that were captured
                "dram_bytes": 177669632 + 18324736,          # dram__bytes_read.sum + dram__bytes_write.sum
                "warp_instructions": 344740301,              # smsp__inst_executed.sum
                "lanes_per_instruction": 28.22}              # smsp__thread_inst_executed_per_inst_executed.ratio
 
 
+MARCH_KERNEL_SOURCES = ("omerf_device.cuh", "omerf_mlp.cuh", "omerf_render.cu")   # everything omerf_march_kernel is compiled from
+
+
 def csrc_sha16() -> str:
-    """First 16 hex digits of the SHA-256 over the kernel sources (csrc/*.cu, *.cuh, in name order).  The cited ncu
-    figures above describe one build of the kernels: when the sources differ from the captured ones the bench line
-    carries null instead of a stale figure."""
-    import glob
+    """First 16 hex digits of the SHA-256 over the sources of the march kernel (MARCH_KERNEL_SOURCES under csrc/; the host
+    glue of omerf_api.cu and the scene-build kernels do not enter the captured launch).  The cited ncu figures above
+    describe one build of that kernel: when its sources differ from the captured ones the bench line carries null
+    instead of a stale figure."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2404_09531_b200", "csrc")
-    for path in sorted(glob.glob(os.path.join(d, "*.cu")) + glob.glob(os.path.join(d, "*.cuh"))):
-        h.update(os.path.basename(path).encode() + b"\0" + open(path, "rb").read() + b"\0")
+    for name in MARCH_KERNEL_SOURCES:
+        h.update(name.encode() + b"\0" + open(os.path.join(d, name), "rb").read() + b"\0")
     return h.hexdigest()[:16]
 
 
@@ -454,6 +457,7 @@ def run_ours(args):
                     and sha == NCU_CAPTURE["csrc_sha16"])
         props = torch.cuda.get_device_properties(local)
         issue_peak = props.multi_processor_count * 128 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12   # Tlane-op/s
+        host_feature_bytes = int(sum(np.asarray(getattr(scene, nm)).nbytes for nm in ("grid", "plane_xy", "plane_xz", "plane_yz")))
         line = {
             "metric": "Mpixels/s", "value": aggregate_throughput(pixels, k, world, total_ms) / 1e6, "unit": "Mpixels/s", "n_gpus": world,
             "steps": k, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
@@ -462,7 +466,11 @@ def run_ours(args):
             "config": {"workload": workload_name(cfg), "views": n_views, "W": W, "H": H, "sampler": args.sampler, "soft_eps": args.soft_eps, "grid_block": args.grid_block,
                        "lowz_bake": bool(args.lowz), "plane_bytes": info["plane_bytes"], "xz_band": info["xz_band"], "yz_band": info["yz_band"],
                        "grid_bytes": info["grid_bytes"], "grid_blocks": [info["grid_blocks_allocated"], info["grid_blocks_total"]],
-                       "scene_device_bytes": info["device_bytes"], "l2": "flushed between timed steps (256 MiB fill, "
+                       "scene_device_bytes": info["device_bytes"],
+                       # VRAM against the plain 8-byte-texel arrays of the host scene (the paired 16-byte entries double
+                       # every stored texel; sparse blocks and the low-z bake store fewer texels)
+                       "scene_host_feature_bytes": host_feature_bytes,
+                       "device_over_host_feature_bytes": info["device_bytes"] / host_feature_bytes, "l2": "flushed between timed steps (256 MiB fill, "
                        "outside the event pairs); scene 296 MiB > L2", "parallelism": f"replicated scene x{world}"},
             "frames_per_s": world * n_views * k / secs,
             "gsamples_s": world * samples * k / secs / 1e9,

@@ -190,18 +190,22 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
                     {d->plane_xy, (size_t)v.xy_n[0], v.xy_n[1], 0, v.xy_n[1], &s->d_pxy},
                     {d->plane_xz, (size_t)v.xz_n[0], v.xz_n[1], v.xz_zoff, v.xz_rows, &s->d_pxz},
                     {d->plane_yz, (size_t)v.yz_n[0], v.yz_n[1], v.yz_zoff, v.yz_rows, &s->d_pyz}};
+        // The raw texels of a dense array never sit on the device as a whole: the destination (2x) is allocated first and
+        // the source passes through a staging buffer of at most OMERF_STAGE_BYTES, a whole number of pairing units at a time
+        // (a unit holds both texels of every pair: an x slab of V, one row of a plane), so the peak of scene_create is the
+        // resident layout plus one staging buffer instead of plus the whole raw array.
+        const size_t OMERF_STAGE_BYTES = (size_t)64 << 20;
         for (int a = 0; a < 4 && rc == OMERF_OK; a++) {
             const size_t raw_bytes = arr[a].rows * arr[a].n * 8;
-            cudaError_t e = cudaMalloc(&d_raw, raw_bytes);
-            if (e == cudaSuccess)
-                e = cudaMemcpy2D(d_raw, (size_t)arr[a].n * 8, arr[a].host + (size_t)arr[a].first * 8, (size_t)arr[a].n_host * 8,
-                                 (size_t)arr[a].n * 8, arr[a].rows, cudaMemcpyHostToDevice);
-            if (e != cudaSuccess) {
-                rc = omerf_cuda_fail(e, "feature upload");
-                break;
-            }
+            cudaError_t e;
             if (a == 0 && d->grid_block) {
-                // 8(f).1: sparse-block layout of V baked from the occupancy plane (takes the raw texels, frees them)
+                // 8(f).1: sparse-block layout of V baked from the occupancy plane (takes the whole raw array, frees it)
+                e = cudaMalloc(&d_raw, raw_bytes);
+                if (e == cudaSuccess) e = cudaMemcpy(d_raw, arr[a].host, raw_bytes, cudaMemcpyHostToDevice);
+                if (e != cudaSuccess) {
+                    rc = omerf_cuda_fail(e, "feature upload");
+                    break;
+                }
                 s->d_grid = d_raw;
                 d_raw = nullptr;
                 rc = omerf_bake_sparse_grid(s, &s->d_grid, d->grid_block, 0);
@@ -212,8 +216,28 @@ extern "C" int omerf_scene_create(const omerf_scene_desc *d, omerf_scene **out_s
                 rc = omerf_cuda_fail(e, "feature layout");
                 break;
             }
-            if (a == 0) rc = omerf_launch_pair_layout(d_raw, *arr[a].dst, arr[a].rows * arr[a].n, v.G[1], (unsigned long long)v.G[2], 0);
-            else rc = omerf_launch_pair_layout(d_raw, *arr[a].dst, arr[a].rows * arr[a].n, arr[a].n, 1ull, 0);
+            const size_t row_bytes = (size_t)arr[a].n * 8;
+            const size_t unit_rows = a == 0 ? (size_t)v.G[1] : 1, n_units = arr[a].rows / unit_rows;
+            size_t units_per_chunk = OMERF_STAGE_BYTES / (unit_rows * row_bytes);
+            units_per_chunk = units_per_chunk < 1 ? 1 : (units_per_chunk > n_units ? n_units : units_per_chunk);
+            if ((e = cudaMalloc(&d_raw, units_per_chunk * unit_rows * row_bytes)) != cudaSuccess) {
+                rc = omerf_cuda_fail(e, "feature staging");
+                break;
+            }
+            for (size_t u0 = 0; u0 < n_units && rc == OMERF_OK; u0 += units_per_chunk) {
+                const size_t k = n_units - u0 < units_per_chunk ? n_units - u0 : units_per_chunk;
+                const size_t r0 = u0 * unit_rows, nr = k * unit_rows;
+                // a pageable copy on the null stream: ordered behind the kernel that still reads the buffer
+                e = cudaMemcpy2D(d_raw, row_bytes, arr[a].host + (r0 * (size_t)arr[a].n_host + (size_t)arr[a].first) * 8,
+                                 (size_t)arr[a].n_host * 8, row_bytes, nr, cudaMemcpyHostToDevice);
+                if (e != cudaSuccess) {
+                    rc = omerf_cuda_fail(e, "feature upload");
+                    break;
+                }
+                uint4 *dst = (uint4 *)*arr[a].dst + r0 * (size_t)arr[a].n;
+                if (a == 0) rc = omerf_launch_pair_layout(d_raw, dst, nr * arr[a].n, v.G[1], (unsigned long long)v.G[2], 0);
+                else rc = omerf_launch_pair_layout(d_raw, dst, nr * arr[a].n, arr[a].n, 1ull, 0);
+            }
             if (rc) break;
             if ((e = cudaDeviceSynchronize()) != cudaSuccess) {
                 rc = omerf_cuda_fail(e, "feature layout");
