@@ -5,6 +5,8 @@ The whole batch is rendered on the GPU in one call.  WHOLE frames are compared w
 samplers, the pitch-20 and pitch-80 views of configs[2], one 2160p view of configs[3] and one low-altitude view; for the
 remaining views of a batch the oracle computes sampled pixels one by one (a random subset plus whole rows).  Properties
 that hold at any size are checked on the full outputs."""
+import os
+
 import numpy as np
 import pytest
 
@@ -12,6 +14,13 @@ import synth
 
 pytestmark = pytest.mark.gpu
 RGB_TOL = 2e-3
+# OMERF_FULL_BATCH=1 (one-off evidence run, minutes of oracle time; profiles/r03_full_batch_parity.md): EVERY view of
+# the batches of configs[2], [3] and [5] is compared whole, element by element, and a line per view is printed (-s).
+FULL_BATCH = os.environ.get("OMERF_FULL_BATCH", "0") not in ("", "0")
+
+
+def _whole(n_views, subset):
+    return list(range(n_views)) if FULL_BATCH else list(subset)
 
 
 @pytest.fixture(scope="module")
@@ -46,6 +55,9 @@ def _check_whole_views(rgb, ns, scene, cams, W, H, sampler, views, **okw):
         err = np.abs(rgb[v].astype(np.float64) - ref["rgb"][0]).max()
         assert err <= RGB_TOL, f"view {v}: max |dRGB| = {err}"
         assert ref["nsamples"].sum() > 0
+        if FULL_BATCH:
+            print(f"FULL_BATCH view {v} of {len(cams)}: {W}x{H} pixels, {int(ref['nsamples'].sum())} samples, "
+                  f"count mismatches 0, max|dRGB| {err:.2e}", flush=True)
 
 
 def _check_sampled(omerf, scene, cams, W, H, sampler, n_random, rows, seed, whole_views=()):
@@ -85,7 +97,7 @@ def test_config2_batch_of_16(omerf, city):
     cams = synth.make_cameras(2)
     W, H = synth.config_resolution(2)
     # whole frames for the flattest (pitch 20 deg, extrapolated near-horizontal) and the steepest (80 deg) view
-    rgb, ns = _check_sampled(omerf, city, cams, W, H, 0, 60000, [3, 540], seed=102, whole_views=[0, 15])
+    rgb, ns = _check_sampled(omerf, city, cams, W, H, 0, 60000, [3, 540], seed=102, whole_views=_whole(16, [0, 15]))
     per_view = ns.reshape(16, -1).sum(axis=1)
     assert np.all(per_view > 0)
 
@@ -111,14 +123,14 @@ def test_config3_large_scene(omerf):
     scene = synth.make_scene(3)
     cams = synth.make_cameras(3)
     W, H = synth.config_resolution(3)
-    _check_sampled(omerf, scene, cams, W, H, 0, 40000, [1080], seed=103, whole_views=[3])
+    _check_sampled(omerf, scene, cams, W, H, 0, 40000, [1080], seed=103, whole_views=_whole(8, [3]))
 
 
 def test_config5_low_altitude_cameras(omerf, city):
     """cameras inside the box, in streets and inside the slab (rays start occupied)."""
     cams = synth.make_cameras(5)
     W, H = synth.config_resolution(5)
-    rgb, ns = _check_sampled(omerf, city, cams, W, H, 0, 30000, [200, 700], seed=105, whole_views=[1])  # inside the slab
+    rgb, ns = _check_sampled(omerf, city, cams, W, H, 0, 30000, [200, 700], seed=105, whole_views=_whole(cams.shape[0], [1]))  # [1]: inside the slab
     per_view = ns.reshape(cams.shape[0], -1).sum(axis=1)
     assert np.all(per_view > 0)
 
