@@ -132,6 +132,23 @@ int omerf_render_tiles(const omerf_scene *scene, const omerf_camera *cameras /*H
 int omerf_render_host(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W,
                       int H, float *out_rgb /*HOST*/, uint32_t *out_nsamples /*HOST*/, void *stream);
 
+/* Pipelined form of omerf_render_host (SURVEY.md 8(b) "Async"): the same banded render + copy-back, but the call returns
+ * as soon as the work is enqueued, so the copy-back of frame N overlaps the render of frame N + 1 (a frame's 16 B per pixel
+ * take longer to cross PCIe than to render).  Two scene-owned scratch sets alternate between calls; a set is rendered
+ * into again only after its previous copy-back has finished (event-ordered on the device, the host never blocks).
+ *   out_rgb / out_nsamples  HOST, as omerf_render_host.  They belong to the library from this call until omerf_wait
+ *                           returns: do not read, reuse or free them before.  PINNED memory is needed for the overlap; with
+ *                           pageable buffers the result is the same but cudaMemcpyAsync blocks the call.
+ *   cameras                 HOST, read before the call returns.
+ * Calls on one scene complete in call order.  The first call with more pixels than any async call before it (re)allocates
+ * both scratch sets (cudaDeviceSynchronize + cudaMalloc inside the call).  Same threading rule as omerf_render; use one
+ * `stream` for consecutive calls, or order the streams yourself.
+ * omerf_wait blocks the host until every omerf_render_host_async call made on this scene so far has delivered its host
+ * buffers (OMERF_OK also when there was none). */
+int omerf_render_host_async(const omerf_scene *scene, const omerf_camera *cameras /*HOST*/, int n_views, int W, int H,
+                            float *out_rgb /*HOST*/, uint32_t *out_nsamples /*HOST*/, void *stream);
+int omerf_wait(const omerf_scene *scene);
+
 /* omerf_render for callers that must not allocate.  omerf_render keeps its per-call scratch - the device copy of the
  * cameras and the head of the march kernel's work queue - in a ring it (re)allocates with cudaMalloc / cudaMallocHost
  * behind a cudaDeviceSynchronize whenever a call brings more views than any call before it.  That is wrong for two kinds

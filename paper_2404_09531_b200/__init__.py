@@ -25,9 +25,11 @@ from .binding import (  # noqa: F401
     pyramid_level,
     render,
     render_host,
+    render_host_async,
     render_static,
     render_tiles,
     scene_create,
     scene_destroy,
     scene_info,
+    wait,
 )

@@ -23,7 +23,7 @@ SAMPLER_GRID = 1
 STATIC_MAX_VIEWS = 32           # OMERF_STATIC_MAX_VIEWS of include/omerf.h
 
 EXPORTS = (
-    "omerf_scene_create", "omerf_render", "omerf_render_tiles", "omerf_render_host", "omerf_render_static", "omerf_gather_probe", "omerf_mlp_smoothness", "omerf_heatmap",
+    "omerf_scene_create", "omerf_render", "omerf_render_tiles", "omerf_render_host", "omerf_render_host_async", "omerf_wait", "omerf_render_static", "omerf_gather_probe", "omerf_mlp_smoothness", "omerf_heatmap",
     "omerf_last_launch_count",
     "omerf_scene_get_info", "omerf_scene_get_pyramid_level", "omerf_scene_get_bitfield", "omerf_scene_get_block_table",
     "omerf_scene_destroy", "omerf_last_error", "omerf_version", "omerf_check_errors",
@@ -80,6 +80,8 @@ def load_library() -> C.CDLL:
     L.omerf_render.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
     L.omerf_render_host.argtypes = L.omerf_render.argtypes
     L.omerf_render_static.argtypes = L.omerf_render.argtypes
+    L.omerf_render_host_async.argtypes = L.omerf_render.argtypes
+    L.omerf_wait.argtypes = [C.c_void_p]
     L.omerf_render_tiles.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_uint32,
                                      C.c_uint32, C.c_void_p]
     L.omerf_gather_probe.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
@@ -269,6 +271,30 @@ def render_host(h: SceneHandle, cameras, W: int, H: int, out_rgb=None, out_nsamp
     _check(load_library().omerf_render_host(h.ptr, cams.ctypes.data, n, W, H, hptr(out_rgb, n * H * W * 12),
                                             hptr(out_nsamples, n * H * W * 4), st.cuda_stream), "omerf_render_host")
     return out_rgb, out_nsamples
+
+
+def render_host_async(h: SceneHandle, cameras, W: int, H: int, out_rgb, out_nsamples, stream=None):
+    """omerf_render_host_async: enqueue a render whose HOST outputs (pinned CPU torch tensors, or numpy arrays over
+    pinned memory) are delivered in the background; they belong to the library until wait(h) returns."""
+    import torch
+    cams = _cams(cameras)
+    n = cams.shape[0]
+
+    def hptr(a, nbytes):
+        if isinstance(a, np.ndarray):
+            assert a.flags["C_CONTIGUOUS"] and a.nbytes == nbytes
+            return a.ctypes.data
+        assert (not a.is_cuda) and a.is_contiguous() and a.numel() * a.element_size() == nbytes
+        return a.data_ptr()
+
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(load_library().omerf_render_host_async(h.ptr, cams.ctypes.data, n, W, H, hptr(out_rgb, n * H * W * 12),
+                                                  hptr(out_nsamples, n * H * W * 4), st.cuda_stream), "omerf_render_host_async")
+
+
+def wait(h: SceneHandle):
+    """omerf_wait: block until every render_host_async call on this scene has delivered its host buffers."""
+    _check(load_library().omerf_wait(h.ptr), "omerf_wait")
 
 
 def gather_probe(h: SceneHandle, camera, W: int, H: int, repeats: int = 10, flush_l2: bool = True) -> dict:

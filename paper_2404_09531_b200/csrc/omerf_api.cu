@@ -59,6 +59,11 @@ static void free_scene(omerf_scene *s)
     cudaFree(s->d_tile_counter);
     cudaFree(s->d_scratch_rgb);
     cudaFree(s->d_scratch_n);
+    for (int i = 0; i < 2; i++) {
+        cudaFree(s->d_async_rgb[i]);
+        cudaFree(s->d_async_n[i]);
+        if (s->async_done[i]) cudaEventDestroy(s->async_done[i]);
+    }
     if (s->h_cams) cudaFreeHost(s->h_cams);
     if (s->copy_stream) {
         cudaStreamDestroy(s->copy_stream);
@@ -456,6 +461,84 @@ extern "C" int omerf_render_host(const omerf_scene *s, const omerf_camera *camer
     }
     OMERF_CUDA(cudaStreamSynchronize(s->copy_stream));
     OMERF_CUDA(cudaStreamSynchronize(st));
+    return OMERF_OK;
+}
+
+// Pipelined form: the loop of omerf_render_host into one of two scratch sets, without the final synchronisation.  The render
+// stream waits (on the device) for the previous copy-back out of the set it is about to overwrite; the copy stream runs the
+// copies of consecutive calls in call order, so waiting for it (omerf_wait) is waiting for every host buffer.
+extern "C" int omerf_render_host_async(const omerf_scene *s, const omerf_camera *cameras, int n_views, int W, int H,
+                                       float *out_rgb, uint32_t *out_nsamples, void *stream)
+{
+    if (!s || !cameras || !out_rgb || !out_nsamples) return invalid("null scene/cameras/output");
+    if (n_views < 0 || W <= 0 || H <= 0) return invalid("n_views >= 0, W > 0, H > 0 required");
+    if (n_views == 0) return OMERF_OK;
+    {
+        int rc = check_device(s);
+        if (rc) return rc;
+    }
+    const uint64_t px = (uint64_t)n_views * W * H;
+    if (px > s->async_pixels) {
+        OMERF_CUDA(cudaDeviceSynchronize());
+        s->async_pixels = 0;
+        for (int i = 0; i < 2; i++) {
+            cudaFree(s->d_async_rgb[i]);
+            cudaFree(s->d_async_n[i]);
+            s->d_async_rgb[i] = nullptr;
+            s->d_async_n[i] = nullptr;
+        }
+        for (int i = 0; i < 2; i++) {
+            OMERF_CUDA(cudaMalloc((void **)&s->d_async_rgb[i], px * 3 * sizeof(float)));
+            OMERF_CUDA(cudaMalloc((void **)&s->d_async_n[i], px * sizeof(uint32_t)));
+            if (!s->async_done[i]) OMERF_CUDA(cudaEventCreateWithFlags(&s->async_done[i], cudaEventDisableTiming));
+        }
+        s->async_pixels = px;
+    }
+    if (!s->copy_stream) {
+        OMERF_CUDA(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 16; i++) OMERF_CUDA(cudaEventCreateWithFlags(&s->band_event[i], cudaEventDisableTiming));
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const int set = (int)(s->async_index++ & 1ull);
+    float *d_rgb = s->d_async_rgb[set];
+    uint32_t *d_n = s->d_async_n[set];
+    OMERF_CUDA(cudaStreamWaitEvent(st, s->async_done[set], 0)); // a never-recorded event counts as finished
+    const unsigned int tiles_x = (unsigned int)((W + 7) / 8), tiles_y = (unsigned int)((H + 3) / 4);
+    const uint64_t tile_rows = (uint64_t)n_views * tiles_y, out_bytes = px * 16;
+    // Bands only shorten the fill of the pipeline (the first copy starts before the whole batch is rendered); in steady state
+    // the overlap comes from the next call.  Every band is a launch with a fixed cost of about 0.08 ms, so bands are coarser
+    // than omerf_render_host's: at least 32 MiB of output each (one 1080p frame: a single launch, 0.71 -> 0.61 ms per frame).
+    int bands = (int)(out_bytes / ((uint64_t)32 << 20));
+    bands = bands < 1 ? 1 : (bands > 16 ? 16 : bands);
+    if ((uint64_t)bands > tile_rows) bands = (int)tile_rows;
+    auto pixel_row = [&](uint64_t R) {
+        const uint64_t view = R / tiles_y, ty = R % tiles_y;
+        const uint64_t v = ty * 4 < (uint64_t)H ? ty * 4 : (uint64_t)H;
+        return view * (uint64_t)H + v;
+    };
+    s->last_launches = 0;
+    int slot = -1;
+    for (int b = 0; b < bands; b++) {
+        const uint64_t R0 = tile_rows * b / bands, R1 = tile_rows * (b + 1) / bands;
+        int rc = render_impl(s, cameras, n_views, W, H, d_rgb, d_n, stream, (unsigned int)(R0 * tiles_x), (unsigned int)(R1 * tiles_x), &slot);
+        if (rc) return rc;
+        // a band event may be re-recorded by the next call while this wait is pending: a wait refers to the record before it
+        OMERF_CUDA(cudaEventRecord(s->band_event[b], st));
+        OMERF_CUDA(cudaStreamWaitEvent(s->copy_stream, s->band_event[b], 0));
+        const uint64_t r0 = pixel_row(R0), r1 = R1 == tile_rows ? (uint64_t)n_views * H : pixel_row(R1);
+        OMERF_CUDA(cudaMemcpyAsync(out_rgb + r0 * W * 3, d_rgb + r0 * W * 3, (r1 - r0) * W * 3 * sizeof(float), cudaMemcpyDeviceToHost,
+                                   s->copy_stream));
+        OMERF_CUDA(cudaMemcpyAsync(out_nsamples + r0 * W, d_n + r0 * W, (r1 - r0) * W * sizeof(uint32_t), cudaMemcpyDeviceToHost,
+                                   s->copy_stream));
+    }
+    OMERF_CUDA(cudaEventRecord(s->async_done[set], s->copy_stream));
+    return OMERF_OK;
+}
+
+extern "C" int omerf_wait(const omerf_scene *s)
+{
+    if (!s) return invalid("null scene");
+    if (s->copy_stream) OMERF_CUDA(cudaStreamSynchronize(s->copy_stream));
     return OMERF_OK;
 }
 

@@ -111,6 +111,12 @@ struct omerf_scene {
     mutable int last_launches;
     mutable cudaStream_t copy_stream;  // omerf_render_host: copies a band back while the next one renders
     mutable cudaEvent_t band_event[16];
+    // omerf_render_host_async: two scratch sets used in turn; async_done[i] = the copy-back out of set i has finished
+    mutable float *d_async_rgb[2];
+    mutable uint32_t *d_async_n[2];
+    mutable uint64_t async_pixels;
+    mutable cudaEvent_t async_done[2];
+    mutable unsigned long long async_index;
     unsigned int *d_tile_counter;     // work-queue heads of the persistent march kernel, one per camera-ring slot
     int persistent_blocks;            // resident CTAs of the march kernel (SMs x occupancy)
 };

@@ -153,6 +153,42 @@ def test_config1_sparse_block_grid(omerf, city):
     _check_whole_views(rgb, ns, city, cams, W, H, 0, [0])        # the whole frame equals the DENSE oracle's
 
 
+def test_render_host_async_frames_in_flight_are_bit_identical(omerf, city):
+    """omerf_render_host_async + omerf_wait: five 1080p frames of an orbit are enqueued back to back (two scratch sets in
+    turn, so frame 2 must wait on the device for frame 0's copy-back, and so on), each into its own pinned host buffers;
+    after one omerf_wait every host image equals the device path's bit for bit.  Then a 2-view batch (the scratch
+    regrows), a ragged small frame, and a wait with nothing pending."""
+    import torch
+    W, H = synth.config_resolution(1)
+    orbit = synth.orbit_cameras(1, 5)
+
+    def pinned(n, w_, h_):
+        r = torch.full((n, h_, w_, 3), -1.0, dtype=torch.float32).pin_memory()
+        c = torch.full((n, h_, w_), -1, dtype=torch.int32).pin_memory()
+        return r, c
+
+    with omerf.scene_create(city) as h:
+        omerf.wait(h)                                           # nothing pending: returns at once
+        refs = []
+        for i in range(5):
+            rgb, ns = omerf.render(h, orbit[i:i + 1], W, H)
+            refs.append((rgb.cpu(), ns.cpu()))
+        bufs = [pinned(1, W, H) for _ in range(5)]
+        for i in range(5):
+            omerf.render_host_async(h, orbit[i:i + 1], W, H, *bufs[i])
+        omerf.wait(h)
+        for i in range(5):
+            assert torch.equal(bufs[i][1], refs[i][1]), f"frame {i}: sample counts differ"
+            assert torch.equal(bufs[i][0], refs[i][0]), f"frame {i}: colours differ"
+        assert not torch.equal(refs[0][1], refs[1][1])          # the frames really differ
+        for cams, w_, h_ in ((orbit[:2], W, H), (orbit[3:4], 61, 45)):
+            rgb, ns = omerf.render(h, cams, w_, h_)
+            b = pinned(cams.shape[0], w_, h_)
+            omerf.render_host_async(h, cams, w_, h_, *b)
+            omerf.wait(h)
+            assert torch.equal(b[1], ns.cpu()) and torch.equal(b[0], rgb.cpu())
+
+
 def test_render_host_banded_copy_is_bit_identical(omerf, city):
     """omerf_render_host renders in bands and copies a band back while the next one renders: the host images must
     equal the device-output path bit for bit, for one view (2 bands), several views and a ragged image height."""
