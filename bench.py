@@ -45,11 +45,11 @@ ORACLE_BLOCK = 128            # rows per oracle call of the cpu_baseline sample 
 TEXEL_BYTES_PER_SAMPLE = 160   # the distinct texels a sample needs: 20 x 8 B (fetched as 10 entries of 16 B)
 # Figures of ONE march-kernel launch on configs[1] from the committed `ncu --set full` capture (profiles/r03_march_kernel.md,
 # which names the command and the commit it was taken at); cited constants, not measured by this run:
-NCU_CAPTURE = {"profile": "profiles/r03_march_kernel.md", "commit": "c81844a",
-               "csrc_sha16": "6162632a9805ac31",            # csrc_sha16() of the kernel sources that were captured
-               "dram_bytes": 177669632 + 18324736,          # dram__bytes_read.sum + dram__bytes_write.sum
-               "warp_instructions": 344740301,              # smsp__inst_executed.sum
-               "lanes_per_instruction": 28.22}              # smsp__thread_inst_executed_per_inst_executed.ratio
+NCU_CAPTURE = {"profile": "profiles/r03_march_kernel.md", "commit": "9ea54f3",
+               "csrc_sha16": "bbd2ed3859f8b911",            # csrc_sha16() of the kernel sources that were captured
+               "dram_bytes": 177942272 + 19446528,          # dram__bytes_read.sum + dram__bytes_write.sum
+               "warp_instructions": 344585510,              # smsp__inst_executed.sum
+               "lanes_per_instruction": 28.23}              # smsp__thread_inst_executed_per_inst_executed.ratio
 
 
 MARCH_KERNEL_SOURCES = ("omerf_device.cuh", "omerf_mlp.cuh", "omerf_render.cu")   # everything omerf_march_kernel is compiled from
